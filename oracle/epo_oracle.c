@@ -1,0 +1,483 @@
+/*
+ * epo_oracle.c -- plain, slow, obviously-correct CPU oracle for the EPO hot path.
+ *
+ * THIS IS TEST INFRASTRUCTURE.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may call it.  It shares no code, header, table or helper with the CUDA
+ * library under paper_2607_00579_b200/ and neither includes the other.
+ *
+ * Everything is double precision on the caller's fp32 inputs (the paper fixes FP32 for the geometry,
+ * PAPER.md:121; double here makes the oracle the "exact" side of every tolerance in BASELINE.json).
+ * There is no blocking, fusion or re-ordering beyond what the cited passage states.  OpenMP is used
+ * over PAIRS only (each pair is an independent unit, Eq. 6); per-pair results are stored
+ * and then reduced serially in ascending pair order, so results do not depend on the thread count.
+ *
+ * Conventions:
+ *   - poses are world-to-camera T = [R|t], x_cam = R X_w + t   ("P=[R|t]")
+ *   - K = (fx, fy, cx, cy); Z is z-depth (the homogeneous pixel is scaled by Z)
+ *   - pixel (u,v) is the sample position; DTF[v][u] is the field value AT (u,v)        (reading S2)
+ *   - pose perturbation: T <- Exp(eps) T, eps = (v, w), translation part first          (reading S9)
+ *
+ * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): Z0..Z10 of SURVEY.md §8(c).  Numerical VALUES of
+ * the loss/gradient on realistic scenes are "parity unpinned" beyond those checks (nothing in the
+ * paper prints one).
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC -o liboracle.so epo_oracle.c -lm
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_PI 3.14159265358979323846
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+  omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
+/* =================================================================================================
+ * O1  Edge list  ("p in E_i"; "sub-sampled to <= E_max points / image")
+ * Raster order (v ascending, then u ascending).  A pixel is kept iff edges != 0 and its depth is
+ * finite and > z_min (reading S7).  If e_max > 0 and n > e_max keep entries floor(j*n/e_max) (S6).
+ * Returns the count; uv = [count][2] (u, v), z = [count].
+ * ================================================================================================= */
+int orc_edge_list(int W, int H, const uint8_t* edges, const float* depth, double z_min, int e_max,
+                  uint16_t* uv, float* z) {
+  int n = 0;
+  for (int v = 0; v < H; ++v)
+    for (int u = 0; u < W; ++u) {
+      float d = depth[(size_t)v * W + u];
+      if (edges[(size_t)v * W + u] != 0 && isfinite(d) && (double)d > z_min) {
+        uv[2 * n] = (uint16_t)u; uv[2 * n + 1] = (uint16_t)v; z[n] = d; ++n;
+      }
+    }
+  if (e_max > 0 && n > e_max) {
+    for (int j = 0; j < e_max; ++j) {
+      int k = (int)(((int64_t)j * n) / e_max);
+      uv[2 * j] = uv[2 * k]; uv[2 * j + 1] = uv[2 * k + 1]; z[j] = z[k];
+    }
+    n = e_max;
+  }
+  return n;
+}
+
+/* =================================================================================================
+ * O2  Exact Euclidean distance transform  ("each pixel encodes the Euclidean distance to
+ * the nearest edge"; "exact L2 distance transform [14]").
+ * Distances between pixel centres, in pixels; an edge pixel has DTF 0; an image without edge pixels
+ * has DTF = W+H everywhere (reading S8).  d2 is an exact integer; DTF = (float)sqrt((double)d2), which
+ * is the correctly rounded fp32 square root because d2 < 2^24 is exact in both formats and rounding
+ * the double root to float cannot double-round here: for a non-square integer n < 2^24 the root is at
+ * least 2^-50 (relative) away from every fp32 rounding midpoint m (n - m^2 is a non-zero multiple of
+ * 2^(2e-48)), far more than the 2^-53 error of the double root.
+ * ================================================================================================= */
+void orc_edt_brute(int W, int H, const uint8_t* edges, float* dtf) { /* the definition, O(n^2) */
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      int64_t best = (int64_t)(W + H) * (W + H);
+      for (int yy = 0; yy < H; ++yy)
+        for (int xx = 0; xx < W; ++xx)
+          if (edges[(size_t)yy * W + xx]) {
+            int64_t d2 = (int64_t)(x - xx) * (x - xx) + (int64_t)(y - yy) * (y - yy);
+            if (d2 < best) best = d2;
+          }
+      dtf[(size_t)y * W + x] = (float)sqrt((double)best);
+    }
+}
+
+/* Separable form: g[y][x] = min_{x' edge in row y} |x-x'| (W+H if the row has none);
+ * d2[y][x] = min_{y'} g[y'][x]^2 + (y-y')^2, every minimum taken by exhaustive search in integers. */
+void orc_edt_separable(int W, int H, const uint8_t* edges, float* dtf) {
+  int32_t* g = (int32_t*)malloc((size_t)W * H * sizeof(int32_t));
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      int best = W + H;
+      for (int xx = 0; xx < W; ++xx)
+        if (edges[(size_t)y * W + xx]) { int d = abs(x - xx); if (d < best) best = d; }
+      g[(size_t)y * W + x] = best;
+    }
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      int64_t best = INT64_MAX;
+      for (int yy = 0; yy < H; ++yy) {
+        int64_t gg = g[(size_t)yy * W + x];
+        int64_t d2 = gg * gg + (int64_t)(y - yy) * (y - yy);
+        if (d2 < best) best = d2;
+      }
+      dtf[(size_t)y * W + x] = (float)sqrt((double)best);
+    }
+  free(g);
+}
+
+void orc_edt_batch(int N, int W, int H, const uint8_t* edges, float* dtf) {
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int i = 0; i < N; ++i)
+    orc_edt_separable(W, H, edges + (size_t)i * W * H, dtf + (size_t)i * W * H);
+}
+
+/* fp16 variant of the field (BASELINE.json config 4): round-to-nearest-even of the fp32 value to IEEE
+ * binary16, returned widened back to float.  Written out on the bits. */
+float orc_round_to_half(float f) {
+  uint32_t x; memcpy(&x, &f, 4);
+  uint32_t sign = x & 0x80000000u, mag = x & 0x7fffffffu;
+  float out;
+  if (mag >= 0x7f800000u) return f;                       /* inf / nan unchanged */
+  if (mag >= 0x477ff000u) { mag = 0x7f800000u; }          /* >= 65520 rounds to inf */
+  else if (mag < 0x38800000u) {                           /* below 2^-14: half subnormal, spacing 2^-24 */
+    float a; memcpy(&a, &mag, 4);
+    double q = nearbyint((double)a * 16777216.0);         /* ties-to-even in the default rounding mode */
+    a = (float)(q / 16777216.0); memcpy(&mag, &a, 4);
+  } else {                                                /* normal: keep 10 mantissa bits */
+    uint32_t rem = mag & 0x1fffu, base = mag & ~0x1fffu;
+    if (rem > 0x1000u || (rem == 0x1000u && (base & 0x2000u))) base += 0x2000u;
+    mag = base;
+  }
+  mag |= sign; memcpy(&out, &mag, 4);
+  return out;
+}
+void orc_round_field_to_half(int64_t n, const float* in, float* out) {
+  for (int64_t i = 0; i < n; ++i) out[i] = orc_round_to_half(in[i]);
+}
+
+/* =================================================================================================
+ * O3  Canonical pair order  (PAPER.md:70 the viewgraph is the pair set; PAPER.md:478-483 batching)
+ * ascending (target, source), stable; duplicates kept.  perm[k] = index in the user list of the
+ * k-th canonical pair.  Plain bottom-up stable merge sort on the 64-bit key (t, s).
+ * ================================================================================================= */
+void orc_canonical_pairs(int64_t P, const int32_t* pairs, int32_t* sorted, int32_t* perm) {
+  for (int64_t k = 0; k < P; ++k) perm[k] = (int32_t)k;
+  int32_t* tmp = (int32_t*)malloc((size_t)P * sizeof(int32_t));
+  for (int64_t width = 1; width < P; width *= 2) {
+    for (int64_t lo = 0; lo < P; lo += 2 * width) {
+      int64_t mid = lo + width < P ? lo + width : P, hi = lo + 2 * width < P ? lo + 2 * width : P;
+      int64_t i = lo, j = mid, o = lo;
+      while (i < mid && j < hi) {
+        int32_t a = perm[i], b = perm[j];
+        int64_t ka = ((int64_t)pairs[2 * a + 1] << 32) | (uint32_t)pairs[2 * a];
+        int64_t kb = ((int64_t)pairs[2 * b + 1] << 32) | (uint32_t)pairs[2 * b];
+        if (kb < ka) tmp[o++] = perm[j++]; else tmp[o++] = perm[i++];   /* ties take the left: stable */
+      }
+      while (i < mid) tmp[o++] = perm[i++];
+      while (j < hi) tmp[o++] = perm[j++];
+    }
+    memcpy(perm, tmp, (size_t)P * sizeof(int32_t));
+  }
+  free(tmp);
+  for (int64_t k = 0; k < P; ++k) { sorted[2 * k] = pairs[2 * perm[k]]; sorted[2 * k + 1] = pairs[2 * perm[k] + 1]; }
+}
+
+/* =================================================================================================
+ * Projective function pi, split as the paper splits it (Eq. 2 / Eq. 8)
+ * ================================================================================================= */
+/* camera-frame point of pixel (u,v) with z-depth Z:  K^-1 [u,v,1]^T Z */
+void orc_backproject_cam(const double K[4], double u, double v, double Z, double x[3]) {
+  x[0] = Z * ((u - K[2]) / K[0]); x[1] = Z * ((v - K[3]) / K[1]); x[2] = Z;
+}
+/* world point X = P^-1 x_cam = R^T (x_cam - t) */
+void orc_cam_to_world(const double T[12], const double x[3], double X[3]) {
+  double d[3] = { x[0] - T[3], x[1] - T[7], x[2] - T[11] };
+  for (int i = 0; i < 3; ++i) X[i] = T[i] * d[0] + T[4 + i] * d[1] + T[8 + i] * d[2];
+}
+/* x_cam = R X + t */
+void orc_world_to_cam(const double T[12], const double X[3], double x[3]) {
+  for (int i = 0; i < 3; ++i) x[i] = T[4 * i] * X[0] + T[4 * i + 1] * X[1] + T[4 * i + 2] * X[2] + T[4 * i + 3];
+}
+/* pixel = (fx X/Z + cx, fy Y/Z + cy) */
+void orc_project_px(const double K[4], const double x[3], double px[2]) {
+  px[0] = K[0] * x[0] / x[2] + K[2]; px[1] = K[1] * x[1] / x[2] + K[3];
+}
+/* relative pose T_ts = T_t T_s^-1:  R_ts = R_t R_s^T,  t_ts = t_t - R_ts t_s */
+void orc_relative_pose(const double Ts[12], const double Tt[12], double Tts[12]) {
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j)
+      Tts[4 * i + j] = Tt[4 * i] * Ts[4 * j] + Tt[4 * i + 1] * Ts[4 * j + 1] + Tt[4 * i + 2] * Ts[4 * j + 2];
+  for (int i = 0; i < 3; ++i)
+    Tts[4 * i + 3] = Tt[4 * i + 3] - (Tts[4 * i] * Ts[3] + Tts[4 * i + 1] * Ts[7] + Tts[4 * i + 2] * Ts[11]);
+}
+
+/* =================================================================================================
+ * O4-O6  One directed pair s -> t: loss sum, valid count and the 12 gradient sums.
+ *
+ * Per source edge pixel p = (u, v, Z)                                    (Eq. 8; 97; 483)
+ *   x_s = K_s^-1 [u,v,1]^T Z ;  x_t = R_ts x_s + t_ts ;  reject if x_t.z <= z_min
+ *   (x, y) = K_t-projection of x_t ; reject unless 0 <= x <= W-1 and 0 <= y <= H-1      (reading S3)
+ *   x0 = min(floor x, W-2), y0 = min(floor y, H-2), wx = x - x0, wy = y - y0
+ *   d  = (1-wy)((1-wx) D00 + wx D01) + wy((1-wx) D10 + wx D11)      "bilinearly samples DTF_j"
+ *   dhat = min(d, lambda) ;  rho = Huber_delta(dhat) = dhat^2/2 if dhat <= delta else delta (dhat - delta/2)
+ *   rho' = [d <= lambda] * min(d, delta)                                              (reading S5)
+ * Gradient w.r.t. left perturbations of both poses (reading S9):
+ *   a = rho' * (dd/dx, dd/dy) * d(x,y)/d x_t
+ *   g_tgt += [ a ; x_t x a ] ;  b = R_ts^T a ;  g_src += [ -b ; -x_s x b ]
+ * All 12 numbers are accumulated independently (identity I1 is NOT used here).
+ * near[0] counts samples within 1e-3 px (or 1e-3 in z) of the validity border, near[1] those with
+ * |d - lambda| < 1e-3 or |d - delta| < 1e-3 -- the discrete events of "Tolerance realism".
+ * ================================================================================================= */
+void orc_pair_loss_grad(int W, int H, int n_edges, const uint16_t* uv, const float* z,
+                        const double Ks[4], const double Kt[4], const double Ts[12], const double Tt[12],
+                        const float* dtf_t, double lambda, double delta, double z_min,
+                        double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2]) {
+  double Tts[12];
+  orc_relative_pose(Ts, Tt, Tts);
+  double S = 0.0; int32_t nv = 0;
+  for (int k = 0; k < 12; ++k) G[k] = 0.0;
+  near[0] = near[1] = 0;
+  for (int e = 0; e < n_edges; ++e) {
+    double xs[3], xt[3], px[2];
+    orc_backproject_cam(Ks, (double)uv[2 * e], (double)uv[2 * e + 1], (double)z[e], xs);
+    for (int i = 0; i < 3; ++i)
+      xt[i] = Tts[4 * i] * xs[0] + Tts[4 * i + 1] * xs[1] + Tts[4 * i + 2] * xs[2] + Tts[4 * i + 3];
+    if (fabs(xt[2] - z_min) < 1e-3 * fabs(z_min)) near[0]++;
+    if (!(xt[2] > z_min)) continue;
+    orc_project_px(Kt, xt, px);
+    double x = px[0], y = px[1];
+    if (fabs(x) < 1e-3 || fabs(x - (W - 1)) < 1e-3 || fabs(y) < 1e-3 || fabs(y - (H - 1)) < 1e-3) near[0]++;
+    if (!(x >= 0.0 && x <= (double)(W - 1) && y >= 0.0 && y <= (double)(H - 1))) continue;
+    int x0 = (int)floor(x), y0 = (int)floor(y);
+    if (x0 > W - 2) x0 = W - 2;
+    if (y0 > H - 2) y0 = H - 2;
+    double wx = x - x0, wy = y - y0;
+    double D00 = dtf_t[(size_t)y0 * W + x0], D01 = dtf_t[(size_t)y0 * W + x0 + 1];
+    double D10 = dtf_t[(size_t)(y0 + 1) * W + x0], D11 = dtf_t[(size_t)(y0 + 1) * W + x0 + 1];
+    double d = (1.0 - wy) * ((1.0 - wx) * D00 + wx * D01) + wy * ((1.0 - wx) * D10 + wx * D11);
+    double ddx = (1.0 - wy) * (D01 - D00) + wy * (D11 - D10);
+    double ddy = (1.0 - wx) * (D10 - D00) + wx * (D11 - D01);
+    if (fabs(d - lambda) < 1e-3 || fabs(d - delta) < 1e-3) near[1]++;
+    double dhat = d < lambda ? d : lambda;
+    double rho = dhat <= delta ? 0.5 * dhat * dhat : delta * (dhat - 0.5 * delta);
+    double drho = (d <= lambda) ? (d < delta ? d : delta) : 0.0;
+    S += rho; nv++;
+    /* d(x,y)/d x_t = [ fx/Z, 0, -fx X/Z^2 ; 0, fy/Z, -fy Y/Z^2 ] */
+    double iz = 1.0 / xt[2];
+    double a[3], b[3];
+    a[0] = drho * ddx * Kt[0] * iz;
+    a[1] = drho * ddy * Kt[1] * iz;
+    a[2] = -drho * (ddx * Kt[0] * xt[0] + ddy * Kt[1] * xt[1]) * iz * iz;
+    G[0] += a[0]; G[1] += a[1]; G[2] += a[2];
+    G[3] += xt[1] * a[2] - xt[2] * a[1];
+    G[4] += xt[2] * a[0] - xt[0] * a[2];
+    G[5] += xt[0] * a[1] - xt[1] * a[0];
+    for (int i = 0; i < 3; ++i) b[i] = Tts[i] * a[0] + Tts[4 + i] * a[1] + Tts[8 + i] * a[2];
+    G[6] -= b[0]; G[7] -= b[1]; G[8] -= b[2];
+    G[9]  -= xs[1] * b[2] - xs[2] * b[1];
+    G[10] -= xs[2] * b[0] - xs[0] * b[2];
+    G[11] -= xs[0] * b[1] - xs[1] * b[0];
+  }
+  *sum_rho = S; *n_valid = nv;
+}
+
+/* =================================================================================================
+ * O5 + row a-9: whole loss and per-camera gradient over a pair list (any order; reduced in list order)
+ *   L_{s->t} = sum_valid rho / n_valid (0 if none)     (Alg. 3, reading A1)
+ *   L = (1/P) sum_D L_{s->t}                           (Eq. 6, reading A3)
+ *   g_c = (1/P) [ sum_{t=c} G^tgt_p / n_p + sum_{s=c} G^src_p / n_p ]
+ * edge_off [N+1], uv [E][2], z [E] hold all views' lists; dtf [N][H][W]; K float [N][4]; poses double [N][12].
+ * Nullable outputs: pair_G [P][12] (un-normalised sums), near [P][2].
+ * ================================================================================================= */
+void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, const int32_t* edge_off,
+                   const uint16_t* uv, const float* z, const float* dtf, int64_t P, const int32_t* pairs,
+                   double lambda, double delta, double z_min, double* pair_loss, int32_t* pair_valid,
+                   double* pair_G, int32_t* near, double* grad, double* loss) {
+  double* Gall = (double*)malloc((size_t)P * 12 * sizeof(double));
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t p = 0; p < P; ++p) {
+    int s = pairs[2 * p], t = pairs[2 * p + 1];
+    double Ks[4], Kt[4], S; int32_t nv, nr[2];
+    for (int i = 0; i < 4; ++i) { Ks[i] = K[4 * s + i]; Kt[i] = K[4 * t + i]; }
+    orc_pair_loss_grad(W, H, edge_off[s + 1] - edge_off[s], uv + 2 * (size_t)edge_off[s], z + edge_off[s],
+                       Ks, Kt, poses + 12 * (size_t)s, poses + 12 * (size_t)t, dtf + (size_t)t * W * H,
+                       lambda, delta, z_min, &S, &nv, Gall + 12 * p, nr);
+    pair_loss[p] = nv > 0 ? S / nv : 0.0;
+    pair_valid[p] = nv;
+    if (near) { near[2 * p] = nr[0]; near[2 * p + 1] = nr[1]; }
+  }
+  for (int i = 0; i < 6 * N; ++i) grad[i] = 0.0;
+  double L = 0.0;
+  for (int64_t p = 0; p < P; ++p) {
+    int s = pairs[2 * p], t = pairs[2 * p + 1];
+    L += pair_loss[p];
+    if (pair_valid[p] > 0)
+      for (int k = 0; k < 6; ++k) {
+        grad[6 * t + k] += Gall[12 * p + k] / pair_valid[p];
+        grad[6 * s + k] += Gall[12 * p + 6 + k] / pair_valid[p];
+      }
+  }
+  for (int i = 0; i < 6 * N; ++i) grad[i] /= (double)P;
+  *loss = L / (double)P;
+  if (pair_G) memcpy(pair_G, Gall, (size_t)P * 12 * sizeof(double));
+  free(Gall);
+}
+
+/* =================================================================================================
+ * O7  Schedules, Adam, SE(3) exponential  (readings S4, S10, S11)
+ * ================================================================================================= */
+/* clamp lambda: clamp_start -> clamp_end linearly over the first clamp_steps steps */
+double orc_lambda(int s, double clamp_start, double clamp_end, int clamp_steps) {
+  int m = s < clamp_steps ? s : clamp_steps;
+  return clamp_start + (clamp_end - clamp_start) * (double)m / (double)clamp_steps;
+}
+/* "linear learning rate warmup from 0 to 3e-3 over the first 25 steps, followed by cosine annealing
+ *  decay over a maximum of N=2000 iterations" */
+double orc_lr(int s, double lr_max, int warmup, int max_steps) {
+  if (s < warmup) return lr_max * (double)(s + 1) / (double)warmup;
+  return lr_max * 0.5 * (1.0 + cos(ORC_PI * (double)(s - warmup) / (double)(max_steps - warmup)));
+}
+
+/* Exp(v, w) = [ Exp_SO3(w), V(w) v ; 0, 1 ]; V = I + (1-cos th)/th^2 [w]x + (th - sin th)/th^3 [w]x^2;
+ * Taylor forms for th < 1e-4. */
+void orc_se3_exp(const double eps[6], double T[12]) {
+  const double* v = eps; const double* w = eps + 3;
+  double th2 = w[0] * w[0] + w[1] * w[1] + w[2] * w[2], th = sqrt(th2);
+  double A, B, C;   /* sin th/th, (1-cos th)/th^2, (th - sin th)/th^3 */
+  if (th < 1e-4) { A = 1.0 - th2 / 6.0; B = 0.5 - th2 / 24.0; C = 1.0 / 6.0 - th2 / 120.0; }
+  else { A = sin(th) / th; B = (1.0 - cos(th)) / th2; C = (th - sin(th)) / (th2 * th); }
+  double Wx[9] = { 0, -w[2], w[1], w[2], 0, -w[0], -w[1], w[0], 0 }, W2[9];
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j)
+      W2[3 * i + j] = Wx[3 * i] * Wx[j] + Wx[3 * i + 1] * Wx[3 + j] + Wx[3 * i + 2] * Wx[6 + j];
+  for (int i = 0; i < 3; ++i) {
+    double tv = 0.0;
+    for (int j = 0; j < 3; ++j) {
+      double I = (i == j) ? 1.0 : 0.0;
+      T[4 * i + j] = I + A * Wx[3 * i + j] + B * W2[3 * i + j];
+      tv += (I + B * Wx[3 * i + j] + C * W2[3 * i + j]) * v[j];
+    }
+    T[4 * i + 3] = tv;
+  }
+}
+/* T <- E T for 3x4 [R|t] matrices */
+void orc_se3_compose(const double E[12], const double T[12], double out[12]) {
+  for (int i = 0; i < 3; ++i) {
+    for (int j = 0; j < 4; ++j)
+      out[4 * i + j] = E[4 * i] * T[j] + E[4 * i + 1] * T[4 + j] + E[4 * i + 2] * T[8 + j];
+    out[4 * i + 3] += E[4 * i + 3];
+  }
+}
+/* One Adam step on the n-vector g (step index s = 0,1,..): returns the increment eps = -lr m^/(sqrt v^ + eps). */
+void orc_adam(int n, const double* g, double* m, double* v, int s, double lr, double beta1, double beta2,
+              double adam_eps, double* eps_out) {
+  double c1 = 1.0 - pow(beta1, (double)(s + 1)), c2 = 1.0 - pow(beta2, (double)(s + 1));
+  for (int i = 0; i < n; ++i) {
+    m[i] = beta1 * m[i] + (1.0 - beta1) * g[i];
+    v[i] = beta2 * v[i] + (1.0 - beta2) * g[i] * g[i];
+    eps_out[i] = -lr * (m[i] / c1) / (sqrt(v[i] / c2) + adam_eps);
+  }
+}
+
+/* =================================================================================================
+ * O8  Pose change and the windowed two-phase stopping rule
+ * ================================================================================================= */
+static double clip1(double c) { return c > 1.0 ? 1.0 : (c < -1.0 ? -1.0 : c); }
+/* Eq. 9 */
+double orc_delta_R_deg(const double Tcur[12], const double Tprev[12]) {
+  double tr = 0.0;                                  /* tr(R^s (R^{s-1})^T) = sum_ij R^s_ij R^{s-1}_ij */
+  for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) tr += Tcur[4 * i + j] * Tprev[4 * i + j];
+  return (180.0 / ORC_PI) * acos(clip1((tr - 1.0) / 2.0));
+}
+/* Eq. 10; 0 if either norm < 1e-12 (reading S13) */
+double orc_delta_t_deg(const double Tcur[12], const double Tprev[12]) {
+  double a[3] = { Tcur[3], Tcur[7], Tcur[11] }, b[3] = { Tprev[3], Tprev[7], Tprev[11] };
+  double na = sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]), nb = sqrt(b[0] * b[0] + b[1] * b[1] + b[2] * b[2]);
+  if (na < 1e-12 || nb < 1e-12) return 0.0;
+  double c = (a[0] / na) * (b[0] / nb) + (a[1] / na) * (b[1] / nb) + (a[2] / na) * (b[2] / nb);
+  return (180.0 / ORC_PI) * acos(clip1(c));
+}
+static int cmp_double(const void* a, const void* b) {
+  double x = *(const double*)a, y = *(const double*)b; return (x > y) - (x < y);
+}
+/* q-th percentile with linear interpolation at rank q/100 (n-1) (reading S12) */
+double orc_percentile(int n, const double* x, double q) {
+  double* a = (double*)malloc((size_t)n * sizeof(double));
+  memcpy(a, x, (size_t)n * sizeof(double));
+  qsort(a, (size_t)n, sizeof(double), cmp_double);
+  double rank = q / 100.0 * (double)(n - 1);
+  int k = (int)floor(rank); double f = rank - k, r;
+  r = (k + 1 < n) ? a[k] + f * (a[k + 1] - a[k]) : a[n - 1];
+  free(a); return r;
+}
+/* theta95 = max(dR95, dt95) */
+double orc_theta95(int N, const double* cur, const double* prev) {
+  double* dR = (double*)malloc((size_t)N * sizeof(double)); double* dt = (double*)malloc((size_t)N * sizeof(double));
+  for (int c = 0; c < N; ++c) { dR[c] = orc_delta_R_deg(cur + 12 * c, prev + 12 * c); dt[c] = orc_delta_t_deg(cur + 12 * c, prev + 12 * c); }
+  double r = orc_percentile(N, dR, 95.0), t = orc_percentile(N, dt, 95.0);
+  free(dR); free(dt);
+  return r > t ? r : t;
+}
+/* Converged(theta_{0..s}; w, eps).  smooth != 0: moving average of width w, "fires only when every
+ * smoothed value in the window is below eps"; smooth == 0: "remains below eps for w
+ * consecutive steps".  Reading A2. */
+int orc_converged(const double* theta, int s, int w, double eps, int smooth) {
+  if (smooth) {
+    if (s < 2 * w - 2) return 0;
+    for (int k = s - w + 1; k <= s; ++k) {
+      double m = 0.0;
+      for (int j = k - w + 1; j <= k; ++j) m += theta[j];
+      if (!(m / w < eps)) return 0;
+    }
+    return 1;
+  }
+  if (s < w - 1) return 0;
+  for (int k = s - w + 1; k <= s; ++k) if (!(theta[k] < eps)) return 0;
+  return 1;
+}
+
+typedef struct {
+  double huber_delta, clamp_start, clamp_end; int32_t clamp_steps;
+  double lr_max; int32_t warmup_steps, max_steps;
+  double beta1, beta2, adam_eps, eps1, eps2; int32_t w1, w2, smooth_window, early_stop;
+  double z_min;
+} orc_config;
+
+/* =================================================================================================
+ * The loop of Alg. 2 with the se(3)-Adam parameterisation (reading S9):
+ *   for s = start .. : lambda_s -> loss + gradient at the current poses -> Adam -> T_c <- Exp(eps_c) T_c
+ *   -> theta95^s vs the previous poses -> Converged tests (phase 0 -> 1 -> 2 = stop).
+ * poses [N][12] in/out; m, v [N][6] in/out; theta_hist [max_steps] in/out; *step, *phase in/out.
+ * trace_loss[s] = loss at the poses BEFORE update s.  Returns the number of iterations executed.
+ * ================================================================================================= */
+int orc_run(const orc_config* cfg, int n_iters, int N, int W, int H, const float* K, double* poses,
+            const int32_t* edge_off, const uint16_t* uv, const float* z, const float* dtf, int64_t P,
+            const int32_t* pairs, double* m, double* v, double* theta_hist, double* trace_loss,
+            int32_t* step, int32_t* phase, double* poses_log /* nullable [n_iters][N][12] */) {
+  double* pl = (double*)malloc((size_t)P * sizeof(double));
+  int32_t* pv = (int32_t*)malloc((size_t)P * sizeof(int32_t));
+  double* g = (double*)malloc((size_t)N * 6 * sizeof(double));
+  double* eps = (double*)malloc((size_t)N * 6 * sizeof(double));
+  double* prev = (double*)malloc((size_t)N * 12 * sizeof(double));
+  int done = 0;
+  while (done < n_iters && *step < cfg->max_steps && !(cfg->early_stop && *phase == 2)) {
+    int s = *step; double L;
+    double lambda = orc_lambda(s, cfg->clamp_start, cfg->clamp_end, cfg->clamp_steps);
+    orc_loss_grad(N, W, H, K, poses, edge_off, uv, z, dtf, P, pairs, lambda, cfg->huber_delta, cfg->z_min,
+                  pl, pv, NULL, NULL, g, &L);
+    trace_loss[s] = L;
+    orc_adam(6 * N, g, m, v, s, orc_lr(s, cfg->lr_max, cfg->warmup_steps, cfg->max_steps), cfg->beta1,
+             cfg->beta2, cfg->adam_eps, eps);
+    memcpy(prev, poses, (size_t)N * 12 * sizeof(double));
+    for (int c = 0; c < N; ++c) {
+      double E[12], Tn[12];
+      orc_se3_exp(eps + 6 * c, E);
+      orc_se3_compose(E, prev + 12 * c, Tn);
+      memcpy(poses + 12 * c, Tn, sizeof(Tn));
+    }
+    theta_hist[s] = orc_theta95(N, poses, prev);
+    if (*phase == 0) { if (orc_converged(theta_hist, s, cfg->w1, cfg->eps1, cfg->smooth_window)) *phase = 1; }
+    else if (*phase == 1) { if (orc_converged(theta_hist, s, cfg->w2, cfg->eps2, cfg->smooth_window)) *phase = 2; }
+    if (poses_log) memcpy(poses_log + (size_t)done * N * 12, poses, (size_t)N * 12 * sizeof(double));
+    *step = s + 1; ++done;
+  }
+  free(pl); free(pv); free(g); free(eps); free(prev);
+  return done;
+}

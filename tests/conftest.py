@@ -1,0 +1,25 @@
+import os
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def pytest_configure(config):
+    config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+
+
+@pytest.fixture(scope="session")
+def tiny_scene():
+    from epo_scenes import make_scene
+    return make_scene(1)
+
+
+@pytest.fixture(scope="session")
+def tiny_problem(tiny_scene):
+    import oracle
+    s = tiny_scene
+    return oracle.preprocess(s.K, s.depth, s.edges)

@@ -1,0 +1,194 @@
+"""Pins for the oracle's optimiser side (O7, O8; checks Z6-Z10 and the loop order).
+
+Expected values: scipy's matrix exponential, torch.optim.Adam on CPU, numpy.percentile, closed forms
+and hand-computed traces.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+from scipy.linalg import expm
+
+import oracle
+from epo_scenes import SplitMix64, rodrigues
+
+
+def _twist(e):
+    X = np.zeros((4, 4))
+    X[:3, :3] = np.array([[0, -e[5], e[4]], [e[5], 0, -e[3]], [-e[4], e[3], 0]])
+    X[:3, 3] = e[:3]
+    return X
+
+
+# ------------------------------------------------------------------------------------------------ Z6
+def test_Z6_se3_exp_matches_scipy_expm():
+    rng = SplitMix64(8)
+    for scale in (1e-9, 1e-5, 9.9e-5, 1.01e-4, 1e-3, 0.3, 2.5):
+        for _ in range(20):
+            e = rng.normal(6) * scale
+            ref = expm(_twist(e))[:3].reshape(12)
+            got = oracle.se3_exp(e)
+            assert np.max(np.abs(got - ref)) < 1e-13 * max(1.0, scale), (scale, got - ref)
+            inv = oracle.se3_compose(oracle.se3_exp(-e), got)      # Exp(-e) Exp(e) = I
+            assert np.max(np.abs(inv - np.eye(4)[:3].reshape(12))) < 1e-13 * max(1.0, scale)
+    # continuity across the Taylor switch at theta = 1e-4
+    ax = np.array([0.3, -0.5, 0.81]); ax /= np.linalg.norm(ax)
+    a = oracle.se3_exp(np.concatenate([[1, 2, 3], ax * (1e-4 * (1 - 1e-9))]))
+    b = oracle.se3_exp(np.concatenate([[1, 2, 3], ax * (1e-4 * (1 + 1e-9))]))
+    assert np.max(np.abs(a - b)) < 1e-11
+
+
+def test_se3_compose_is_matrix_product():
+    rng = SplitMix64(9)
+    A = np.eye(4); B = np.eye(4)
+    A[:3] = rng.normal(12).reshape(3, 4); B[:3] = rng.normal(12).reshape(3, 4)
+    assert np.allclose(oracle.se3_compose(A[:3].reshape(12), B[:3].reshape(12)), (A @ B)[:3].reshape(12), atol=1e-14)
+
+
+# ------------------------------------------------------------------------------------------------ Z7
+def test_Z7_adam_matches_torch_optim_adam():
+    rng = SplitMix64(10)
+    n, steps = 30, 40
+    cfg = oracle.Config()
+    m = np.zeros(n); v = np.zeros(n)
+    p = torch.zeros(n, dtype=torch.float64, requires_grad=True)
+    opt = torch.optim.Adam([p], lr=1.0, betas=(cfg.beta1, cfg.beta2), eps=cfg.adam_eps)
+    acc = np.zeros(n)
+    for s in range(steps):
+        g = rng.normal(n) * (10.0 ** float(rng.uniform(1, -3, 2)[0]))
+        lr = oracle.lr_schedule(s, cfg)
+        inc = oracle.adam(g, m, v, s, lr)
+        acc += inc
+        for grp in opt.param_groups:
+            grp["lr"] = lr
+        p.grad = torch.from_numpy(g.copy())
+        opt.step()
+        assert np.max(np.abs(p.detach().numpy() - acc)) < 1e-12
+        if s == 0:    # closed form of the first step: |eps_k| = lr |g| / (|g| + eps)
+            assert np.allclose(np.abs(inc), lr * np.abs(g) / (np.abs(g) + cfg.adam_eps), rtol=1e-12, atol=0)
+
+
+# ------------------------------------------------------------------------------------------------ Z8
+def test_Z8_pose_change_closed_forms_and_percentile():
+    rng = SplitMix64(12)
+    for _ in range(50):
+        R0 = rodrigues(rng.unit_vectors(1)[0], float(rng.uniform(1, 0, 3)[0]))
+        T0 = np.concatenate([R0, rng.normal(3)[:, None]], axis=1).reshape(12)
+        w = rng.unit_vectors(1)[0] * float(10 ** rng.uniform(1, -4, 0)[0])
+        eps = np.concatenate([rng.normal(3) * 1e-3, w])
+        T1 = oracle.se3_compose(oracle.se3_exp(eps), T0)
+        # R^s (R^{s-1})^T = Exp(w)  =>  Delta R = (180/pi) |w|       (Eq. 9)
+        assert abs(oracle.delta_R_deg(T1, T0) - math.degrees(np.linalg.norm(w))) < 2e-5 * math.degrees(np.linalg.norm(w)) + 1e-9
+        t0, t1 = T0.reshape(3, 4)[:, 3], T1.reshape(3, 4)[:, 3]
+        ang = math.degrees(math.atan2(np.linalg.norm(np.cross(t0, t1)), float(t0 @ t1)))   # Eq. 10, atan2 form
+        assert abs(oracle.delta_t_deg(T1, T0) - ang) < 1e-6
+    Z = np.eye(4)[:3].reshape(12)            # t = 0 (first camera is the world frame): Delta t = 0 (reading S13)
+    T = Z.copy(); T[3] = 1.0
+    assert oracle.delta_t_deg(T, Z) == 0.0 and oracle.delta_t_deg(Z, T) == 0.0
+    assert oracle.delta_R_deg(Z, Z) == 0.0
+    for n in (2, 3, 4, 21, 100, 500):
+        x = rng.uniform(n, 0, 5)
+        assert abs(oracle.percentile(x, 95.0) - np.percentile(x, 95)) < 1e-12
+    # theta95 = max of the two percentiles
+    N = 21
+    prev = np.stack([np.concatenate([rodrigues(rng.unit_vectors(1)[0], 0.3), rng.normal(3)[:, None]], axis=1).reshape(12) for _ in range(N)])
+    cur = np.stack([oracle.se3_compose(oracle.se3_exp(rng.normal(6) * 1e-3), prev[i]) for i in range(N)])
+    dR = [oracle.delta_R_deg(cur[i], prev[i]) for i in range(N)]; dt = [oracle.delta_t_deg(cur[i], prev[i]) for i in range(N)]
+    assert abs(oracle.theta95(cur, prev) - max(np.percentile(dR, 95), np.percentile(dt, 95))) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ Z9
+def test_Z9_convergence_logic_on_hand_traces():
+    w, eps = 5, 0.5
+    th = np.full(40, 0.1)
+    # constant trace below eps: smoothed fires first at s = 2w-2, raw at s = w-1
+    assert [s for s in range(40) if oracle.converged(th, s, w, eps, 1)][0] == 2 * w - 2
+    assert [s for s in range(40) if oracle.converged(th, s, w, eps, 0)][0] == w - 1
+    # a single spike at k = 10: raw needs w clean steps after it -> first true again at s = 15
+    th2 = th.copy(); th2[10] = 3.0
+    raw = [oracle.converged(th2, s, w, eps, 0) for s in range(40)]
+    assert raw[9] and not any(raw[10:15]) and raw[15]
+    # smoothed: spike of 3.0 lifts every window mean containing it to (3.0 + 4*0.1)/5 = 0.68 >= eps; the means
+    # with k in [10, 14] are affected, so windows of smoothed values [s-4, s] are clean again from s = 19
+    sm = [oracle.converged(th2, s, w, eps, 1) for s in range(40)]
+    assert sm[9] and not any(sm[10:19]) and sm[19]
+    # a spike smaller than eps*w spread over the window stays below eps: (2.0 + 0.4)/5 = 0.48 < 0.5
+    th3 = th.copy(); th3[10] = 2.0
+    assert all(oracle.converged(th3, s, w, eps, 1) for s in range(8, 40))
+    assert not oracle.converged(th3, 10, w, eps, 0)
+    # values equal to eps do not count as below
+    assert not oracle.converged(np.full(20, 0.5), 15, w, eps, 0)
+
+
+# ------------------------------------------------------------------------------------------------ Z10
+def test_Z10_schedules():
+    cfg = oracle.Config()
+    lam = {0: 10.0, 24: 9.904, 25: 9.9, 999: 6.004, 1000: 6.0, 1999: 6.0}        # PAPER.md:462, linear (S4)
+    for s, val in lam.items():
+        assert abs(oracle.lam_schedule(s, cfg) - val) < 1e-12
+    assert abs(oracle.lr_schedule(0, cfg) - 1.2e-4) < 1e-18                       # PAPER.md:121, reading S11
+    assert abs(oracle.lr_schedule(24, cfg) - 3e-3) < 1e-18
+    assert abs(oracle.lr_schedule(25, cfg) - 3e-3) < 1e-18
+    mid = 25 + (2000 - 25) / 2
+    assert abs(oracle.lr_schedule(int(mid), cfg) - 1.5e-3 * (1 + math.cos(math.pi * (int(mid) - 25) / 1975))) < 1e-15
+    assert oracle.lr_schedule(1999, cfg) < 2e-9 and oracle.lr_schedule(1999, cfg) > 0
+    # torch's own schedulers chained the same way give the same numbers
+    p = torch.zeros(1, requires_grad=True)
+    opt = torch.optim.SGD([p], lr=3e-3)
+    warm = torch.optim.lr_scheduler.LambdaLR(opt, lambda k: (k + 1) / 25)
+    cos = torch.optim.lr_scheduler.CosineAnnealingLR(opt, T_max=1975)
+    sched = torch.optim.lr_scheduler.SequentialLR(opt, [warm, cos], milestones=[25])
+    for s in range(200):
+        assert abs(opt.param_groups[0]["lr"] - oracle.lr_schedule(s, cfg)) < 1e-12, s
+        opt.step(); sched.step()
+
+
+# --------------------------------------------------------------------------------------- loop order
+def test_loop_is_the_composition_of_the_pinned_pieces(tiny_scene, tiny_problem):
+    """Alg. 2 order: loss -> backward -> optimizer step -> pose change -> Converged.
+    orc_run must equal the pinned primitives chained in that order; state machine as Alg. 2 l.13-17."""
+    s = tiny_scene
+    cfg = oracle.Config(w1=4, w2=6, eps1=0.5, eps2=0.2, early_stop=1)
+    opt = oracle.Optimizer(tiny_problem, s.poses_init, s.pairs, cfg)
+    done, log = opt.run(150, log_poses=True)
+    N = s.n_views
+    poses = s.poses_init.astype(np.float64).reshape(N, 12).copy()
+    m = np.zeros((N, 6)); v = np.zeros((N, 6)); theta = []; phase = 0; k = 0
+    while k < 150 and phase != 2:
+        out = oracle.loss_grad(tiny_problem, poses, s.pairs, oracle.lam_schedule(k, cfg))
+        assert out["loss"] == opt.loss[k]
+        inc = oracle.adam(out["grad"].reshape(-1), m.reshape(-1), v.reshape(-1), k, oracle.lr_schedule(k, cfg)).reshape(N, 6)
+        new = np.stack([oracle.se3_compose(oracle.se3_exp(inc[c]), poses[c]) for c in range(N)])
+        theta.append(oracle.theta95(new, poses))
+        poses = new
+        assert np.array_equal(poses, log[k])
+        if phase == 0:
+            if oracle.converged(np.array(theta), k, cfg.w1, cfg.eps1): phase = 1
+        elif oracle.converged(np.array(theta), k, cfg.w2, cfg.eps2): phase = 2
+        k += 1
+    assert k == done and phase == opt.phase.value == 2 and done < 150
+    assert np.array_equal(np.array(theta), opt.theta[:done])
+    # a second call after the stop does nothing
+    assert opt.run(10)[0] == 0
+
+
+def test_optimisation_descends_towards_ground_truth(tiny_scene, tiny_problem):
+    """Sign of the whole update: 200 iterations lower the loss to the GT level and shrink the relative
+    rotation error of every pair (the paper evaluates relative poses)."""
+    s = tiny_scene
+    opt = oracle.Optimizer(tiny_problem, s.poses_init, s.pairs, oracle.Config())
+    done, _ = opt.run(200)
+    assert done == 200
+    L_gt = oracle.loss_grad(tiny_problem, s.poses_gt, s.pairs, oracle.lam_schedule(199))["loss"]
+    assert opt.loss[0] > 5 * L_gt and opt.loss[199] < 1.5 * L_gt
+
+    def rel_rot_err(P):
+        errs = []
+        for a, b in s.pairs:
+            Rel = oracle.relative_pose(P[a], P[b]).reshape(3, 4)[:, :3]
+            Rgt = oracle.relative_pose(s.poses_gt[a], s.poses_gt[b]).reshape(3, 4)[:, :3]
+            errs.append(math.degrees(math.acos(max(-1, min(1, (np.trace(Rel @ Rgt.T) - 1) / 2)))))
+        return np.array(errs)
+    e0 = rel_rot_err(s.poses_init.astype(np.float64)); e1 = rel_rot_err(opt.poses)
+    assert e1.mean() < 0.25 * e0.mean()
