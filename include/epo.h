@@ -1,0 +1,154 @@
+/*
+ * epo.h -- C ABI of the B200-native hot path of EPO (Edge-based Pose Optimization, arxiv 2607.00579).
+ *
+ * The library evaluates, for every selected directed image pair (s -> t), the edge-based reprojection
+ * loss of the paper (Eq. 6-8) and its analytic gradient w.r.t. both cameras' 6-DoF
+ * poses, reduces them per camera, and runs the first-order optimisation loop of Alg. 2
+ * with Adam on se(3) increments and the paper's pose-change stopping rule
+ * entirely on the device.  Every step runs in hand-written CUDA kernels
+ * for sm_100a; there is no CPU fallback: without a CUDA device every compute entry point returns
+ * EPO_ERR_CUDA.
+ *
+ * Conventions
+ *   poses     world-to-camera [R|t], row-major 3x4, x_cam = R X_w + t
+ *   K         (fx, fy, cx, cy) per view; pixel (u,v) is the sample position (no half-pixel offset)
+ *   depth     z-depth along the optical axis
+ *   gradient  w.r.t. a left perturbation T_c <- Exp(eps_c) T_c, eps = (v, w), translation part first
+ *   pairs     (source, target): edge pixels of `source` are projected into `target`  (Eq. 8)
+ *
+ * Pointers.  Every array argument may be a HOST or a DEVICE pointer (detected with
+ * cudaPointerGetAttributes; device pointers must belong to cfg.device).  The caller owns every array
+ * it passes; the library copies inputs during the call and never retains caller pointers.  The context
+ * owns all device memory it allocates and frees it in epo_destroy.
+ * Streams.  All work is enqueued on cfg.stream.  Calls that return data through HOST pointers
+ * synchronise that stream before returning; calls given only DEVICE output pointers do not.
+ * Errors.  Every function returns an epo_status; nothing throws or aborts.  On error the context is
+ * left unchanged (epo_set_views / epo_set_pairs are all-or-nothing); epo_last_error gives a
+ * context-owned, NUL-terminated description valid until the next call on that context.
+ * Threads.  One context per thread at a time; no global state.
+ * Determinism.  Edge lists, distance fields and pair lists are bit-reproducible.  Loss and gradient
+ * are reproducible up to the order of a few fp64 atomic additions per pair (relative 1e-16).
+ */
+#ifndef EPO_H_
+#define EPO_H_
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define EPO_API __attribute__((visibility("default")))
+#else
+#define EPO_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct epo_ctx epo_ctx;
+
+typedef enum {
+  EPO_OK = 0,
+  EPO_ERR_INVALID_ARG = 1,   /* NULL required pointer, bad size, non-finite intrinsics, bad pair index ... */
+  EPO_ERR_BAD_STATE = 2,     /* call order: set_pairs before set_views, loss_grad/step before both        */
+  EPO_ERR_OUT_OF_MEMORY = 3,
+  EPO_ERR_CUDA = 4,          /* any CUDA runtime failure, including "no device"                           */
+  EPO_ERR_UNSUPPORTED = 5
+} epo_status;
+
+typedef struct {
+  int32_t n_views, width, height;   /* one resolution per context (all images resized to width 518) */
+  float   huber_delta;              /* Huber threshold; 1.0 (paper silent: DESIGN.md reading S1)            */
+  float   clamp_start, clamp_end;   /* lambda: 10 -> 6 ...                                                  */
+  int32_t clamp_steps;              /* ... linearly over the first 1000 steps               */
+  float   lr_max;                   /* 3e-3                                                  */
+  int32_t warmup_steps, max_steps;  /* 25, 2000: linear warm-up then cosine decay           */
+  float   beta1, beta2, adam_eps;   /* 0.9, 0.999, 1e-8 (reading S10)                       */
+  float   eps1, eps2;               /* 0.5, 0.1 degrees                                      */
+  int32_t w1, w2;                   /* 25, 50 steps                                          */
+  int32_t smooth_window;            /* 1: moving average of width w; 0: raw  */
+  int32_t early_stop;               /* 1: epo_step stops at phase 2; 0: phase is tracked but never stops    */
+  int32_t dtf_format;               /* 0: fp32 distance fields; 1: fp16 fields (BASELINE.json config 4)    */
+  int32_t e_max;                    /* 0: keep all edge pixels; >0: keep entries floor(j n / e_max) (S6)    */
+  float   z_min;                    /* 1e-6: depths and projected z at or below it are invalid             */
+  int32_t device;                   /* CUDA device ordinal                                                  */
+  void*   stream;                   /* cudaStream_t (NULL = legacy default stream)                          */
+} epo_config;
+
+/* Fill *cfg with the paper's hyper-parameters (n_views/width/height = 0, device 0, stream NULL). */
+EPO_API epo_status epo_config_default(epo_config* cfg);
+
+/* Create a context.  Requires n_views >= 2, 2 <= width,height <= 65535 (16-bit pixel coordinates). */
+EPO_API epo_status epo_create(const epo_config* cfg, epo_ctx** out);
+
+/* Free everything the context owns.  NULL-safe. */
+EPO_API void epo_destroy(epo_ctx* ctx);
+
+/*
+ * Load the initial estimate G = {K_i, P_i, Z_i} (Eq. 1) and the edge maps E_i
+ * (PAPER.md:62), and run the one-time preprocessing (Alg. 1 l.6-7):
+ *   - edge-pixel compaction: per view, the list of (u, v, Z) with edges != 0 and finite Z > z_min, in
+ *     raster order (v ascending, then u), optionally sub-sampled to e_max entries;
+ *   - exact Euclidean distance transform DTF_i (distance in pixels to the nearest pixel with
+ *     edges != 0; W+H everywhere if the view has none), fp32 = correctly rounded sqrt of the exact
+ *     integer squared distance; optionally rounded (RNE) to fp16.
+ * K [N][4]; poses [N][12]; depth [N][H][W] fp32; edges [N][H][W] u8 (non-zero = edge).
+ * Resets poses, Adam moments, step counter, phase and traces; keeps no pair list (call epo_set_pairs).
+ */
+EPO_API epo_status epo_set_views(epo_ctx* ctx, const float* K, const float* poses, const float* depth,
+                         const uint8_t* edges);
+
+/*
+ * Set the viewgraph as a list of DIRECTED pairs [P][2] = (source, target), P >= 1,
+ * indices in [0, N), source != target; duplicates are kept (they weigh twice).  Builds the canonical
+ * order (ascending (target, source), stable), the per-target and per-source incidence lists and the
+ * work list of the fused kernel.  Resets Adam moments, step counter, phase and traces.
+ */
+EPO_API epo_status epo_set_pairs(epo_ctx* ctx, const int32_t* pairs, int64_t n_pairs);
+
+/*
+ * One evaluation at the CURRENT poses with clamp `lambda`:
+ *   pair_loss[p]  = sum_valid H_delta(min(d, lambda)) / n_valid   (0 if n_valid = 0; Alg. 3 l.11-12)
+ *   loss          = mean over the P directed pairs                 (Eq. 6; = 1/2 Eq. 6 for symmetric lists)
+ *   grad[c]       = d loss / d eps_c, (v, w) order, n_valid held fixed
+ * loss [1] required; pair_loss [P], pair_valid [P] (user pair order) and grad [N][6] are nullable.
+ * Does not change poses or optimiser state.
+ */
+EPO_API epo_status epo_loss_grad(epo_ctx* ctx, float lambda, float* loss, float* pair_loss, int32_t* pair_valid,
+                         float* grad);
+
+/*
+ * Run up to n_iters iterations of Alg. 2 on the device without host synchronisation between them:
+ *   lambda_s -> loss + gradient -> Adam (lr_s: PAPER.md:121) -> T_c <- Exp(eps_c) T_c
+ *   -> theta95^s (Eq. 9-10, 95th percentiles) -> Converged tests (phase 0 -> 1 -> 2).
+ * Iterations stop early when the step counter reaches max_steps or, if early_stop, when phase 2 is
+ * reached.  iters_done / phase (0, 1, or 2 = second convergence reached) are nullable; host pointers
+ * there make the call synchronise.
+ */
+EPO_API epo_status epo_step(epo_ctx* ctx, int32_t n_iters, int32_t* iters_done, int32_t* phase);
+
+/* Current poses, [N][12] fp32 (rounded from the fp64 device state) / fp64 (exact). */
+EPO_API epo_status epo_get_poses(epo_ctx* ctx, float* poses);
+EPO_API epo_status epo_get_poses_f64(epo_ctx* ctx, double* poses);
+
+/* Replace the current poses ([N][12] fp32; NULL = the poses given to epo_set_views) and reset Adam
+ * moments, step counter, phase and traces.  Preprocessing and pair lists are kept. */
+EPO_API epo_status epo_reset(epo_ctx* ctx, const float* poses);
+
+/* ---- introspection (used by the parity tests and the benchmark) ------------------------------- */
+EPO_API epo_status epo_get_edge_counts(epo_ctx* ctx, int32_t* offsets /* [N+1] exclusive prefix sums */);
+EPO_API epo_status epo_get_edge_list(epo_ctx* ctx, int32_t view, uint16_t* uv /* [E][2] (u,v) */, float* z /* [E] */);
+EPO_API epo_status epo_get_dtf(epo_ctx* ctx, int32_t view, float* dtf /* [H][W]; fp16 fields are widened */);
+EPO_API epo_status epo_get_pair_order(epo_ctx* ctx, int32_t* canonical_pairs /* [P][2] */, int32_t* perm /* [P]:
+                              index in the user list of the k-th canonical pair */);
+/* loss (at the poses before update s) and theta95 of steps first .. first+count-1 (<= steps done) */
+EPO_API epo_status epo_get_trace(epo_ctx* ctx, int32_t first, int32_t count, float* loss, float* theta95);
+/* attempted reprojections per evaluation = sum over pairs of the source's edge count */
+EPO_API epo_status epo_get_work(epo_ctx* ctx, int64_t* reprojections_per_eval, int64_t* kernel_launches_so_far);
+
+EPO_API const char* epo_last_error(const epo_ctx* ctx);
+EPO_API const char* epo_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EPO_H_ */

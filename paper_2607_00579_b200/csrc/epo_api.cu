@@ -1,0 +1,446 @@
+// Host side of the C ABI declared in include/epo.h: argument validation, host/device pointer
+// marshalling, device-memory ownership and launch sequencing.  No arithmetic of the method lives here.
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include <new>
+
+#include "epo_internal.h"
+
+epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...) {
+  if (ctx) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+    va_end(ap);
+  }
+  return st;
+}
+
+namespace {
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes a;
+  cudaError_t e = cudaPointerGetAttributes(&a, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// copy caller memory (host or device) into library device memory on the context's stream
+cudaError_t copy_in(void* dst, const void* src, size_t bytes, cudaStream_t st) {
+  return cudaMemcpyAsync(dst, src, bytes, is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
+}
+// copy library device memory to caller memory; *synced is set when the destination is host memory
+cudaError_t copy_out(void* dst, const void* src, size_t bytes, cudaStream_t st, bool* need_sync) {
+  bool dev = is_device_ptr(dst);
+  if (!dev) *need_sync = true;
+  return cudaMemcpyAsync(dst, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st);
+}
+
+void free_views(epo_ctx* c) {
+  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_dtf); cudaFree(c->d_dtf_h);
+  c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_dtf = nullptr; c->d_dtf_h = nullptr;
+  c->have_views = false;
+}
+void free_pairs(epo_ctx* c) {
+  cudaFree(c->d_pairs); cudaFree(c->d_perm); cudaFree(c->d_tgt_off); cudaFree(c->d_src_off); cudaFree(c->d_src_inc);
+  cudaFree(c->d_work); cudaFree(c->d_acc); cudaFree(c->d_pair_loss); cudaFree(c->d_pair_valid); cudaFree(c->d_out_f);
+  cudaFree(c->d_out_i);
+  c->d_pairs = nullptr; c->d_perm = nullptr; c->d_tgt_off = nullptr; c->d_src_off = nullptr; c->d_src_inc = nullptr;
+  c->d_work = nullptr; c->d_acc = nullptr; c->d_pair_loss = nullptr; c->d_pair_valid = nullptr; c->d_out_f = nullptr;
+  c->d_out_i = nullptr;
+  c->have_pairs = false; c->P = 0; c->n_work = 0;
+}
+
+epo_status reset_optimiser(epo_ctx* c) {
+  cudaStream_t st = c->stream;
+  EPO_CUDA(c, cudaMemsetAsync(c->d_m, 0, (size_t)c->N * 6 * sizeof(double), st));
+  EPO_CUDA(c, cudaMemsetAsync(c->d_v, 0, (size_t)c->N * 6 * sizeof(double), st));
+  EPO_CUDA(c, cudaMemsetAsync(c->d_state, 0, sizeof(DevState), st));
+  EPO_CUDA(c, cudaMemsetAsync(c->d_theta, 0, (size_t)c->cfg.max_steps * sizeof(double), st));
+  EPO_CUDA(c, cudaMemsetAsync(c->d_loss_trace, 0, (size_t)c->cfg.max_steps * sizeof(double), st));
+  return EPO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* epo_version(void) { return "epo-b200 0.1 (sm_100a)"; }
+
+const char* epo_last_error(const epo_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+epo_status epo_config_default(epo_config* cfg) {
+  if (!cfg) return EPO_ERR_INVALID_ARG;
+  std::memset(cfg, 0, sizeof(*cfg));
+  cfg->huber_delta = 1.0f;
+  cfg->clamp_start = 10.0f; cfg->clamp_end = 6.0f; cfg->clamp_steps = 1000;
+  cfg->lr_max = 3e-3f; cfg->warmup_steps = 25; cfg->max_steps = 2000;
+  cfg->beta1 = 0.9f; cfg->beta2 = 0.999f; cfg->adam_eps = 1e-8f;
+  cfg->eps1 = 0.5f; cfg->eps2 = 0.1f; cfg->w1 = 25; cfg->w2 = 50;
+  cfg->smooth_window = 1; cfg->early_stop = 1; cfg->dtf_format = 0; cfg->e_max = 0;
+  cfg->z_min = 1e-6f; cfg->device = 0; cfg->stream = nullptr;
+  return EPO_OK;
+}
+
+epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
+  if (!cfg || !out) return EPO_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (cfg->n_views < 2 || cfg->width < 2 || cfg->height < 2 || cfg->width > 65535 || cfg->height > 65535)
+    return EPO_ERR_INVALID_ARG;
+  if (!(cfg->huber_delta > 0.f) || cfg->clamp_steps < 1 || cfg->warmup_steps < 0 || cfg->max_steps <= cfg->warmup_steps ||
+      cfg->w1 < 1 || cfg->w2 < 1 || (cfg->dtf_format != 0 && cfg->dtf_format != 1) || cfg->e_max < 0 ||
+      !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
+    return EPO_ERR_INVALID_ARG;
+  epo_ctx* c = new (std::nothrow) epo_ctx();
+  if (!c) return EPO_ERR_OUT_OF_MEMORY;
+  c->cfg = *cfg; c->stream = (cudaStream_t)cfg->stream;
+  c->N = cfg->n_views; c->W = cfg->width; c->H = cfg->height;
+  c->have_views = c->have_pairs = false; c->P = c->E = c->n_work = c->reproj_per_eval = c->launches = 0;
+  c->err[0] = 0;
+  cudaError_t e = cudaSetDevice(cfg->device);
+  const size_t N = (size_t)c->N;
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_K, N * 4 * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_poses, N * 12 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_poses_init, N * 12 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_grad, N * 6 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_loss_part, N * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_m, N * 6 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_v, N * 6 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_dR, N * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_dt, N * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_state, sizeof(DevState));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_theta, (size_t)cfg->max_steps * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_loss_trace, (size_t)cfg->max_steps * sizeof(double));
+  if (e != cudaSuccess) {
+    epo_status st = (e == cudaErrorMemoryAllocation) ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA;
+    cudaGetLastError();
+    epo_destroy(c);
+    return st;
+  }
+  *out = c;
+  return EPO_OK;
+}
+
+void epo_destroy(epo_ctx* c) {
+  if (!c) return;
+  cudaSetDevice(c->cfg.device);
+  cudaStreamSynchronize(c->stream);
+  free_pairs(c); free_views(c);
+  cudaFree(c->d_K); cudaFree(c->d_poses); cudaFree(c->d_poses_init); cudaFree(c->d_grad); cudaFree(c->d_loss_part);
+  cudaFree(c->d_m); cudaFree(c->d_v); cudaFree(c->d_dR); cudaFree(c->d_dt); cudaFree(c->d_state);
+  cudaFree(c->d_theta); cudaFree(c->d_loss_trace);
+  cudaGetLastError();
+  delete c;
+}
+
+epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const float* depth, const uint8_t* edges) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!K || !poses || !depth || !edges) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_views: NULL argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t N = (size_t)c->N, px = (size_t)c->W * c->H;
+  // validate intrinsics and poses on the host (small arrays)
+  std::vector<float> hK(N * 4), hP(N * 12);
+  EPO_CUDA(c, cudaMemcpyAsync(hK.data(), K, N * 4 * sizeof(float), cudaMemcpyDefault, st));
+  EPO_CUDA(c, cudaMemcpyAsync(hP.data(), poses, N * 12 * sizeof(float), cudaMemcpyDefault, st));
+  EPO_CUDA(c, cudaStreamSynchronize(st));
+  for (size_t i = 0; i < N; ++i) {
+    if (!(std::isfinite(hK[4 * i]) && hK[4 * i] > 0.f && std::isfinite(hK[4 * i + 1]) && hK[4 * i + 1] > 0.f &&
+          std::isfinite(hK[4 * i + 2]) && std::isfinite(hK[4 * i + 3])))
+      return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_views: view %zu has non-finite or non-positive intrinsics", i);
+    for (int k = 0; k < 12; ++k)
+      if (!std::isfinite(hP[12 * i + k]))
+        return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_views: view %zu has a non-finite pose", i);
+  }
+  // build everything into temporaries; commit only on success (all-or-nothing)
+  float* d_depth = nullptr; uint8_t* d_e = nullptr; float* d_dtf = nullptr; __half* d_dtf_h = nullptr;
+  float* d_pose_f = nullptr; int32_t* off = nullptr; EdgeRec* rec = nullptr; int64_t E = 0;
+  std::vector<int32_t> hoff;
+  epo_status rc = EPO_OK;
+  cudaError_t e = cudaMalloc(&d_depth, N * px * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&d_e, N * px);
+  if (e == cudaSuccess) e = cudaMalloc(&d_dtf, N * px * sizeof(float));
+  if (e == cudaSuccess && c->cfg.dtf_format == 1) e = cudaMalloc(&d_dtf_h, N * px * sizeof(__half));
+  if (e == cudaSuccess) e = cudaMalloc(&d_pose_f, N * 12 * sizeof(float));
+  if (e == cudaSuccess) e = copy_in(d_depth, depth, N * px * sizeof(float), st);
+  if (e == cudaSuccess) e = copy_in(d_e, edges, N * px, st);
+  if (e != cudaSuccess)
+    rc = epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_set_views: %s",
+                  cudaGetErrorString(e));
+  if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff);
+  if (rc == EPO_OK) rc = epo_build_dtf(c, d_e, d_dtf, d_dtf_h);
+  cudaFree(d_depth); cudaFree(d_e);
+  if (rc != EPO_OK) {
+    cudaGetLastError();
+    cudaFree(d_dtf); cudaFree(d_dtf_h); cudaFree(d_pose_f); cudaFree(off); cudaFree(rec);
+    return rc;
+  }
+  free_pairs(c); free_views(c);
+  c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff; c->d_dtf = d_dtf; c->d_dtf_h = d_dtf_h;
+  EPO_CUDA(c, cudaMemcpyAsync(c->d_K, hK.data(), N * 4 * sizeof(float), cudaMemcpyHostToDevice, st));
+  EPO_CUDA(c, cudaMemcpyAsync(d_pose_f, hP.data(), N * 12 * sizeof(float), cudaMemcpyHostToDevice, st));
+  epo_launch_f32_to_f64(st, d_pose_f, c->d_poses_init, (int64_t)N * 12);
+  EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  c->launches += 1;
+  EPO_TRY(reset_optimiser(c));
+  EPO_CUDA(c, cudaStreamSynchronize(st));   // hK / hP are stack-owned
+  cudaFree(d_pose_f);
+  c->have_views = true;
+  return EPO_OK;
+}
+
+epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_set_pairs before epo_set_views");
+  if (!pairs || P <= 0 || P > (int64_t)1 << 30) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_pairs: NULL list or bad count");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  std::vector<int32_t> hp((size_t)P * 2);
+  EPO_CUDA(c, cudaMemcpyAsync(hp.data(), pairs, (size_t)P * 2 * sizeof(int32_t), cudaMemcpyDefault, st));
+  EPO_CUDA(c, cudaStreamSynchronize(st));
+  int64_t reproj = 0;
+  for (int64_t k = 0; k < P; ++k) {
+    int s = hp[2 * k], t = hp[2 * k + 1];
+    if (s < 0 || s >= c->N || t < 0 || t >= c->N || s == t)
+      return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_pairs: pair %lld = (%d, %d) is invalid", (long long)k, s, t);
+    reproj += c->h_edge_off[s + 1] - c->h_edge_off[s];
+  }
+  int32_t* d_user = nullptr;
+  EPO_CUDA(c, cudaMalloc(&d_user, (size_t)P * 2 * sizeof(int32_t)));
+  cudaError_t e = cudaMemcpyAsync(d_user, hp.data(), (size_t)P * 2 * sizeof(int32_t), cudaMemcpyHostToDevice, st);
+  int2 *canon = nullptr, *work = nullptr; int32_t *perm = nullptr, *toff = nullptr, *soff = nullptr, *sinc = nullptr;
+  int64_t n_work = 0;
+  epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &n_work)
+                                     : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
+  cudaFree(d_user);
+  double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
+  if (rc == EPO_OK) {
+    // output staging: [loss | grad 6N | pair_loss P | loss trace | theta trace]
+    size_t nf = 1 + (size_t)c->N * 6 + (size_t)P + (size_t)c->cfg.max_steps * 2;
+    e = cudaMalloc(&acc, (size_t)P * kAccStride * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&pl, (size_t)P * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&pv, (size_t)P * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&of, nf * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&oi, (size_t)P * sizeof(int32_t));
+    if (e != cudaSuccess)
+      rc = epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_set_pairs: %s",
+                    cudaGetErrorString(e));
+  }
+  if (rc != EPO_OK) {
+    cudaGetLastError();
+    cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(toff); cudaFree(soff); cudaFree(sinc);
+    cudaFree(acc); cudaFree(pl); cudaFree(pv); cudaFree(of); cudaFree(oi);
+    return rc;
+  }
+  free_pairs(c);
+  c->d_pairs = canon; c->d_perm = perm; c->d_tgt_off = toff; c->d_src_off = soff; c->d_src_inc = sinc; c->d_work = work;
+  c->n_work = n_work; c->P = P; c->d_acc = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
+  c->h_pairs.swap(hp); c->reproj_per_eval = reproj;
+  c->have_pairs = true;
+  EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, (size_t)c->N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  EPO_TRY(reset_optimiser(c));
+  return EPO_OK;
+}
+
+epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss, int32_t* pair_valid, float* grad) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_loss_grad before epo_set_views/epo_set_pairs");
+  if (!loss || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_loss_grad: NULL loss or negative lambda");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  EPO_TRY(epo_launch_loss_grad(c, lambda, false));
+  bool sync = false;
+  // loss: DevState.loss (double) -> float
+  epo_launch_f64_to_f32(st, &c->d_state->loss, c->d_out_f, 1);
+  EPO_CUDA(c, copy_out(loss, c->d_out_f, sizeof(float), st, &sync));
+  if (grad) {
+    epo_launch_f64_to_f32(st, c->d_grad, c->d_out_f + 1, (int64_t)c->N * 6);
+    EPO_CUDA(c, copy_out(grad, c->d_out_f + 1, (size_t)c->N * 6 * sizeof(float), st, &sync));
+    c->launches += 1;
+  }
+  c->launches += 1;
+  if (pair_loss || pair_valid) {
+    // user-order outputs: written straight into device destinations, staged in d_out_f / d_out_i for host ones
+    float* stage_pl = c->d_out_f + 1 + (size_t)c->N * 6;
+    float* opl = pair_loss ? (is_device_ptr(pair_loss) ? pair_loss : stage_pl) : nullptr;
+    int32_t* opv = pair_valid ? (is_device_ptr(pair_valid) ? pair_valid : c->d_out_i) : nullptr;
+    epo_launch_scatter_pair_outputs(st, c->d_pair_loss, c->d_pair_valid, c->d_perm, opl, opv, c->P);
+    c->launches += 1;
+    if (opl == stage_pl) EPO_CUDA(c, copy_out(pair_loss, stage_pl, (size_t)c->P * sizeof(float), st, &sync));
+    if (opv == c->d_out_i) EPO_CUDA(c, copy_out(pair_valid, c->d_out_i, (size_t)c->P * sizeof(int32_t), st, &sync));
+  }
+  if (sync) EPO_CUDA(c, cudaStreamSynchronize(st));
+  EPO_CUDA(c, cudaGetLastError());
+  return EPO_OK;
+}
+
+epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* phase) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_step before epo_set_views/epo_set_pairs");
+  if (n_iters < 0) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_step: negative iteration count");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  EPO_TRY(epo_launch_begin_step_call(c));
+  for (int i = 0; i < n_iters; ++i) {
+    EPO_TRY(epo_launch_loss_grad(c, -1.0f, true));
+    EPO_TRY(epo_launch_update(c));
+  }
+  bool sync = false;
+  if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));
+  if (phase) EPO_CUDA(c, copy_out(phase, &c->d_state->phase, sizeof(int32_t), st, &sync));
+  if (sync) EPO_CUDA(c, cudaStreamSynchronize(st));
+  return EPO_OK;
+}
+
+epo_status epo_get_poses_f64(epo_ctx* c, double* poses) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_poses before epo_set_views");
+  if (!poses) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_poses: NULL output");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  bool sync = false;
+  EPO_CUDA(c, copy_out(poses, c->d_poses, (size_t)c->N * 12 * sizeof(double), c->stream, &sync));
+  if (sync) EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+  return EPO_OK;
+}
+
+epo_status epo_get_poses(epo_ctx* c, float* poses) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_poses before epo_set_views");
+  if (!poses) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_poses: NULL output");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const int64_t n = (int64_t)c->N * 12;
+  if (is_device_ptr(poses)) {
+    epo_launch_f64_to_f32(st, c->d_poses, poses, n);
+    c->launches += 1;
+    EPO_CUDA(c, cudaGetLastError());
+    return EPO_OK;
+  }
+  float* tmp = nullptr;
+  EPO_CUDA(c, cudaMalloc(&tmp, (size_t)n * sizeof(float)));
+  epo_launch_f64_to_f32(st, c->d_poses, tmp, n);
+  c->launches += 1;
+  cudaError_t e = cudaMemcpyAsync(poses, tmp, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(tmp);
+  if (e != cudaSuccess) return epo_fail(c, EPO_ERR_CUDA, "epo_get_poses: %s", cudaGetErrorString(e));
+  return EPO_OK;
+}
+
+epo_status epo_reset(epo_ctx* c, const float* poses) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_reset before epo_set_views");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t n = (size_t)c->N * 12;
+  if (poses) {
+    std::vector<float> hP(n);
+    EPO_CUDA(c, cudaMemcpyAsync(hP.data(), poses, n * sizeof(float), cudaMemcpyDefault, st));
+    EPO_CUDA(c, cudaStreamSynchronize(st));
+    for (size_t k = 0; k < n; ++k)
+      if (!std::isfinite(hP[k])) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_reset: non-finite pose");
+    float* tmp = nullptr;
+    EPO_CUDA(c, cudaMalloc(&tmp, n * sizeof(float)));
+    cudaError_t e = cudaMemcpyAsync(tmp, hP.data(), n * sizeof(float), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) { epo_launch_f32_to_f64(st, tmp, c->d_poses_init, (int64_t)n); c->launches += 1; e = cudaStreamSynchronize(st); }
+    cudaFree(tmp);
+    if (e != cudaSuccess) return epo_fail(c, EPO_ERR_CUDA, "epo_reset: %s", cudaGetErrorString(e));
+  }
+  EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  EPO_TRY(reset_optimiser(c));
+  return EPO_OK;
+}
+
+epo_status epo_get_edge_counts(epo_ctx* c, int32_t* offsets) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_edge_counts before epo_set_views");
+  if (!offsets) return epo_fail(c, EPO_ERR_INVALID_ARG, "NULL output");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  bool sync = false;
+  EPO_CUDA(c, copy_out(offsets, c->d_edge_off, (size_t)(c->N + 1) * sizeof(int32_t), c->stream, &sync));
+  if (sync) EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+  return EPO_OK;
+}
+
+epo_status epo_get_edge_list(epo_ctx* c, int32_t view, uint16_t* uv, float* z) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_edge_list before epo_set_views");
+  if (view < 0 || view >= c->N || !uv || !z) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_edge_list: bad argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  const int32_t lo = c->h_edge_off[view], n = c->h_edge_off[view + 1] - lo;
+  if (n == 0) return EPO_OK;
+  // records are (u | v << 16, z): de-interleave on the host side of the boundary (marshalling only)
+  std::vector<EdgeRec> h((size_t)n);
+  EPO_CUDA(c, cudaMemcpyAsync(h.data(), c->d_edges + lo, (size_t)n * sizeof(EdgeRec), cudaMemcpyDeviceToHost, c->stream));
+  EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+  std::vector<uint16_t> huv((size_t)n * 2); std::vector<float> hz((size_t)n);
+  for (int32_t i = 0; i < n; ++i) { huv[2 * i] = (uint16_t)(h[i].uv & 0xffffu); huv[2 * i + 1] = (uint16_t)(h[i].uv >> 16); hz[i] = h[i].z; }
+  EPO_CUDA(c, cudaMemcpyAsync(uv, huv.data(), (size_t)n * 2 * sizeof(uint16_t), cudaMemcpyDefault, c->stream));
+  EPO_CUDA(c, cudaMemcpyAsync(z, hz.data(), (size_t)n * sizeof(float), cudaMemcpyDefault, c->stream));
+  EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+  return EPO_OK;
+}
+
+epo_status epo_get_dtf(epo_ctx* c, int32_t view, float* dtf) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_dtf before epo_set_views");
+  if (view < 0 || view >= c->N || !dtf) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_dtf: bad argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  const size_t px = (size_t)c->W * c->H;
+  bool sync = false;
+  if (c->cfg.dtf_format == 1) {   // widen the fp16 field that the kernel actually samples
+    std::vector<__half> h(px);
+    EPO_CUDA(c, cudaMemcpyAsync(h.data(), c->d_dtf_h + view * px, px * sizeof(__half), cudaMemcpyDeviceToHost, c->stream));
+    EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+    std::vector<float> f(px);
+    for (size_t i = 0; i < px; ++i) f[i] = __half2float(h[i]);
+    EPO_CUDA(c, cudaMemcpyAsync(dtf, f.data(), px * sizeof(float), cudaMemcpyDefault, c->stream));
+    EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+    return EPO_OK;
+  }
+  EPO_CUDA(c, copy_out(dtf, c->d_dtf + view * px, px * sizeof(float), c->stream, &sync));
+  if (sync) EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+  return EPO_OK;
+}
+
+epo_status epo_get_pair_order(epo_ctx* c, int32_t* canonical_pairs, int32_t* perm) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_pair_order before epo_set_pairs");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  bool sync = false;
+  if (canonical_pairs) EPO_CUDA(c, copy_out(canonical_pairs, c->d_pairs, (size_t)c->P * sizeof(int2), c->stream, &sync));
+  if (perm) EPO_CUDA(c, copy_out(perm, c->d_perm, (size_t)c->P * sizeof(int32_t), c->stream, &sync));
+  if (sync) EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+  return EPO_OK;
+}
+
+epo_status epo_get_trace(epo_ctx* c, int32_t first, int32_t count, float* loss, float* theta95) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_trace before epo_set_pairs");
+  if (first < 0 || count < 0 || first + count > c->cfg.max_steps) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_trace: bad range");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  bool sync = false;
+  if (loss) {
+    float* stage = c->d_out_f + 1 + (size_t)c->N * 6 + (size_t)c->P;
+    epo_launch_f64_to_f32(st, c->d_loss_trace + first, stage, count);
+    EPO_CUDA(c, copy_out(loss, stage, (size_t)count * sizeof(float), st, &sync));
+  }
+  if (theta95) {
+    float* stage = c->d_out_f + 1 + (size_t)c->N * 6 + (size_t)c->P + c->cfg.max_steps;
+    epo_launch_f64_to_f32(st, c->d_theta + first, stage, count);
+    EPO_CUDA(c, copy_out(theta95, stage, (size_t)count * sizeof(float), st, &sync));
+  }
+  if (sync) EPO_CUDA(c, cudaStreamSynchronize(st));
+  return EPO_OK;
+}
+
+epo_status epo_get_work(epo_ctx* c, int64_t* reprojections_per_eval, int64_t* kernel_launches_so_far) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (reprojections_per_eval) *reprojections_per_eval = c->have_pairs ? c->reproj_per_eval : 0;
+  if (kernel_launches_so_far) *kernel_launches_so_far = c->launches;
+  return EPO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,120 @@
+// Internal declarations of the EPO CUDA library (not part of the C ABI; see include/epo.h).
+#pragma once
+
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <vector>
+
+#include "epo.h"
+
+// One compacted edge pixel: (u | v << 16, Z).  8 bytes, loaded with one LDG.64 (row a-P1 of DESIGN.md).
+struct __align__(8) EdgeRec {
+  uint32_t uv;
+  float z;
+};
+
+// Per-pair accumulators written by the fused kernel (row a-8): S = sum rho, n = valid count,
+// A = sum a, M = sum x_t x a (six-accumulator identity I1).  fp64, 64 bytes per pair.
+constexpr int kAccStride = 8;
+
+// Edge pixels handled by one CTA of the fused kernel: kLgThreads threads x kLgPerThread samples.
+constexpr int kLgThreads = 256;
+constexpr int kLgPerThread = 8;
+constexpr int kLgChunk = kLgThreads * kLgPerThread;
+
+// Device-resident control block of the optimisation loop (rows a-10..a-12): lets epo_step enqueue
+// n iterations without any host synchronisation; every kernel of an iteration checks `stopped`.
+struct DevState {
+  int32_t step;        // optimiser step counter s (0-based index of the NEXT update)
+  int32_t phase;       // 0, 1, 2 (Alg. 2 l.13-17)
+  int32_t stopped;     // step >= max_steps, or early_stop && phase == 2
+  int32_t iters_done;  // iterations executed since the last epo_step began
+  double loss;         // loss of the last evaluation
+};
+
+struct epo_ctx {
+  epo_config cfg;
+  cudaStream_t stream;
+  int N, W, H;
+  bool have_views, have_pairs;
+  int64_t P, E, n_work, reproj_per_eval, launches;
+
+  // views
+  float* d_K;             // [N][4]
+  double* d_poses;        // [N][12] current (fp64: T_ts is formed without fp32 cancellation)
+  double* d_poses_init;   // [N][12] as given to epo_set_views / epo_reset
+  int32_t* d_edge_off;    // [N+1]
+  EdgeRec* d_edges;       // [E]
+  float* d_dtf;           // [N][H][W] fp32 field (always kept: epo_get_dtf, fp32 kernel)
+  __half* d_dtf_h;        // [N][H][W] fp16 field when cfg.dtf_format == 1
+  std::vector<int32_t> h_edge_off;
+
+  // pairs
+  int2* d_pairs;          // [P] canonical (s, t), ascending (t, s)
+  int32_t* d_perm;        // [P] user index of canonical pair k
+  int32_t* d_tgt_off;     // [N+1] CSR by target over canonical ids
+  int32_t* d_src_off;     // [N+1]
+  int32_t* d_src_inc;     // [P] canonical ids grouped by source, ascending
+  int2* d_work;           // [n_work] (canonical pair, first edge index of the chunk)
+  std::vector<int32_t> h_pairs;   // user order, for reprojection counting
+
+  // per-evaluation buffers
+  double* d_acc;          // [P][8]
+  float* d_pair_loss;     // [P] canonical order
+  int32_t* d_pair_valid;  // [P]
+  double* d_grad;         // [N][6]
+  double* d_loss_part;    // [N] per-target partial sums of pair losses
+
+  // optimiser
+  double *d_m, *d_v;      // [N][6]
+  double *d_dR, *d_dt;    // [N] per-camera pose change (degrees)
+  DevState* d_state;
+  double* d_theta;        // [max_steps]
+  double* d_loss_trace;   // [max_steps]
+
+  // scratch for outputs in user order / fp32
+  float* d_out_f;         // max(P, 12 N, max_steps) floats
+  int32_t* d_out_i;       // P ints
+
+  char err[512];
+};
+
+// ---- error plumbing ---------------------------------------------------------------------------
+epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
+
+#define EPO_CUDA(ctx, call)                                                                         \
+  do {                                                                                              \
+    cudaError_t e_ = (call);                                                                        \
+    if (e_ != cudaSuccess)                                                                          \
+      return epo_fail((ctx), e_ == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, \
+                      "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);   \
+  } while (0)
+
+#define EPO_TRY(call)              \
+  do {                             \
+    epo_status s_ = (call);        \
+    if (s_ != EPO_OK) return s_;   \
+  } while (0)
+
+// ---- kernel launchers (each .cu file owns its kernels) ----------------------------------------
+// preprocess.cu
+epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
+                                int32_t** out_off, EdgeRec** out_rec, int64_t* out_E,
+                                std::vector<int32_t>* h_off);
+epo_status epo_build_dtf(epo_ctx* ctx, const uint8_t* d_edges_u8, float* d_dtf, __half* d_dtf_h);
+// pairs.cu
+epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,
+                           int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
+                           int32_t** out_src_inc, int2** out_work, int64_t* out_n_work);
+// lossgrad.cu
+epo_status epo_launch_loss_grad(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
+// update.cu
+epo_status epo_launch_update(epo_ctx* ctx);
+epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done, recompute `stopped`
+void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n);
+void epo_launch_f32_to_f64(cudaStream_t st, const float* in, double* out, int64_t n);
+void epo_launch_scatter_pair_outputs(cudaStream_t st, const float* pl, const int32_t* pv, const int32_t* perm,
+                                     float* out_pl, int32_t* out_pv, int64_t P);
