@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""Benchmark of the EPO hot path on B200 (contract: see the task prompt).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one iteration of the optimisation loop (rows a-1..a-12 of DESIGN.md): lambda/lr schedules,
+fused forward+backward over all pairs, per-camera reduction, Adam + SE(3) exponential, pose change and
+the stop test -- `epo_step(ctx, 1)`.  The workload is BASELINE.json config 3 (the "100 views" the metric
+names) unless --config says otherwise.  value = attempted edge-pixel reprojections per second
+(sum over directed pairs of the source's edge count, per step), inputs resident in HBM; L2 is flushed
+between timed steps.  e2e = the same metric through the C ABI with HOST buffers: epo_set_views
+(H2D + preprocessing) + epo_set_pairs + epo_step(iters) + epo_get_poses (D2H) inside the timed region.
+
+Multi-GPU: the path is not sharded in this tier ("replicas only"): under torchrun every rank
+runs the same workload on its own GPU and value is the sum over ranks / max time.
+--impl reference times the CPU oracle (oracle/), as it stands, on the host cores.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "edge-pixel reprojections/s (fused fwd+bwd)"
+UNIT = "reprojections/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--views", type=int, default=None, help="shrink the config (debugging only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--refine-iters", type=int, default=200)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(sc):
+    m = sc.meta
+    return (f"config{m['config']}:{sc.name} N={sc.n_views} {sc.W}x{sc.H} pairs={len(sc.pairs)} "
+            f"depth_noise={m['depth_noise']} outliers={m['outliers']} seed={m['seed']}")
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(np.max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def oracle_cfg_like_library():
+    """Oracle hyper-parameters = the library's fp32 defaults widened to double; fixed iteration count."""
+    import oracle
+    f = lambda x: float(np.float32(x))
+    return oracle.Config(lr_max=f(3e-3), beta1=f(0.9), beta2=f(0.999), adam_eps=f(1e-8), eps1=f(0.5), eps2=f(0.1),
+                         z_min=f(1e-6), early_stop=0)
+
+
+def cpu_baseline(sc, seconds_target=12.0):
+    """The oracle, as it stands, on the host cores: a bounded sample of the same workload (whole
+    iterations of Alg. 2 over all pairs until ~seconds_target of CPU time)."""
+    import oracle
+    t0 = time.time()
+    prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=float(np.float32(1e-6)))
+    t_pre = time.time() - t0
+    reproj = int(sum(prob.edge_off[s + 1] - prob.edge_off[s] for s, _ in sc.pairs))
+    opt = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_cfg_like_library())
+    iters = 0; t0 = time.time()
+    while True:
+        opt.run(1); iters += 1
+        dt = time.time() - t0
+        if dt >= seconds_target or iters >= 50:
+            break
+    return dict(value=reproj * iters / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample=f"{iters} whole iterations (all {len(sc.pairs)} pairs, {reproj} reprojections each) in {dt:.1f} s; "
+                       f"oracle preprocessing (edge lists + exact EDT) took {t_pre:.1f} s, not included"), prob
+
+
+def run_reference(args, sc):
+    """--impl reference: K timed steps of the oracle (one iteration of Alg. 2 each) on the host cores."""
+    import oracle
+    prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=float(np.float32(1e-6)))
+    reproj = int(sum(prob.edge_off[s + 1] - prob.edge_off[s] for s, _ in sc.pairs))
+    # bound the run to a few minutes: each step is a sample of `frac` of the pairs (whole pairs, list order)
+    probe = oracle.Optimizer(prob, sc.poses_init, sc.pairs[: max(1, len(sc.pairs) // 50)], oracle_cfg_like_library())
+    t0 = time.time(); probe.run(1); t_probe = time.time() - t0
+    r_probe = int(sum(prob.edge_off[s + 1] - prob.edge_off[s] for s, _ in probe.pairs))
+    est_full = t_probe * reproj / max(r_probe, 1)
+    budget = 150.0 / max(args.steps + args.warmup, 1)
+    frac = min(1.0, budget / max(est_full, 1e-9))
+    n_pairs = max(1, int(len(sc.pairs) * frac))
+    pairs = sc.pairs[:n_pairs]
+    r_step = int(sum(prob.edge_off[s + 1] - prob.edge_off[s] for s, _ in pairs))
+    opt = oracle.Optimizer(prob, sc.poses_init, pairs, oracle_cfg_like_library())
+    opt.run(args.warmup)
+    t0 = time.time(); opt.run(args.steps); dt = time.time() - t0
+    val = r_step * args.steps / dt
+    sample = f"each step = one oracle iteration over the first {n_pairs} of {len(sc.pairs)} pairs ({r_step} reprojections)"
+    line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * dt / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f64", data="synthetic", impl="reference",
+                config=dict(workload=workload_name(sc), sample=sample),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=oracle.num_threads(), kind="oracle", sample=sample),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from epo_scenes import make_scene
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args, make_scene(args.config, n_views=args.views))
+        return
+    import torch
+    import torch.distributed as dist
+    from paper_2607_00579_b200 import Epo, epo_config_default, build
+    if rank == 0:
+        build.build()
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist.barrier()
+    sc = make_scene(args.config, n_views=args.views)
+    stream = torch.cuda.current_stream()
+    cfg = epo_config_default(n_views=sc.n_views, width=sc.W, height=sc.H, early_stop=0, device=local,
+                             stream=stream.cuda_stream)
+    e = Epo(cfg)
+    # inputs resident in HBM before the timed region
+    dK, dP, dD, dE = (torch.from_numpy(a).cuda() for a in (sc.K, sc.poses_init, sc.depth, sc.edges))
+    dpairs = torch.from_numpy(sc.pairs).cuda()
+    torch.cuda.synchronize()
+    t0 = time.time(); e.set_views(dK, dP, dD, dE); torch.cuda.synchronize(); t_views = time.time() - t0
+    t0 = time.time(); e.set_pairs(dpairs); torch.cuda.synchronize(); t_pairs = time.time() - t0
+    reproj, _ = e.get_work()
+    edge_off = e.get_edge_counts()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def one_step(timed):
+        flush.zero_()                                                  # L2 flush, outside the events
+        if timed is not None:
+            timed[0].record(stream)
+        e.step(1, sync=False)
+        if timed is not None:
+            timed[1].record(stream)
+
+    for _ in range(args.warmup):
+        one_step(None)
+    e.reset()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    time.sleep(0.25)
+    _, k0 = e.get_work()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    for ev in evs:
+        one_step(ev)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    _, k1 = e.get_work()
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(step_ms))
+    # warm-L2 back-to-back steps and the fused kernel alone (roofline), still under the clock sampler
+    e.reset(); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(stream); e.step(args.steps, sync=False); b.record(stream); torch.cuda.synchronize()
+    warm_ms = a.elapsed_time(b) / args.steps
+    e.reset(); torch.cuda.synchronize()
+    k_ms_cold, k_min_cold = e.time_loss_grad_kernel(10.0, args.steps, True)
+    k_ms_warm, k_min_warm = e.time_loss_grad_kernel(10.0, args.steps, False)
+    clocks = sampler.stop()
+    got = e.loss_grad(10.0)
+    n_valid = int(got["pair_valid"].sum())
+    # full refinement: fixed number of iterations from the initial poses, one host sync at the end
+    e.reset(); torch.cuda.synchronize()
+    a.record(stream); done, phase = e.step(args.refine_iters); b.record(stream); torch.cuda.synchronize()
+    refine_s = a.elapsed_time(b) / 1e3
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); total_ms = float(t.item())
+    value = world * reproj * args.steps / (total_ms / 1e3)
+
+    # e2e through the C ABI with pinned HOST buffers (H2D + preprocessing + pairs + iterations + D2H)
+    e2e = None
+    if not args.no_e2e:
+        hK, hP, hD, hE = (torch.from_numpy(x).pin_memory() for x in (sc.K, sc.poses_init, sc.depth, sc.edges))
+        hpairs = torch.from_numpy(sc.pairs).pin_memory()
+        hout = torch.empty((sc.n_views, 12), dtype=torch.float32).pin_memory()
+        times = []
+        for rep in range(3):
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            e2 = Epo(cfg)
+            e2.set_views(hK, hP, hD, hE); e2.set_pairs(hpairs)
+            d2, _ = e2.step(args.refine_iters)
+            e2.get_poses(hout)
+            torch.cuda.synchronize(); times.append(time.perf_counter() - t0)
+            e2.destroy()
+        t_e2e = min(times[1:]) if len(times) > 1 else times[0]
+        h2d = sum(int(x.numel() * x.element_size()) for x in (hK, hP, hD, hE, hpairs))
+        e2e = dict(value=world * reproj * args.refine_iters / t_e2e, unit=UNIT, h2d_bytes_per_step=h2d,
+                   d2h_bytes_per_step=int(hout.numel() * 4) + 8, seconds=t_e2e,
+                   what=f"epo_create + epo_set_views(host) + epo_set_pairs(host) + epo_step({args.refine_iters}) + epo_get_poses(host)")
+
+    if rank != 0:
+        return
+    peak, peak_src = peaks()
+    alg_bytes = 8.0 * reproj + 16.0 * n_valid          # 8 B record per attempted + 16 B of taps per valid
+    ach = alg_bytes / (k_ms_cold / 1e3) / 1e9
+    line = dict(
+        metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+        ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+        data="synthetic",
+        config=dict(workload=workload_name(sc), l2="flushed between timed steps (256 MiB write)",
+                    reprojections_per_step=reproj, valid_per_step=n_valid, valid_fraction=n_valid / max(reproj, 1),
+                    edge_pixels=int(edge_off[-1]), parallelism="replicas only" if world > 1 else "1 GPU"),
+        clocks=clocks, gpu_launches=int(k1 - k0),
+        roofline=dict(bound="hbm", achieved=ach, peak=peak, unit="GB/s", frac=ach / peak, traffic=None,
+                      kernel="k_loss_grad<float>", kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
+                      algorithmic_bytes=alg_bytes, peak_source=peak_src,
+                      note="algorithmic bytes = 8 B x attempted + 16 B x valid reprojections (DESIGN.md)"),
+        warm_l2=dict(ms_per_step=warm_ms, value=world * reproj / (warm_ms / 1e3)),
+        refinement=dict(iters=int(done), seconds=refine_s, views=sc.n_views),
+        preprocessing=dict(set_views_s=t_views, set_pairs_s=t_pairs),
+    )
+    if e2e:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"], _ = cpu_baseline(sc)
+    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(prof):
+        try:
+            line["roofline"]["traffic"] = json.load(open(prof)).get(f"config{args.config}")
+        except Exception:
+            pass
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

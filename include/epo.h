@@ -145,6 +145,13 @@ EPO_API epo_status epo_get_trace(epo_ctx* ctx, int32_t first, int32_t count, flo
 /* attempted reprojections per evaluation = sum over pairs of the source's edge count */
 EPO_API epo_status epo_get_work(epo_ctx* ctx, int64_t* reprojections_per_eval, int64_t* kernel_launches_so_far);
 
+/* Measurement hook (bench.py "roofline"): launch ONLY the fused loss+gradient kernel `reps` times on
+ * cfg.stream at the current poses, each launch bracketed by CUDA events recorded on that stream; if
+ * flush_l2, a buffer larger than the L2 is overwritten before each launch (outside the events).
+ * Returns the mean and minimum launch duration in milliseconds (host pointers, nullable). Synchronises. */
+EPO_API epo_status epo_time_loss_grad_kernel(epo_ctx* ctx, float lambda, int32_t reps, int32_t flush_l2,
+                                             float* ms_mean, float* ms_min);
+
 EPO_API const char* epo_last_error(const epo_ctx* ctx);
 EPO_API const char* epo_version(void);
 

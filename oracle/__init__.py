@@ -37,7 +37,7 @@ class _Cfg(C.Structure):
                 ("max_steps", C.c_int32), ("beta1", C.c_double), ("beta2", C.c_double),
                 ("adam_eps", C.c_double), ("eps1", C.c_double), ("eps2", C.c_double), ("w1", C.c_int32),
                 ("w2", C.c_int32), ("smooth_window", C.c_int32), ("early_stop", C.c_int32),
-                ("z_min", C.c_double)]
+                ("z_min", C.c_double), ("coord_fp32", C.c_int32)]
 
 
 @dataclass
@@ -60,6 +60,7 @@ class Config:
     smooth_window: int = 1
     early_stop: int = 0
     z_min: float = 1e-6
+    coord_fp32: int = 0      # 1: projected positions decided in fp32 (reading P1)
 
     def c(self) -> _Cfg:
         return _Cfg(**{f[0]: getattr(self, f[0]) for f in _Cfg._fields_})
@@ -93,12 +94,12 @@ def lib():
         L.orc_pair_loss_grad.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint16), C.POINTER(C.c_float),
                                          C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
                                          C.POINTER(C.c_double), C.POINTER(C.c_float), C.c_double, C.c_double,
-                                         C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int32),
+                                         C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int32),
                                          C.POINTER(C.c_double), C.POINTER(C.c_int32)]
         L.orc_loss_grad.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
                                     C.POINTER(C.c_int32), C.POINTER(C.c_uint16), C.POINTER(C.c_float),
                                     C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_int32), C.c_double,
-                                    C.c_double, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int32),
+                                    C.c_double, C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int32),
                                     C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_double),
                                     C.POINTER(C.c_double)]
         L.orc_run.restype = C.c_int
@@ -211,7 +212,7 @@ def relative_pose(Ts, Tt):
 
 
 # ------------------------------------------------------------------------------------------- O4-O6
-def pair_loss_grad(uv, z, Ks, Kt, Ts, Tt, dtf_t, lam, delta=1.0, z_min=1e-6):
+def pair_loss_grad(uv, z, Ks, Kt, Ts, Tt, dtf_t, lam, delta=1.0, z_min=1e-6, coord_fp32=0):
     """One directed pair: (sum_rho, n_valid, G[12] = [tgt(v,w), src(v,w)] un-normalised, near[2])."""
     H, W = dtf_t.shape
     uv = np.ascontiguousarray(uv, np.uint16); z = np.ascontiguousarray(z, np.float32)
@@ -219,7 +220,7 @@ def pair_loss_grad(uv, z, Ks, Kt, Ts, Tt, dtf_t, lam, delta=1.0, z_min=1e-6):
     S = C.c_double(); nv = C.c_int32(); G = np.empty(12); near = np.zeros(2, np.int32)
     lib().orc_pair_loss_grad(W, H, len(z), _p(uv, C.c_uint16), _p(z, C.c_float), _p(_d(Ks, 4), C.c_double),
                              _p(_d(Kt, 4), C.c_double), _p(_d(Ts, 12), C.c_double), _p(_d(Tt, 12), C.c_double),
-                             _p(dtf_t, C.c_float), lam, delta, z_min, C.byref(S), C.byref(nv),
+                             _p(dtf_t, C.c_float), lam, delta, z_min, coord_fp32, C.byref(S), C.byref(nv),
                              _p(G, C.c_double), _p(near, C.c_int32))
     return S.value, nv.value, G, near
 
@@ -249,7 +250,7 @@ def preprocess(K, depth, edges, z_min=1e-6, e_max=0, half=False) -> Problem:
     return Problem(W, H, np.ascontiguousarray(K, np.float32), off, uv, z, dtf)
 
 
-def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair_G=False):
+def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair_G=False, coord_fp32=0):
     """Returns dict(loss, pair_loss [P], pair_valid [P], grad [N,6], near [P,2], pair_G [P,12]?)."""
     N = prob.n_views
     poses = np.ascontiguousarray(np.asarray(poses, np.float64).reshape(N, 12))
@@ -259,7 +260,7 @@ def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair
     grad = np.empty((N, 6)); L = C.c_double()
     lib().orc_loss_grad(N, prob.W, prob.H, _p(prob.K, C.c_float), _p(poses, C.c_double),
                         _p(prob.edge_off, C.c_int32), _p(prob.uv, C.c_uint16), _p(prob.z, C.c_float),
-                        _p(prob.dtf, C.c_float), P, _p(pairs, C.c_int32), lam, delta, z_min,
+                        _p(prob.dtf, C.c_float), P, _p(pairs, C.c_int32), lam, delta, z_min, coord_fp32,
                         _p(pl, C.c_double), _p(pv, C.c_int32), _p(pG, C.c_double), _p(near, C.c_int32),
                         _p(grad, C.c_double), C.byref(L))
     return dict(loss=L.value, pair_loss=pl, pair_valid=pv, grad=grad, near=near, pair_G=pG)

@@ -225,12 +225,88 @@ void orc_relative_pose(const double Ts[12], const double Tt[12], double Tts[12])
  * near[0] counts samples within 1e-3 px (or 1e-3 in z) of the validity border, near[1] those with
  * |d - lambda| < 1e-3 or |d - delta| < 1e-3 -- the discrete events of "Tolerance realism".
  * ================================================================================================= */
+/* Variant "coord_fp32" (reading P1).  The paper computes the geometry in FP32, and
+ * the projected position decides three integers per sample -- valid or not, and the bilinear cell (x0, y0) --
+ * at which the gradient is discontinuous.  Deciding them in double here and in fp32 on the GPU flips a few
+ * samples per 10^5 (those within ~3e-5 px of a cell or image border), each worth ~1/n_valid of a pair's
+ * gradient.  In this variant steps a-2..a-4 (back-project, transform, project) are therefore evaluated in
+ * IEEE binary32 with the operation order stated below (every operation individually rounded; fmaf is the
+ * correctly rounded fused multiply-add), and everything after the position (weights, interpolation, robust
+ * loss, Jacobian, sums) continues in double exactly as in the default path.
+ *   T_ts, K rounded once to float;  ifx = 1/fx_s, ify = 1/fy_s
+ *   x_s = Z ((u - cx_s) ifx), y_s = Z ((v - cy_s) ify), z_s = Z
+ *   X = fma(r00, x_s, fma(r01, y_s, fma(r02, z_s, t_x)))   (same for Y, Z)
+ *   iz = 1/Z ;  x = fma(fx_t X, iz, cx_t) ;  y = fma(fy_t Y, iz, cy_t)
+ */
+static void orc_pair_loss_grad_f32coords(int W, int H, int n_edges, const uint16_t* uv, const float* z,
+                                         const double Ks[4], const double Kt[4], const double Tts[12],
+                                         const float* dtf_t, double lambda, double delta, double z_min,
+                                         double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2]) {
+  float T[12];
+  for (int k = 0; k < 12; ++k) T[k] = (float)Tts[k];
+  const float ifx = 1.0f / (float)Ks[0], ify = 1.0f / (float)Ks[1], cxs = (float)Ks[2], cys = (float)Ks[3];
+  const float fxt = (float)Kt[0], fyt = (float)Kt[1], cxt = (float)Kt[2], cyt = (float)Kt[3];
+  const float zmin = (float)z_min, xmax = (float)(W - 1), ymax = (float)(H - 1);
+  double S = 0.0; int32_t nv = 0;
+  for (int k = 0; k < 12; ++k) G[k] = 0.0;
+  near[0] = near[1] = 0;
+  for (int e = 0; e < n_edges; ++e) {
+    const float u = (float)uv[2 * e], v = (float)uv[2 * e + 1], Zs = z[e];
+    const float a_ = (u - cxs) * ifx, b_ = (v - cys) * ify;
+    const float xsf = Zs * a_, ysf = Zs * b_, zsf = Zs;
+    const float Xf = fmaf(T[0], xsf, fmaf(T[1], ysf, fmaf(T[2], zsf, T[3])));
+    const float Yf = fmaf(T[4], xsf, fmaf(T[5], ysf, fmaf(T[6], zsf, T[7])));
+    const float Zf = fmaf(T[8], xsf, fmaf(T[9], ysf, fmaf(T[10], zsf, T[11])));
+    if (!(Zf > zmin)) continue;
+    const float izf = 1.0f / Zf;
+    const float fxX = fxt * Xf, fyY = fyt * Yf;
+    const float xf = fmaf(fxX, izf, cxt), yf = fmaf(fyY, izf, cyt);
+    if (!(xf >= 0.0f && xf <= xmax && yf >= 0.0f && yf <= ymax)) continue;
+    /* from here on: the default path, in double, on the fp32 position */
+    const double xs[3] = { xsf, ysf, zsf }, xt[3] = { Xf, Yf, Zf };
+    const double x = xf, y = yf;
+    int x0 = (int)floor(x), y0 = (int)floor(y);
+    if (x0 > W - 2) x0 = W - 2;
+    if (y0 > H - 2) y0 = H - 2;
+    double wx = x - x0, wy = y - y0;
+    double D00 = dtf_t[(size_t)y0 * W + x0], D01 = dtf_t[(size_t)y0 * W + x0 + 1];
+    double D10 = dtf_t[(size_t)(y0 + 1) * W + x0], D11 = dtf_t[(size_t)(y0 + 1) * W + x0 + 1];
+    double d = (1.0 - wy) * ((1.0 - wx) * D00 + wx * D01) + wy * ((1.0 - wx) * D10 + wx * D11);
+    double ddx = (1.0 - wy) * (D01 - D00) + wy * (D11 - D10);
+    double ddy = (1.0 - wx) * (D10 - D00) + wx * (D11 - D01);
+    if (fabs(d - lambda) < 1e-3 || fabs(d - delta) < 1e-3) near[1]++;
+    double dhat = d < lambda ? d : lambda;
+    double rho = dhat <= delta ? 0.5 * dhat * dhat : delta * (dhat - 0.5 * delta);
+    double drho = (d <= lambda) ? (d < delta ? d : delta) : 0.0;
+    S += rho; nv++;
+    double iz = 1.0 / xt[2];
+    double a[3], b[3];
+    a[0] = drho * ddx * Kt[0] * iz;
+    a[1] = drho * ddy * Kt[1] * iz;
+    a[2] = -drho * (ddx * Kt[0] * xt[0] + ddy * Kt[1] * xt[1]) * iz * iz;
+    G[0] += a[0]; G[1] += a[1]; G[2] += a[2];
+    G[3] += xt[1] * a[2] - xt[2] * a[1];
+    G[4] += xt[2] * a[0] - xt[0] * a[2];
+    G[5] += xt[0] * a[1] - xt[1] * a[0];
+    for (int i = 0; i < 3; ++i) b[i] = Tts[i] * a[0] + Tts[4 + i] * a[1] + Tts[8 + i] * a[2];
+    G[6] -= b[0]; G[7] -= b[1]; G[8] -= b[2];
+    G[9]  -= xs[1] * b[2] - xs[2] * b[1];
+    G[10] -= xs[2] * b[0] - xs[0] * b[2];
+    G[11] -= xs[0] * b[1] - xs[1] * b[0];
+  }
+  *sum_rho = S; *n_valid = nv;
+}
+
 void orc_pair_loss_grad(int W, int H, int n_edges, const uint16_t* uv, const float* z,
                         const double Ks[4], const double Kt[4], const double Ts[12], const double Tt[12],
-                        const float* dtf_t, double lambda, double delta, double z_min,
+                        const float* dtf_t, double lambda, double delta, double z_min, int coord_fp32,
                         double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2]) {
   double Tts[12];
   orc_relative_pose(Ts, Tt, Tts);
+  if (coord_fp32) {
+    orc_pair_loss_grad_f32coords(W, H, n_edges, uv, z, Ks, Kt, Tts, dtf_t, lambda, delta, z_min, sum_rho, n_valid, G, near);
+    return;
+  }
   double S = 0.0; int32_t nv = 0;
   for (int k = 0; k < 12; ++k) G[k] = 0.0;
   near[0] = near[1] = 0;
@@ -288,8 +364,8 @@ void orc_pair_loss_grad(int W, int H, int n_edges, const uint16_t* uv, const flo
  * ================================================================================================= */
 void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, const int32_t* edge_off,
                    const uint16_t* uv, const float* z, const float* dtf, int64_t P, const int32_t* pairs,
-                   double lambda, double delta, double z_min, double* pair_loss, int32_t* pair_valid,
-                   double* pair_G, int32_t* near, double* grad, double* loss) {
+                   double lambda, double delta, double z_min, int coord_fp32, double* pair_loss,
+                   int32_t* pair_valid, double* pair_G, int32_t* near, double* grad, double* loss) {
   double* Gall = (double*)malloc((size_t)P * 12 * sizeof(double));
 #pragma omp parallel for schedule(dynamic, 1)
   for (int64_t p = 0; p < P; ++p) {
@@ -298,7 +374,7 @@ void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, con
     for (int i = 0; i < 4; ++i) { Ks[i] = K[4 * s + i]; Kt[i] = K[4 * t + i]; }
     orc_pair_loss_grad(W, H, edge_off[s + 1] - edge_off[s], uv + 2 * (size_t)edge_off[s], z + edge_off[s],
                        Ks, Kt, poses + 12 * (size_t)s, poses + 12 * (size_t)t, dtf + (size_t)t * W * H,
-                       lambda, delta, z_min, &S, &nv, Gall + 12 * p, nr);
+                       lambda, delta, z_min, coord_fp32, &S, &nv, Gall + 12 * p, nr);
     pair_loss[p] = nv > 0 ? S / nv : 0.0;
     pair_valid[p] = nv;
     if (near) { near[2 * p] = nr[0]; near[2 * p + 1] = nr[1]; }
@@ -438,6 +514,7 @@ typedef struct {
   double lr_max; int32_t warmup_steps, max_steps;
   double beta1, beta2, adam_eps, eps1, eps2; int32_t w1, w2, smooth_window, early_stop;
   double z_min;
+  int32_t coord_fp32;   /* 0: everything in double; 1: projected positions decided in fp32 (reading P1) */
 } orc_config;
 
 /* =================================================================================================
@@ -461,7 +538,7 @@ int orc_run(const orc_config* cfg, int n_iters, int N, int W, int H, const float
     int s = *step; double L;
     double lambda = orc_lambda(s, cfg->clamp_start, cfg->clamp_end, cfg->clamp_steps);
     orc_loss_grad(N, W, H, K, poses, edge_off, uv, z, dtf, P, pairs, lambda, cfg->huber_delta, cfg->z_min,
-                  pl, pv, NULL, NULL, g, &L);
+                  cfg->coord_fp32, pl, pv, NULL, NULL, g, &L);
     trace_loss[s] = L;
     orc_adam(6 * N, g, m, v, s, orc_lr(s, cfg->lr_max, cfg->warmup_steps, cfg->max_steps), cfg->beta1,
              cfg->beta2, cfg->adam_eps, eps);

@@ -436,6 +436,44 @@ epo_status epo_get_trace(epo_ctx* c, int32_t first, int32_t count, float* loss, 
   return EPO_OK;
 }
 
+epo_status epo_time_loss_grad_kernel(epo_ctx* c, float lambda, int32_t reps, int32_t flush_l2, float* ms_mean,
+                                     float* ms_min) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_time_loss_grad_kernel before set_views/set_pairs");
+  if (reps < 1 || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_time_loss_grad_kernel: bad argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t flush_bytes = (size_t)256 << 20;   // > 126 MB L2
+  void* flush = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (flush_l2) EPO_CUDA(c, cudaMalloc(&flush, flush_bytes));
+  cudaError_t e = cudaEventCreate(&e0);
+  if (e == cudaSuccess) e = cudaEventCreate(&e1);
+  double sum = 0.0; float mn = 1e30f;
+  epo_status rc = EPO_OK;
+  for (int r = 0; r < reps && e == cudaSuccess && rc == EPO_OK; ++r) {
+    if (flush) e = cudaMemsetAsync(flush, r & 0xff, flush_bytes, st);
+    if (e == cudaSuccess) e = cudaEventRecord(e0, st);
+    if (e == cudaSuccess) rc = epo_launch_fused_only(c, lambda);
+    if (e == cudaSuccess) e = cudaEventRecord(e1, st);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    sum += ms; if (ms < mn) mn = ms;
+  }
+  // leave the accumulators clean for the next evaluation
+  if (e == cudaSuccess) e = cudaMemsetAsync(c->d_acc, 0, (size_t)c->P * kAccStride * sizeof(double), st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(flush);
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  if (rc != EPO_OK) return rc;
+  if (e != cudaSuccess) return epo_fail(c, EPO_ERR_CUDA, "epo_time_loss_grad_kernel: %s", cudaGetErrorString(e));
+  if (ms_mean) *ms_mean = (float)(sum / reps);
+  if (ms_min) *ms_min = mn;
+  return EPO_OK;
+}
+
 epo_status epo_get_work(epo_ctx* c, int64_t* reprojections_per_eval, int64_t* kernel_launches_so_far) {
   if (!c) return EPO_ERR_INVALID_ARG;
   if (reprojections_per_eval) *reprojections_per_eval = c->have_pairs ? c->reproj_per_eval : 0;

@@ -111,6 +111,7 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P,
                            int32_t** out_src_inc, int2** out_work, int64_t* out_n_work);
 // lossgrad.cu
 epo_status epo_launch_loss_grad(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
+epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)
 // update.cu
 epo_status epo_launch_update(epo_ctx* ctx);
 epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done, recompute `stopped`
