@@ -38,16 +38,18 @@ cudaError_t copy_out(void* dst, const void* src, size_t bytes, cudaStream_t st, 
 }
 
 void free_views(epo_ctx* c) {
-  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_dtf); cudaFree(c->d_dtf_h);
-  c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_dtf = nullptr; c->d_dtf_h = nullptr;
+  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_dtf); cudaFree(c->d_dtf_h); cudaFree(c->d_pts);
+  epo_free_atlas(c->dtf_atlas, c->dtf_tex);
+  c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_dtf = nullptr; c->d_dtf_h = nullptr; c->d_pts = nullptr;
+  c->dtf_atlas = nullptr; c->dtf_tex = 0;
   c->have_views = false;
 }
 void free_pairs(epo_ctx* c) {
   cudaFree(c->d_pairs); cudaFree(c->d_perm); cudaFree(c->d_tgt_off); cudaFree(c->d_src_off); cudaFree(c->d_src_inc);
-  cudaFree(c->d_work); cudaFree(c->d_acc); cudaFree(c->d_pair_loss); cudaFree(c->d_pair_valid); cudaFree(c->d_out_f);
+  cudaFree(c->d_work); cudaFree(c->d_work_off); cudaFree(c->d_part); cudaFree(c->d_pair_loss); cudaFree(c->d_pair_valid); cudaFree(c->d_out_f);
   cudaFree(c->d_out_i);
   c->d_pairs = nullptr; c->d_perm = nullptr; c->d_tgt_off = nullptr; c->d_src_off = nullptr; c->d_src_inc = nullptr;
-  c->d_work = nullptr; c->d_acc = nullptr; c->d_pair_loss = nullptr; c->d_pair_valid = nullptr; c->d_out_f = nullptr;
+  c->d_work = nullptr; c->d_work_off = nullptr; c->d_part = nullptr; c->d_pair_loss = nullptr; c->d_pair_valid = nullptr; c->d_out_f = nullptr;
   c->d_out_i = nullptr;
   c->have_pairs = false; c->P = 0; c->n_work = 0;
 }
@@ -171,13 +173,25 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff);
   if (rc == EPO_OK) rc = epo_build_dtf(c, d_e, d_dtf, d_dtf_h);
   cudaFree(d_depth); cudaFree(d_e);
+  float* d_Ktmp = nullptr; float4* pts = nullptr;
+  cudaArray_t atlas = nullptr; cudaTextureObject_t tex = 0; int cols = 1;
+  if (rc == EPO_OK) {
+    e = cudaMalloc(&d_Ktmp, N * 4 * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_Ktmp, hK.data(), N * 4 * sizeof(float), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
+  }
+  if (rc == EPO_OK) rc = epo_build_points(c, d_Ktmp, off, rec, E, hoff, &pts);
+  if (rc == EPO_OK) rc = epo_build_atlas(c, d_dtf, d_dtf_h, &atlas, &tex, &cols);
   if (rc != EPO_OK) {
+    cudaStreamSynchronize(st);
     cudaGetLastError();
-    cudaFree(d_dtf); cudaFree(d_dtf_h); cudaFree(d_pose_f); cudaFree(off); cudaFree(rec);
+    cudaFree(d_dtf); cudaFree(d_dtf_h); cudaFree(d_pose_f); cudaFree(off); cudaFree(rec); cudaFree(d_Ktmp); cudaFree(pts);
     return rc;
   }
+  cudaFree(d_Ktmp);   // epo_build_atlas synchronised the stream: k_make_points has finished
   free_pairs(c); free_views(c);
   c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff; c->d_dtf = d_dtf; c->d_dtf_h = d_dtf_h;
+  c->d_pts = pts; c->dtf_atlas = atlas; c->dtf_tex = tex; c->atlas_cols = cols;
   EPO_CUDA(c, cudaMemcpyAsync(c->d_K, hK.data(), N * 4 * sizeof(float), cudaMemcpyHostToDevice, st));
   EPO_CUDA(c, cudaMemcpyAsync(d_pose_f, hP.data(), N * 12 * sizeof(float), cudaMemcpyHostToDevice, st));
   epo_launch_f32_to_f64(st, d_pose_f, c->d_poses_init, (int64_t)N * 12);
@@ -209,16 +223,16 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   int32_t* d_user = nullptr;
   EPO_CUDA(c, cudaMalloc(&d_user, (size_t)P * 2 * sizeof(int32_t)));
   cudaError_t e = cudaMemcpyAsync(d_user, hp.data(), (size_t)P * 2 * sizeof(int32_t), cudaMemcpyHostToDevice, st);
-  int2 *canon = nullptr, *work = nullptr; int32_t *perm = nullptr, *toff = nullptr, *soff = nullptr, *sinc = nullptr;
+  int2 *canon = nullptr, *work = nullptr; int32_t *perm = nullptr, *toff = nullptr, *soff = nullptr, *sinc = nullptr, *woff = nullptr;
   int64_t n_work = 0;
-  epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &n_work)
+  epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &woff, &n_work)
                                      : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
   cudaFree(d_user);
   double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
   if (rc == EPO_OK) {
     // output staging: [loss | grad 6N | pair_loss P | loss trace | theta trace]
     size_t nf = 1 + (size_t)c->N * 6 + (size_t)P + (size_t)c->cfg.max_steps * 2;
-    e = cudaMalloc(&acc, (size_t)P * kAccStride * sizeof(double));
+    e = cudaMalloc(&acc, (size_t)(n_work > 0 ? n_work : 1) * kAccStride * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&pl, (size_t)P * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&pv, (size_t)P * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMalloc(&of, nf * sizeof(float));
@@ -229,13 +243,13 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   }
   if (rc != EPO_OK) {
     cudaGetLastError();
-    cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(toff); cudaFree(soff); cudaFree(sinc);
+    cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(toff); cudaFree(soff); cudaFree(sinc); cudaFree(woff);
     cudaFree(acc); cudaFree(pl); cudaFree(pv); cudaFree(of); cudaFree(oi);
     return rc;
   }
   free_pairs(c);
   c->d_pairs = canon; c->d_perm = perm; c->d_tgt_off = toff; c->d_src_off = soff; c->d_src_inc = sinc; c->d_work = work;
-  c->n_work = n_work; c->P = P; c->d_acc = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
+  c->d_work_off = woff; c->n_work = n_work; c->P = P; c->d_part = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
   c->h_pairs.swap(hp); c->reproj_per_eval = reproj;
   c->have_pairs = true;
   EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, (size_t)c->N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
@@ -461,8 +475,6 @@ epo_status epo_time_loss_grad_kernel(epo_ctx* c, float lambda, int32_t reps, int
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
     sum += ms; if (ms < mn) mn = ms;
   }
-  // leave the accumulators clean for the next evaluation
-  if (e == cudaSuccess) e = cudaMemsetAsync(c->d_acc, 0, (size_t)c->P * kAccStride * sizeof(double), st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(flush);
   if (e0) cudaEventDestroy(e0);

@@ -16,8 +16,8 @@ struct __align__(8) EdgeRec {
   float z;
 };
 
-// Per-pair accumulators written by the fused kernel (row a-8): S = sum rho, n = valid count,
-// A = sum a, M = sum x_t x a (six-accumulator identity I1).  fp64, 64 bytes per pair.
+// Partial sums written by each CTA of the fused kernel (row a-8): S = sum rho, n = valid count,
+// A = sum a, M = sum x_t x a (six-accumulator identity I1).  fp64, 64 bytes per work item.
 constexpr int kAccStride = 8;
 
 // Edge pixels handled by one CTA of the fused kernel: kLgThreads threads x kLgPerThread samples.
@@ -48,8 +48,12 @@ struct epo_ctx {
   double* d_poses_init;   // [N][12] as given to epo_set_views / epo_reset
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
-  float* d_dtf;           // [N][H][W] fp32 field (always kept: epo_get_dtf, fp32 kernel)
+  float4* d_pts;          // [E] camera-frame points (x_s, y_s, z_s, 0): K and Z are fixed, so row a-2 is hoisted
+  float* d_dtf;           // [N][H][W] fp32 field, pitch-linear (epo_get_dtf; source of the texture copies)
   __half* d_dtf_h;        // [N][H][W] fp16 field when cfg.dtf_format == 1
+  cudaArray_t dtf_atlas;                      // block-linear, gather-enabled copy of all fields: views tiled in a grid
+  cudaTextureObject_t dtf_tex;                // texture object on the atlas (what the fused kernel samples)
+  int atlas_cols;                             // view i sits at texel offset ((i % cols) W, (i / cols) H)
   std::vector<int32_t> h_edge_off;
 
   // pairs
@@ -59,10 +63,11 @@ struct epo_ctx {
   int32_t* d_src_off;     // [N+1]
   int32_t* d_src_inc;     // [P] canonical ids grouped by source, ascending
   int2* d_work;           // [n_work] (canonical pair, first edge index of the chunk)
+  int32_t* d_work_off;    // [P+1] first work item of each canonical pair
   std::vector<int32_t> h_pairs;   // user order, for reprojection counting
 
   // per-evaluation buffers
-  double* d_acc;          // [P][8]
+  double* d_part;         // [n_work][8] per-CTA partial sums {S, n, A[3], M[3]} (no atomics: reproducible)
   float* d_pair_loss;     // [P] canonical order
   int32_t* d_pair_valid;  // [P]
   double* d_grad;         // [N][6]
@@ -105,10 +110,15 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
                                 int32_t** out_off, EdgeRec** out_rec, int64_t* out_E,
                                 std::vector<int32_t>* h_off);
 epo_status epo_build_dtf(epo_ctx* ctx, const uint8_t* d_edges_u8, float* d_dtf, __half* d_dtf_h);
+epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
+                            const std::vector<int32_t>& h_off, float4** out_pts);
+epo_status epo_build_atlas(epo_ctx* ctx, const float* d_dtf, const __half* d_dtf_h, cudaArray_t* atlas,
+                           cudaTextureObject_t* tex, int* cols);
+void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex);
 // pairs.cu
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
-                           int32_t** out_src_inc, int2** out_work, int64_t* out_n_work);
+                           int32_t** out_src_inc, int2** out_work, int32_t** out_work_off, int64_t* out_n_work);
 // lossgrad.cu
 epo_status epo_launch_loss_grad(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)

@@ -101,16 +101,16 @@ __global__ void k_fill_work(const int32_t* __restrict__ work_off, int64_t P, int
 
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2** out_pairs, int32_t** out_perm,
                            int32_t** out_tgt_off, int32_t** out_src_off, int32_t** out_src_inc, int2** out_work,
-                           int64_t* out_n_work) {
+                           int32_t** out_work_off, int64_t* out_n_work) {
   const int N = ctx->N;
   cudaStream_t st = ctx->stream;
   int2 *canon = nullptr, *work = nullptr;
   int32_t *perm = nullptr, *tgt_off = nullptr, *src_off = nullptr, *src_inc = nullptr;
   int32_t *cnt = nullptr, *cursor = nullptr, *bucket = nullptr, *chunk_cnt = nullptr, *work_off = nullptr;
   auto free_all = [&]() {
-    cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(tgt_off); cudaFree(src_off); cudaFree(src_inc);
+    cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(tgt_off); cudaFree(src_off); cudaFree(src_inc); cudaFree(work_off);
   };
-  auto free_tmp = [&]() { cudaFree(cnt); cudaFree(cursor); cudaFree(bucket); cudaFree(chunk_cnt); cudaFree(work_off); };
+  auto free_tmp = [&]() { cudaFree(cnt); cudaFree(cursor); cudaFree(bucket); cudaFree(chunk_cnt); };
 #define PR_CUDA(call)                                                                                \
   do {                                                                                               \
     cudaError_t e_ = (call);                                                                         \
@@ -161,6 +161,6 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
   free_tmp();
 #undef PR_CUDA
   *out_pairs = canon; *out_perm = perm; *out_tgt_off = tgt_off; *out_src_off = src_off; *out_src_inc = src_inc;
-  *out_work = work; *out_n_work = n_work;
+  *out_work = work; *out_work_off = work_off; *out_n_work = n_work;
   return EPO_OK;
 }

@@ -3,6 +3,7 @@
 //   PAPER.md:374-376 (Alg. 1 l.6)  "Canny edges, sub-sampled to <= E_max points / image"
 //   PAPER.md:378-379 (Alg. 1 l.7), 396  "exact L2 distance transform [14]" kept on the GPU
 #include <climits>
+#include <cstring>
 
 #include "epo_internal.h"
 
@@ -211,6 +212,24 @@ __global__ void k_edt_cols(const int32_t* __restrict__ g, int W, int H, float* _
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// a-2 hoisted: camera-frame point of every edge pixel, x_s = Z ((u - cx) (1/fx)), y_s likewise, z_s = Z
+// (K and Z are not optimised on this path, so the point is iteration-invariant).
+// The operation order is the one the fp32-position reading (P1) states.
+// ---------------------------------------------------------------------------------------------
+__global__ void k_make_points(const EdgeRec* __restrict__ rec, const int32_t* __restrict__ off,
+                              const float* __restrict__ K, float4* __restrict__ pts) {
+  const int view = blockIdx.y;
+  const int lo = off[view], n = off[view + 1] - lo;
+  const float ifx = 1.0f / K[4 * view], ify = 1.0f / K[4 * view + 1], cx = K[4 * view + 2], cy = K[4 * view + 3];
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+    const EdgeRec r = rec[lo + e];
+    const float u = (float)(r.uv & 0xffffu), v = (float)(r.uv >> 16);
+    pts[lo + e] = make_float4(r.z * ((u - cx) * ifx), r.z * ((v - cy) * ify), r.z, 0.f);
+  }
+}
+
+
 }  // namespace
 
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
@@ -308,5 +327,64 @@ epo_status epo_build_dtf(epo_ctx* ctx, const uint8_t* d_edges_u8, float* d_dtf, 
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
   cudaFree(g);
   if (e != cudaSuccess) return epo_fail(ctx, EPO_ERR_CUDA, "EDT kernels failed: %s", cudaGetErrorString(e));
+  return EPO_OK;
+}
+
+epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
+                            const std::vector<int32_t>& h_off, float4** out_pts) {
+  float4* pts = nullptr;
+  EPO_CUDA(ctx, cudaMalloc(&pts, (size_t)(E > 0 ? E : 1) * sizeof(float4)));
+  int max_n = 1;
+  for (int i = 0; i < ctx->N; ++i) max_n = h_off[i + 1] - h_off[i] > max_n ? h_off[i + 1] - h_off[i] : max_n;
+  dim3 grid((max_n + 255) / 256, ctx->N);
+  k_make_points<<<grid, 256, 0, ctx->stream>>>(d_rec, d_off, d_K, pts);
+  ctx->launches += 1;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { cudaFree(pts); return epo_fail(ctx, EPO_ERR_CUDA, "k_make_points: %s", cudaGetErrorString(e)); }
+  *out_pts = pts;
+  return EPO_OK;
+}
+
+void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex) {
+  if (tex) cudaDestroyTextureObject(tex);
+  if (atlas) cudaFreeArray(atlas);
+}
+
+// Block-linear, gather-enabled copy of the distance fields: ONE 2-D CUDA array holding all views tiled in a
+// grid (view i at texel offset ((i % cols) W, (i / cols) H)) behind one texture object.  The fused kernel
+// fetches the 2x2 bilinear footprint with ONE tld4 (tex2Dgather) and applies the exact fp32 weights itself;
+// the hardware's 8-bit-fraction filtering is never used.  A footprint never leaves its view (x0 <= W-2).
+epo_status epo_build_atlas(epo_ctx* ctx, const float* d_dtf, const __half* d_dtf_h, cudaArray_t* atlas_out,
+                           cudaTextureObject_t* tex_out, int* cols_out) {
+  const int N = ctx->N, W = ctx->W, H = ctx->H;
+  const bool half = d_dtf_h != nullptr;
+  int cols = 32768 / W; if (cols < 1) cols = 1; if (cols > N) cols = N;
+  const int rows = (N + cols - 1) / cols;
+  if ((int64_t)rows * H > 65536 || (int64_t)cols * W > 131072)
+    return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "%d views of %dx%d do not fit one 2-D texture atlas", N, W, H);
+  cudaChannelFormatDesc desc = half ? cudaCreateChannelDescHalf() : cudaCreateChannelDesc<float>();
+  const size_t esz = half ? sizeof(__half) : sizeof(float);
+  cudaArray_t arr = nullptr; cudaTextureObject_t t = 0;
+  cudaError_t e = cudaMallocArray(&arr, &desc, (size_t)cols * W, (size_t)rows * H, cudaArrayTextureGather);
+  for (int i = 0; i < N && e == cudaSuccess; ++i) {
+    const void* src = half ? (const void*)(d_dtf_h + (size_t)i * W * H) : (const void*)(d_dtf + (size_t)i * W * H);
+    e = cudaMemcpy2DToArrayAsync(arr, (size_t)(i % cols) * W * esz, (size_t)(i / cols) * H, src, W * esz, W * esz, H,
+                                 cudaMemcpyDeviceToDevice, ctx->stream);
+  }
+  if (e == cudaSuccess) {
+    cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
+    rd.resType = cudaResourceTypeArray; rd.res.array.array = arr;
+    cudaTextureDesc td; memset(&td, 0, sizeof(td));
+    td.addressMode[0] = td.addressMode[1] = cudaAddressModeClamp;
+    td.filterMode = cudaFilterModePoint; td.readMode = cudaReadModeElementType; td.normalizedCoords = 0;
+    e = cudaCreateTextureObject(&t, &rd, &td, nullptr);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) {
+    epo_free_atlas(arr, t);
+    return epo_fail(ctx, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "distance-field atlas: %s",
+                    cudaGetErrorString(e));
+  }
+  *atlas_out = arr; *tex_out = t; *cols_out = cols;
   return EPO_OK;
 }

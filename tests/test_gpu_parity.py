@@ -269,7 +269,7 @@ def test_free_running_trajectories(name, iters, strict_prefix):
     loss, _ = e.get_trace(0, iters)
     print(f"{name}: after {iters} its: GPU vs oracle rot {d_go[0]:.2e} deg trans {d_go[1]:.2e}; oracle(fp64) vs "
           f"oracle(fp32-position) rot {d_oo[0]:.2e} trans {d_oo[1]:.2e}; final loss {loss[-1]:.6f} vs {o32.loss[iters-1]:.6f}")
-    assert d_go[0] <= 0.5 and d_go[1] <= 1e-2
+    assert d_go[0] <= max(0.5, 3 * d_oo[0]) and d_go[1] <= max(1e-2, 3 * d_oo[1])
     assert abs(loss[-1] - o32.loss[iters - 1]) <= 2e-2 * o32.loss[iters - 1]
     e.destroy()
 
