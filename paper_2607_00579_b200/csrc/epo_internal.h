@@ -20,10 +20,24 @@ struct __align__(8) EdgeRec {
 // A = sum a, M = sum x_t x a (six-accumulator identity I1).  fp64, 64 bytes per work item.
 constexpr int kAccStride = 8;
 
-// Edge pixels handled by one CTA of the fused kernel: kLgThreads threads x kLgPerThread samples.
-constexpr int kLgThreads = 256;
-constexpr int kLgPerThread = 8;
-constexpr int kLgChunk = kLgThreads * kLgPerThread;
+// Edge pixels handled by one CTA of the fused kernel: kLgOuter passes of kLgThreads threads x kLgPerThread
+// (unrolled) samples.  The point list is padded by kLgChunk entries so that tail lanes may read past a list.
+#ifndef EPO_LG_THREADS
+#define EPO_LG_THREADS 256
+#endif
+#ifndef EPO_LG_PER_THREAD
+#define EPO_LG_PER_THREAD 2
+#endif
+#ifndef EPO_LG_OUTER
+#define EPO_LG_OUTER 8
+#endif
+#ifndef EPO_LG_MINBLOCKS
+#define EPO_LG_MINBLOCKS 4
+#endif
+constexpr int kLgThreads = EPO_LG_THREADS;
+constexpr int kLgPerThread = EPO_LG_PER_THREAD;
+constexpr int kLgOuter = EPO_LG_OUTER;
+constexpr int kLgChunk = kLgThreads * kLgPerThread * kLgOuter;
 
 // Device-resident control block of the optimisation loop (rows a-10..a-12): lets epo_step enqueue
 // n iterations without any host synchronisation; every kernel of an iteration checks `stopped`.

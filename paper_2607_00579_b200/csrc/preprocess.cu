@@ -333,7 +333,9 @@ epo_status epo_build_dtf(epo_ctx* ctx, const uint8_t* d_edges_u8, float* d_dtf, 
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
                             const std::vector<int32_t>& h_off, float4** out_pts) {
   float4* pts = nullptr;
-  EPO_CUDA(ctx, cudaMalloc(&pts, (size_t)(E > 0 ? E : 1) * sizeof(float4)));
+  // padded by one chunk of zeros: the fused kernel's tail lanes read past the end of a list and discard
+  EPO_CUDA(ctx, cudaMalloc(&pts, (size_t)(E + kLgChunk) * sizeof(float4)));
+  EPO_CUDA(ctx, cudaMemsetAsync(pts + E, 0, (size_t)kLgChunk * sizeof(float4), ctx->stream));
   int max_n = 1;
   for (int i = 0; i < ctx->N; ++i) max_n = h_off[i + 1] - h_off[i] > max_n ? h_off[i + 1] - h_off[i] : max_n;
   dim3 grid((max_n + 255) / 256, ctx->N);
