@@ -43,6 +43,8 @@ def parse():
     ap.add_argument("--refine-iters", type=int, default=200)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--plumbing-test", action="store_true",
+                    help="CPU-only check of the multi-rank plumbing (gloo): fake per-rank timings, no GPU work")
     return ap.parse_args()
 
 
@@ -58,6 +60,25 @@ def peaks():
         d = json.load(open(p))
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(config: int):
+    """dram read + write bytes per launch of the fused kernel from the committed ncu summary
+    (profiles/traffic.csv: config,kernel,dram_read_bytes,dram_write_bytes,source); None if not captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(p):
+        return None
+    best = None
+    for ln in open(p):
+        c = [x.strip() for x in ln.split(",")]
+        if ln.startswith("#") or len(c) < 4:
+            continue
+        try:
+            if int(c[0]) == config and c[1] == "k_loss_grad":
+                best = float(c[2]) + float(c[3])
+        except ValueError:
+            continue
+    return best
 
 
 class ClockSampler:
@@ -166,11 +187,47 @@ def run_reference(args, sc):
     print(json.dumps(line))
 
 
+def max_over_ranks(x: float, world: int, device) -> float:
+    """Timing rule of the contract: a multi-rank number is the MAX over ranks."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, units_per_rank_step: int, steps: int, total_ms: float) -> float:
+    """Replicas only: every rank processes the same number of units; value = all ranks'
+    units / the slowest rank's time."""
+    return world * units_per_rank_step * steps / (total_ms / 1e3)
+
+
+def plumbing_test(args, rank, world):
+    """No GPU: rendezvous over gloo, rank-dependent fake timings, the same reduction and printing rules."""
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    total_ms = max_over_ranks(10.0 * (rank + 1), world, "cpu")
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(dict(metric=METRIC, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                              value=whole_job_value(world, 1000, args.steps, total_ms),
+                              ms_per_step=total_ms / args.steps, scaling="weak", plumbing_test=True)))
+
+
 def main():
     args = parse()
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     from epo_scenes import make_scene
+    if args.plumbing_test:
+        plumbing_test(args, rank, world)
+        return
     if args.impl == "reference":
         if rank == 0:
             run_reference(args, make_scene(args.config, n_views=args.views))
@@ -241,9 +298,8 @@ def main():
     e.reset(); torch.cuda.synchronize()
     a.record(stream); done, phase = e.step(args.refine_iters); b.record(stream); torch.cuda.synchronize()
     refine_s = a.elapsed_time(b) / 1e3
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); total_ms = float(t.item())
-    value = world * reproj * args.steps / (total_ms / 1e3)
+    total_ms = max_over_ranks(total_ms, world, "cuda")
+    value = whole_job_value(world, reproj, args.steps, total_ms)
 
     # e2e through the C ABI with pinned HOST buffers (H2D + preprocessing + pairs + iterations + D2H)
     e2e = None
@@ -291,12 +347,7 @@ def main():
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = cpu_baseline(sc)
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(prof):
-        try:
-            line["roofline"]["traffic"] = json.load(open(prof)).get(f"config{args.config}")
-        except Exception:
-            pass
+    line["roofline"]["traffic"] = ncu_traffic(args.config)
     print(json.dumps(line))
 
 

@@ -1,0 +1,116 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same library build, same
+work decomposition, device-resident inputs): every pair and every camera of configs 2-5 against the CPU oracle
+(it is C + OpenMP, so whole evaluations at full size take seconds), plus bit-exact preprocessing on sampled
+views and a few lock-step optimiser iterations."""
+import numpy as np
+import pytest
+
+import oracle
+from epo_scenes import make_scene
+from parity_utils import Z_MIN, check_camera_grads, check_pair_losses, make_ctx, oracle_config, pose_errors
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_00579_b200 import build
+    build.build()
+
+
+def _full(config, **cfg_over):
+    sc = make_scene(config)
+    e = make_ctx(sc, device_inputs=True, **cfg_over)
+    prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
+    return sc, e, prob
+
+
+@pytest.mark.parametrize("config", [2, 3, 4, 5])
+def test_full_size_loss_gradient_and_preprocessing(config):
+    sc, e, prob = _full(config, early_stop=0)
+    N = sc.n_views
+    # preprocessing: offsets of all views; lists and fields bit-exact on a seeded sample of views (+ first, last)
+    off = e.get_edge_counts()
+    assert np.array_equal(off, prob.edge_off)
+    views = sorted({0, N - 1} | {int(v) for v in np.random.default_rng(config).choice(N, size=min(6, N), replace=False)})
+    for i in views:
+        uv, z = e.get_edge_list(i, off[i + 1] - off[i])
+        assert np.array_equal(uv, prob.uv[off[i]:off[i + 1]]) and np.array_equal(z, prob.z[off[i]:off[i + 1]])
+        assert np.array_equal(e.get_dtf(i), prob.dtf[i]), i
+    cp, perm = e.get_pair_order()
+    ocp, operm = oracle.canonical_pairs(sc.pairs)
+    assert np.array_equal(cp, ocp) and np.array_equal(perm, operm)
+    # loss + gradient, all pairs, all cameras
+    poses = sc.poses_init.astype(np.float64)
+    for lam in (10.0, 6.0):
+        got = e.loss_grad(lam)
+        ref32 = oracle.loss_grad(prob, poses, sc.pairs, lam, z_min=Z_MIN, coord_fp32=1)
+        assert np.array_equal(got["pair_valid"], ref32["pair_valid"])
+        w32 = check_pair_losses(got["pair_loss"], got["pair_valid"], ref32, lam, max_event_frac=0.0)
+        assert abs(got["loss"] - ref32["loss"]) <= 1e-5 * abs(ref32["loss"])
+        g32 = check_camera_grads(got["grad"], ref32["grad"])
+        print(f"config {config} full size lam={lam}: {len(sc.pairs)} pairs, {int(got['pair_valid'].sum())} valid samples; "
+              f"pair loss rel err {w32:.2e}, camera grad rel err {g32:.2e}")
+    ref64 = oracle.loss_grad(prob, poses, sc.pairs, 10.0, z_min=Z_MIN)
+    got = e.loss_grad(10.0)
+    check_pair_losses(got["pair_loss"], got["pair_valid"], ref64, 10.0)
+    # three lock-step iterations of the loop at full size
+    ocfg = oracle_config(coord_fp32=1, early_stop=0)
+    m = np.zeros((N, 6)); v = np.zeros((N, 6))
+    P = e.get_poses_f64()
+    for k in range(3):
+        ref = oracle.loss_grad(prob, P, sc.pairs, oracle.lam_schedule(k, ocfg), z_min=Z_MIN, coord_fp32=1)
+        inc = oracle.adam(ref["grad"].reshape(-1), m.reshape(-1), v.reshape(-1), k, oracle.lr_schedule(k, ocfg),
+                          ocfg.beta1, ocfg.beta2, ocfg.adam_eps).reshape(N, 6)
+        pred = np.stack([oracle.se3_compose(oracle.se3_exp(inc[c]), P[c]) for c in range(N)])
+        assert e.step(1)[0] == 1
+        new = e.get_poses_f64()
+        rot, tr = pose_errors(new, pred)
+        loss, theta = e.get_trace(k, 1)
+        assert rot <= 1e-3 and tr <= 1e-4, (k, rot, tr)
+        assert abs(float(loss[0]) - ref["loss"]) <= 1e-5 * abs(ref["loss"])
+        th = oracle.theta95(pred, P)
+        assert abs(float(theta[0]) - th) <= 1e-3 * th + 1e-7
+        P = new
+    e.destroy()
+
+
+def test_full_size_config4_fp16_fields():
+    """BASELINE.json config 4 variant: fp16 distance fields against the fp32 oracle at 1e-3 relative."""
+    sc, e, prob = _full(4, dtf_format=1)
+    poses = sc.poses_init.astype(np.float64)
+    got = e.loss_grad(10.0)
+    ref = oracle.loss_grad(prob, poses, sc.pairs, 10.0, z_min=Z_MIN)
+    check_pair_losses(got["pair_loss"], got["pair_valid"], ref, 10.0, rtol=1e-3)
+    assert abs(got["loss"] - ref["loss"]) <= 1e-3 * abs(ref["loss"])
+    err = np.linalg.norm(got["grad"] - ref["grad"], axis=1) / np.linalg.norm(ref["grad"], axis=1)
+    print(f"config 4 fp16 fields: loss rel err {abs(got['loss'] - ref['loss']) / ref['loss']:.2e}, camera grad rel err max {err.max():.2e}")
+    # the fp16 field's gradient differs from the fp32 field's by the rounding of neighbouring taps (2^-11 relative
+    # on values up to ~100 px against differences of ~1 px): reported, bounded loosely
+    assert err.max() <= 5e-2
+    e.destroy()
+
+
+def test_full_size_config5_early_stop_runs_to_its_own_stop():
+    """Config 5 as stated: early stop active, max 2000 steps, one epo_step call with no host sync inside."""
+    sc, e, prob = _full(5, early_stop=1)
+    done, phase = e.step(2000)
+    loss, theta = e.get_trace(0, done)
+    print(f"config 5 full size: stopped after {done} iterations in phase {phase}; loss {loss[0]:.4f} -> {loss[-1]:.4f}; "
+          f"theta95 {theta[0]:.3f} -> {theta[-1]:.4f} deg")
+    assert phase == 2 and 100 <= done < 2000
+    assert loss[-1] < 0.5 * loss[0]
+    # the rule, re-run by the oracle on the GPU's own theta trace, fires at exactly that step and not before
+    ocfg = oracle_config(early_stop=1)
+    th = theta.astype(np.float64); ph = 0; fired = None
+    for s in range(done):
+        if ph == 0:
+            if oracle.converged(th, s, ocfg.w1, ocfg.eps1, ocfg.smooth_window): ph = 1
+        elif ph == 1 and oracle.converged(th, s, ocfg.w2, ocfg.eps2, ocfg.smooth_window):
+            ph = 2; fired = s + 1; break
+    assert fired == done, (fired, done)
+    assert e.step(10) == (0, 2)
+    e.destroy()
