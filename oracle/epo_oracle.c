@@ -232,7 +232,8 @@ void orc_relative_pose(const double Ts[12], const double Tt[12], double Tts[12])
  * gradient.  In this variant steps a-2..a-4 (back-project, transform, project) are therefore evaluated in
  * IEEE binary32 with the operation order stated below (every operation individually rounded; fmaf is the
  * correctly rounded fused multiply-add), and everything after the position (weights, interpolation, robust
- * loss, Jacobian, sums) continues in double exactly as in the default path.
+ * loss, Jacobian, sums) continues in double exactly as in the default path -- except the one remaining discrete
+ * decision, the clamp test d <= lambda (rho' jumps there), taken on the binary32 value of d stated at that line.
  *   T_ts, K rounded once to float;  ifx = 1/fx_s, ify = 1/fy_s
  *   x_s = Z ((u - cx_s) ifx), y_s = Z ((v - cy_s) ify), z_s = Z
  *   X = fma(r00, x_s, fma(r01, y_s, fma(r02, z_s, t_x)))   (same for Y, Z)
@@ -277,7 +278,16 @@ static void orc_pair_loss_grad_f32coords(int W, int H, int n_edges, const uint16
     if (fabs(d - lambda) < 1e-3 || fabs(d - delta) < 1e-3) near[1]++;
     double dhat = d < lambda ? d : lambda;
     double rho = dhat <= delta ? 0.5 * dhat * dhat : delta * (dhat - 0.5 * delta);
-    double drho = (d <= lambda) ? (d < delta ? d : delta) : 0.0;
+    /* reading P1 (clamp decision): rho' jumps from delta to 0 at d = lambda, so "d <= lambda" is a discrete
+     * decision like the cell index; in this variant it is taken on the binary32 value of d, evaluated as
+     *   dx0 = D01 - D00, dy0 = D10 - D00, c = (D11 - D10) - dx0, d32 = fma(wy, fma(wx, c, dy0), fma(wx, dx0, D00))
+     * (wx, wy are exact in binary32: x - x0 with x0 <= x < x0 + 1).  Values (rho, rho', gradient) stay double. */
+    const float wxf = (float)wx, wyf = (float)wy;
+    const float D00f = dtf_t[(size_t)y0 * W + x0], D01f = dtf_t[(size_t)y0 * W + x0 + 1];
+    const float D10f = dtf_t[(size_t)(y0 + 1) * W + x0], D11f = dtf_t[(size_t)(y0 + 1) * W + x0 + 1];
+    const float dx0f = D01f - D00f, dy0f = D10f - D00f, cf = (D11f - D10f) - dx0f;
+    const float d32 = fmaf(wyf, fmaf(wxf, cf, dy0f), fmaf(wxf, dx0f, D00f));
+    double drho = (d32 <= (float)lambda) ? (d < delta ? d : delta) : 0.0;
     S += rho; nv++;
     double iz = 1.0 / xt[2];
     double a[3], b[3];
