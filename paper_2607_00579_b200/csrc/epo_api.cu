@@ -1,6 +1,8 @@
 // Host side of the C ABI declared in include/epo.h: argument validation, host/device pointer
 // marshalling, device-memory ownership and launch sequencing.  No arithmetic of the method lives here.
+#include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstdarg>
 #include <cstring>
 #include <new>
@@ -26,6 +28,24 @@ bool is_device_ptr(const void* p) {
   return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
+// EPO_TRACE=1 in the environment: print the wall-clock duration of each phase of a call to stderr (each mark
+// drains the stream first, so the phases do not overlap while tracing).  Off: no synchronisation, no output.
+struct PhaseTrace {
+  cudaStream_t st; const char* what; bool on; std::chrono::steady_clock::time_point t0;
+  PhaseTrace(cudaStream_t s, const char* w) : st(s), what(w) {
+    const char* v = std::getenv("EPO_TRACE");
+    on = v && v[0] && v[0] != '0';
+    if (on) { cudaStreamSynchronize(st); t0 = std::chrono::steady_clock::now(); }
+  }
+  void mark(const char* phase) {
+    if (!on) return;
+    cudaStreamSynchronize(st);
+    auto t1 = std::chrono::steady_clock::now();
+    fprintf(stderr, "[epo trace] %s: %-18s %8.3f ms\n", what, phase, std::chrono::duration<double, std::milli>(t1 - t0).count());
+    t0 = t1;
+  }
+};
+
 // copy caller memory (host or device) into library device memory on the context's stream
 cudaError_t copy_in(void* dst, const void* src, size_t bytes, cudaStream_t st) {
   return cudaMemcpyAsync(dst, src, bytes, is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
@@ -38,9 +58,9 @@ cudaError_t copy_out(void* dst, const void* src, size_t bytes, cudaStream_t st, 
 }
 
 void free_views(epo_ctx* c) {
-  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_dtf); cudaFree(c->d_dtf_h); cudaFree(c->d_pts);
+  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_pts);
   epo_free_atlas(c->dtf_atlas, c->dtf_tex);
-  c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_dtf = nullptr; c->d_dtf_h = nullptr; c->d_pts = nullptr;
+  c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_pts = nullptr;
   c->dtf_atlas = nullptr; c->dtf_tex = 0;
   c->have_views = false;
 }
@@ -156,51 +176,64 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
         return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_views: view %zu has a non-finite pose", i);
   }
   // build everything into temporaries; commit only on success (all-or-nothing)
-  float* d_depth = nullptr; uint8_t* d_e = nullptr; float* d_dtf = nullptr; __half* d_dtf_h = nullptr;
-  float* d_pose_f = nullptr; int32_t* off = nullptr; EdgeRec* rec = nullptr; int64_t E = 0;
+  PhaseTrace tr(st, "epo_set_views");
+  float* d_depth = nullptr; uint8_t* d_e = nullptr; float* d_small = nullptr;
+  int32_t* off = nullptr; EdgeRec* rec = nullptr; int64_t E = 0;
+  float4* pts = nullptr; cudaArray_t atlas = nullptr; cudaTextureObject_t tex = 0; int cols = 1;
+  EpoDtfScratch scratch = {nullptr, 0};
   std::vector<int32_t> hoff;
   epo_status rc = EPO_OK;
   cudaError_t e = cudaMalloc(&d_depth, N * px * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&d_e, N * px);
-  if (e == cudaSuccess) e = cudaMalloc(&d_dtf, N * px * sizeof(float));
-  if (e == cudaSuccess && c->cfg.dtf_format == 1) e = cudaMalloc(&d_dtf_h, N * px * sizeof(__half));
-  if (e == cudaSuccess) e = cudaMalloc(&d_pose_f, N * 12 * sizeof(float));
-  if (e == cudaSuccess) e = copy_in(d_depth, depth, N * px * sizeof(float), st);
+  if (e == cudaSuccess) e = cudaMalloc(&d_small, N * 16 * sizeof(float));   // [K 4N | poses 12N] staging
+  tr.mark("alloc inputs");
+  // the edge maps first: the distance transform needs nothing else and runs while the depth maps arrive
   if (e == cudaSuccess) e = copy_in(d_e, edges, N * px, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_small, hK.data(), N * 4 * sizeof(float), cudaMemcpyHostToDevice, st);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_small + N * 4, hP.data(), N * 12 * sizeof(float), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess)
     rc = epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_set_views: %s",
                   cudaGetErrorString(e));
-  if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff);
-  if (rc == EPO_OK) rc = epo_build_dtf(c, d_e, d_dtf, d_dtf_h);
-  cudaFree(d_depth); cudaFree(d_e);
-  float* d_Ktmp = nullptr; float4* pts = nullptr;
-  cudaArray_t atlas = nullptr; cudaTextureObject_t tex = 0; int cols = 1;
+  tr.mark("copy edges");
+  if (rc == EPO_OK) rc = epo_build_dtf_atlas(c, d_e, &atlas, &tex, &cols, &scratch);
+  tr.mark("distance fields");
   if (rc == EPO_OK) {
-    e = cudaMalloc(&d_Ktmp, N * 4 * sizeof(float));
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_Ktmp, hK.data(), N * 4 * sizeof(float), cudaMemcpyHostToDevice, st);
+    e = copy_in(d_depth, depth, N * px * sizeof(float), st);
     if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
   }
-  if (rc == EPO_OK) rc = epo_build_points(c, d_Ktmp, off, rec, E, hoff, &pts);
-  if (rc == EPO_OK) rc = epo_build_atlas(c, d_dtf, d_dtf_h, &atlas, &tex, &cols);
+  tr.mark("copy depth");
+  if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff);
+  tr.mark("edge lists");
+  if (rc == EPO_OK) rc = epo_build_points(c, d_small, off, rec, E, hoff, &pts);
+  if (rc == EPO_OK) {
+    // commit the small state on the stream, then drain it once
+    e = cudaMemcpyAsync(c->d_K, d_small, N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, st);
+    if (e == cudaSuccess) {
+      epo_launch_f32_to_f64(st, d_small + N * 4, c->d_poses_init, (int64_t)N * 12);
+      c->launches += 1;
+      e = cudaMemcpyAsync(c->d_poses, c->d_poses_init, N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
+  }
+  if (rc == EPO_OK) rc = reset_optimiser(c);
+  e = cudaStreamSynchronize(st);
+  if (rc == EPO_OK && e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
+  tr.mark("points + drain");
+  epo_free_dtf_scratch(&scratch);
+  cudaFree(d_depth); cudaFree(d_e); cudaFree(d_small);
   if (rc != EPO_OK) {
-    cudaStreamSynchronize(st);
+    // d_K / d_poses may have been overwritten only if every build step succeeded and the final drain failed
+    // (a sticky CUDA error: the context is unusable anyway)
     cudaGetLastError();
-    cudaFree(d_dtf); cudaFree(d_dtf_h); cudaFree(d_pose_f); cudaFree(off); cudaFree(rec); cudaFree(d_Ktmp); cudaFree(pts);
+    cudaFree(off); cudaFree(rec); cudaFree(pts); epo_free_atlas(atlas, tex);
     return rc;
   }
-  cudaFree(d_Ktmp);   // epo_build_atlas synchronised the stream: k_make_points has finished
   free_pairs(c); free_views(c);
-  c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff; c->d_dtf = d_dtf; c->d_dtf_h = d_dtf_h;
+  c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff;
   c->d_pts = pts; c->dtf_atlas = atlas; c->dtf_tex = tex; c->atlas_cols = cols;
-  EPO_CUDA(c, cudaMemcpyAsync(c->d_K, hK.data(), N * 4 * sizeof(float), cudaMemcpyHostToDevice, st));
-  EPO_CUDA(c, cudaMemcpyAsync(d_pose_f, hP.data(), N * 12 * sizeof(float), cudaMemcpyHostToDevice, st));
-  epo_launch_f32_to_f64(st, d_pose_f, c->d_poses_init, (int64_t)N * 12);
-  EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
-  c->launches += 1;
-  EPO_TRY(reset_optimiser(c));
-  EPO_CUDA(c, cudaStreamSynchronize(st));   // hK / hP are stack-owned
-  cudaFree(d_pose_f);
   c->have_views = true;
+  tr.mark("free temporaries");
   return EPO_OK;
 }
 
@@ -401,20 +434,24 @@ epo_status epo_get_dtf(epo_ctx* c, int32_t view, float* dtf) {
   if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_dtf before epo_set_views");
   if (view < 0 || view >= c->N || !dtf) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_dtf: bad argument");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
-  const size_t px = (size_t)c->W * c->H;
-  bool sync = false;
-  if (c->cfg.dtf_format == 1) {   // widen the fp16 field that the kernel actually samples
-    std::vector<__half> h(px);
-    EPO_CUDA(c, cudaMemcpyAsync(h.data(), c->d_dtf_h + view * px, px * sizeof(__half), cudaMemcpyDeviceToHost, c->stream));
+  // the field lives only in the atlas the kernel samples: read view's tile back (fp16 fields are widened)
+  const size_t W = (size_t)c->W, H = (size_t)c->H;
+  const size_t ax = (size_t)(view % c->atlas_cols) * W, ay = (size_t)(view / c->atlas_cols) * H;
+  if (c->cfg.dtf_format == 1) {
+    std::vector<__half> h(W * H);
+    EPO_CUDA(c, cudaMemcpy2DFromArrayAsync(h.data(), W * sizeof(__half), c->dtf_atlas, ax * sizeof(__half), ay,
+                                           W * sizeof(__half), H, cudaMemcpyDeviceToHost, c->stream));
     EPO_CUDA(c, cudaStreamSynchronize(c->stream));
-    std::vector<float> f(px);
-    for (size_t i = 0; i < px; ++i) f[i] = __half2float(h[i]);
-    EPO_CUDA(c, cudaMemcpyAsync(dtf, f.data(), px * sizeof(float), cudaMemcpyDefault, c->stream));
+    std::vector<float> f(W * H);
+    for (size_t i = 0; i < W * H; ++i) f[i] = __half2float(h[i]);
+    EPO_CUDA(c, cudaMemcpyAsync(dtf, f.data(), W * H * sizeof(float), cudaMemcpyDefault, c->stream));
     EPO_CUDA(c, cudaStreamSynchronize(c->stream));
     return EPO_OK;
   }
-  EPO_CUDA(c, copy_out(dtf, c->d_dtf + view * px, px * sizeof(float), c->stream, &sync));
-  if (sync) EPO_CUDA(c, cudaStreamSynchronize(c->stream));
+  const bool dev = is_device_ptr(dtf);
+  EPO_CUDA(c, cudaMemcpy2DFromArrayAsync(dtf, W * sizeof(float), c->dtf_atlas, ax * sizeof(float), ay, W * sizeof(float), H,
+                                         dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+  if (!dev) EPO_CUDA(c, cudaStreamSynchronize(c->stream));
   return EPO_OK;
 }
 

@@ -63,9 +63,7 @@ struct epo_ctx {
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
   float4* d_pts;          // [E] camera-frame points (x_s, y_s, z_s, 0): K and Z are fixed, so row a-2 is hoisted
-  float* d_dtf;           // [N][H][W] fp32 field, pitch-linear (epo_get_dtf; source of the texture copies)
-  __half* d_dtf_h;        // [N][H][W] fp16 field when cfg.dtf_format == 1
-  cudaArray_t dtf_atlas;                      // block-linear, gather-enabled copy of all fields: views tiled in a grid
+  cudaArray_t dtf_atlas;                      // block-linear, gather-enabled array of all fields (fp32 or fp16): views tiled in a grid
   cudaTextureObject_t dtf_tex;                // texture object on the atlas (what the fused kernel samples)
   int atlas_cols;                             // view i sits at texel offset ((i % cols) W, (i / cols) H)
   std::vector<int32_t> h_edge_off;
@@ -123,11 +121,12 @@ epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
                                 int32_t** out_off, EdgeRec** out_rec, int64_t* out_E,
                                 std::vector<int32_t>* h_off);
-epo_status epo_build_dtf(epo_ctx* ctx, const uint8_t* d_edges_u8, float* d_dtf, __half* d_dtf_h);
+struct EpoDtfScratch { int32_t* g; cudaSurfaceObject_t surf; };   // alive until the EDT kernels have run
+epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArray_t* atlas, cudaTextureObject_t* tex,
+                               int* cols, EpoDtfScratch* scratch);
+void epo_free_dtf_scratch(EpoDtfScratch* s);
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
                             const std::vector<int32_t>& h_off, float4** out_pts);
-epo_status epo_build_atlas(epo_ctx* ctx, const float* d_dtf, const __half* d_dtf_h, cudaArray_t* atlas,
-                           cudaTextureObject_t* tex, int* cols);
 void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex);
 // pairs.cu
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,

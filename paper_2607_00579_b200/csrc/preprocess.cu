@@ -163,52 +163,51 @@ __global__ void k_edt_rows(const uint8_t* __restrict__ edges, int64_t rows, int 
 }
 
 // ---------------------------------------------------------------------------------------------
-// a-P3  EDT pass 2: d2[y][x] = min_{y'} g[y'][x]^2 + (y - y')^2 by the lower envelope of parabolas,
-// with the integer-only separator of Meijster, Roerdink & Hesselink (2000): every comparison is an
-// exact integer comparison, so d2 is the exact minimum.  One thread per column; its two stacks
-// (s: parabola apex rows, t: first row where that parabola is the minimum) live in shared memory,
-// laid out [stack index][column] so that threads never collide on a bank.
-// DTF = correctly rounded fp32 sqrt of d2 (d2 < 2^24 exactly representable; else via fp64 sqrt).
+// a-P3  EDT pass 2: d2[y][x] = min_{y'} g[y'][x]^2 + (y - y')^2, exactly, in integers.
+// One thread per PIXEL (not per column): a CTA stages the g values of a strip of 32 columns x H rows in
+// shared memory (coalesced 128-byte rows), then every pixel searches outwards dy = 1, 2, ... in both
+// directions and stops as soon as dy^2 >= the best value so far -- no farther row can improve it, so the
+// minimum is exact.  The search length is the distance itself (a few to a few tens of rows at the paper's
+// edge densities, at most H), all H x W pixels of a view run in parallel, and lanes of a warp are
+// neighbouring columns of one row, whose distances differ by at most 31 (the field is 1-Lipschitz), so a warp
+// stays converged.  An out-of-range row is clamped to the border row: its candidate only over-estimates
+// that row's true candidate, so the minimum is unchanged and the loop is branch-free.
+// DTF = correctly rounded fp32 sqrt of d2 (d2 < 2^24 is exact in fp32; else via fp64 sqrt), written
+// straight into the block-linear atlas the fused kernel samples (surface store; fp16 = RNE of the fp32).
 // ---------------------------------------------------------------------------------------------
-template <typename I>
-__device__ __forceinline__ I parab(I x, I i, I gi) { return (x - i) * (x - i) + gi * gi; }
+constexpr int kEdtStrip = 32, kEdtWarps = 8;
 
-template <typename I>
-__global__ void k_edt_cols(const int32_t* __restrict__ g, int W, int H, float* __restrict__ dtf,
-                           __half* __restrict__ dtf_h) {
-  extern __shared__ uint16_t stacks[];
-  const int C = blockDim.x;
-  uint16_t* s = stacks;                       // [H][C]
-  uint16_t* t = stacks + (size_t)H * C;       // [H][C]
-  const int col = blockIdx.x * C + threadIdx.x;
-  const int view = blockIdx.y;
-  if (col >= W) return;
-  const int c = threadIdx.x;
-  const int32_t* gv = g + (size_t)view * W * H + col;
-  int q = 0;
-  s[c] = 0; t[c] = 0;
-  for (int u = 1; u < H; ++u) {
-    I gu = (I)gv[(size_t)u * W];
-    while (q >= 0) {
-      I tq = (I)t[q * C + c], sq = (I)s[q * C + c];
-      if (parab<I>(tq, sq, (I)gv[(size_t)sq * W]) > parab<I>(tq, (I)u, gu)) --q; else break;
-    }
-    if (q < 0) { q = 0; s[c] = (uint16_t)u; }
-    else {
-      I i = (I)s[q * C + c], gi = (I)gv[(size_t)i * W];
-      I sep = ((I)u * u - i * i + gu * gu - gi * gi) / (2 * ((I)u - i));   // >= t[q] >= 0: floor == trunc
-      I w = sep + 1;
-      if (w < (I)H) { ++q; s[q * C + c] = (uint16_t)u; t[q * C + c] = (uint16_t)w; }
-    }
+template <typename I, bool kStage>
+__global__ void __launch_bounds__(kEdtStrip * kEdtWarps)
+k_edt_cols(const int32_t* __restrict__ g, int W, int H, cudaSurfaceObject_t atlas, int atlas_cols, int half) {
+  extern __shared__ int32_t sg[];             // [H][32] when kStage
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int view = blockIdx.y, x = blockIdx.x * kEdtStrip + lane;
+  const bool in = x < W;
+  const int32_t* gv = g + (size_t)view * W * H + (in ? x : W - 1);
+  if (kStage) {
+    for (int y = warp; y < H; y += kEdtWarps) sg[y * kEdtStrip + lane] = gv[(size_t)y * W];
+    __syncthreads();
   }
-  for (int u = H - 1; u >= 0; --u) {
-    I i = (I)s[q * C + c];
-    I d2 = parab<I>((I)u, i, (I)gv[(size_t)i * W]);
-    float r = (d2 < (I)(1 << 24)) ? __fsqrt_rn((float)d2) : (float)sqrt((double)d2);
-    size_t o = ((size_t)view * H + u) * W + col;
-    dtf[o] = r;
-    if (dtf_h) dtf_h[o] = __float2half_rn(r);
-    if (u == (int)t[q * C + c]) --q;
+  auto G = [&](int y) -> I { return kStage ? (I)sg[y * kEdtStrip + lane] : (I)__ldg(gv + (size_t)y * W); };
+  const int ox = (view % atlas_cols) * W + x, oy = (view / atlas_cols) * H;
+  for (int y = warp; y < H; y += kEdtWarps) {
+    const I g0 = G(y);
+    I best = g0 * g0;
+    const int dmax = max(y, H - 1 - y);
+    for (int dy = 1; dy <= dmax; ++dy) {
+      const I dd = (I)dy * dy;
+      if (dd >= best) break;
+      const I a = G(max(y - dy, 0)), b = G(min(y + dy, H - 1));
+      const I m = a < b ? a : b;
+      const I c = m * m + dd;
+      best = c < best ? c : best;
+    }
+    if (in) {
+      const float r = (best < (I)(1 << 24)) ? __fsqrt_rn((float)best) : (float)sqrt((double)best);
+      if (half) surf2Dwrite(__half_as_ushort(__float2half_rn(r)), atlas, ox * 2, oy + y);
+      else surf2Dwrite(r, atlas, ox * 4, oy + y);
+    }
   }
 }
 
@@ -298,35 +297,77 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
   return EPO_OK;
 }
 
-epo_status epo_build_dtf(epo_ctx* ctx, const uint8_t* d_edges_u8, float* d_dtf, __half* d_dtf_h) {
+void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex) {
+  if (tex) cudaDestroyTextureObject(tex);
+  if (atlas) cudaFreeArray(atlas);
+}
+
+// Distance fields of all views (rows a-P2, a-P3), written straight into ONE block-linear, gather-enabled 2-D
+// CUDA array (view i at texel offset ((i % cols) W, (i / cols) H)) behind one texture object.  The fused kernel
+// fetches the 2x2 bilinear footprint with ONE tld4 (tex2Dgather) and applies the exact fp32 weights itself;
+// the hardware's 8-bit-fraction filtering is never used.  A footprint never leaves its view (x0 <= W-2).
+// Enqueues on the context's stream and does NOT synchronise; the caller releases *scratch_out (row-pass
+// buffer + the surface handle the column kernel writes through) with epo_free_dtf_scratch once the stream
+// has drained.
+void epo_free_dtf_scratch(EpoDtfScratch* s) {
+  if (s->surf) cudaDestroySurfaceObject(s->surf);
+  cudaFree(s->g);
+  s->surf = 0; s->g = nullptr;
+}
+
+epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArray_t* atlas_out,
+                               cudaTextureObject_t* tex_out, int* cols_out, EpoDtfScratch* scratch_out) {
   const int N = ctx->N, W = ctx->W, H = ctx->H;
   const int64_t rows = (int64_t)N * H;
   cudaStream_t st = ctx->stream;
-  int32_t* g = nullptr;
-  EPO_CUDA(ctx, cudaMalloc(&g, (size_t)rows * W * sizeof(int32_t)));
-  const int grid_rows = (int)((rows + kWarpsPerBlock - 1) / kWarpsPerBlock);
-  k_edt_rows<<<grid_rows, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, rows, W, W + H, g);
-  // columns per CTA: as many as fit the two uint16 stacks [H][C] in shared memory
-  int C = 128;
-  const size_t budget = 200 * 1024;
-  while (C > 1 && (size_t)H * C * 2 * sizeof(uint16_t) > budget) C >>= 1;
-  const size_t smem = (size_t)H * C * 2 * sizeof(uint16_t);
-  if (smem > 227 * 1024) { cudaFree(g); return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "height %d too large for the EDT column pass", H); }
-  const bool wide = (int64_t)(W + H) * (W + H) + (int64_t)H * H >= (int64_t)INT32_MAX / 2;
-  dim3 grid((W + C - 1) / C, N);
-  cudaError_t e;
-  if (wide) {
-    e = cudaFuncSetAttribute(k_edt_cols<long long>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) k_edt_cols<long long><<<grid, C, smem, st>>>(g, W, H, d_dtf, d_dtf_h);
-  } else {
-    e = cudaFuncSetAttribute(k_edt_cols<int>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) k_edt_cols<int><<<grid, C, smem, st>>>(g, W, H, d_dtf, d_dtf_h);
+  const bool half = ctx->cfg.dtf_format == 1;
+  int cols = 32768 / W; if (cols < 1) cols = 1; if (cols > N) cols = N;
+  const int arows = (N + cols - 1) / cols;
+  if ((int64_t)arows * H > 65536 || (int64_t)cols * W > 131072)
+    return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "%d views of %dx%d do not fit one 2-D texture atlas", N, W, H);
+  cudaChannelFormatDesc desc = half ? cudaCreateChannelDescHalf() : cudaCreateChannelDesc<float>();
+  cudaArray_t arr = nullptr; cudaTextureObject_t t = 0; cudaSurfaceObject_t surf = 0; int32_t* g = nullptr;
+  cudaError_t e = cudaMallocArray(&arr, &desc, (size_t)cols * W, (size_t)arows * H,
+                                  cudaArrayTextureGather | cudaArraySurfaceLoadStore);
+  cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
+  rd.resType = cudaResourceTypeArray; rd.res.array.array = arr;
+  if (e == cudaSuccess) e = cudaCreateSurfaceObject(&surf, &rd);
+  if (e == cudaSuccess) e = cudaMalloc(&g, (size_t)rows * W * sizeof(int32_t));
+  if (e == cudaSuccess) {
+    const int grid_rows = (int)((rows + kWarpsPerBlock - 1) / kWarpsPerBlock);
+    k_edt_rows<<<grid_rows, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, rows, W, W + H, g);
+    // 64-bit arithmetic only when (W+H)^2 + H^2 could overflow int32
+    const bool wide = (int64_t)(W + H) * (W + H) + (int64_t)H * H >= (int64_t)INT32_MAX / 2;
+    const size_t smem = (size_t)H * kEdtStrip * sizeof(int32_t);
+    const bool stage = smem <= 200 * 1024;   // taller images read g through L1/L2 instead of a staged strip
+    dim3 grid((W + kEdtStrip - 1) / kEdtStrip, N);
+    const int thr = kEdtStrip * kEdtWarps;
+#define EDT_LAUNCH(I, S)                                                                                       \
+    do {                                                                                                        \
+      if (S) e = cudaFuncSetAttribute(k_edt_cols<I, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+      if (e == cudaSuccess) k_edt_cols<I, S><<<grid, thr, (S) ? smem : 0, st>>>(g, W, H, surf, cols, half ? 1 : 0); \
+    } while (0)
+    if (wide) { if (stage) EDT_LAUNCH(long long, true); else EDT_LAUNCH(long long, false); }
+    else      { if (stage) EDT_LAUNCH(int, true);       else EDT_LAUNCH(int, false); }
+#undef EDT_LAUNCH
+    ctx->launches += 2;
+    if (e == cudaSuccess) e = cudaGetLastError();
   }
-  ctx->launches += 2;
-  if (e == cudaSuccess) e = cudaGetLastError();
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(g);
-  if (e != cudaSuccess) return epo_fail(ctx, EPO_ERR_CUDA, "EDT kernels failed: %s", cudaGetErrorString(e));
+  if (e == cudaSuccess) {
+    cudaTextureDesc td; memset(&td, 0, sizeof(td));
+    td.addressMode[0] = td.addressMode[1] = cudaAddressModeClamp;
+    td.filterMode = cudaFilterModePoint; td.readMode = cudaReadModeElementType; td.normalizedCoords = 0;
+    e = cudaCreateTextureObject(&t, &rd, &td, nullptr);
+  }
+  if (e != cudaSuccess) {
+    cudaStreamSynchronize(st);
+    if (surf) cudaDestroySurfaceObject(surf);
+    cudaFree(g);
+    epo_free_atlas(arr, t);
+    return epo_fail(ctx, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "distance fields: %s",
+                    cudaGetErrorString(e));
+  }
+  *atlas_out = arr; *tex_out = t; *cols_out = cols; scratch_out->g = g; scratch_out->surf = surf;
   return EPO_OK;
 }
 
@@ -344,49 +385,5 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { cudaFree(pts); return epo_fail(ctx, EPO_ERR_CUDA, "k_make_points: %s", cudaGetErrorString(e)); }
   *out_pts = pts;
-  return EPO_OK;
-}
-
-void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex) {
-  if (tex) cudaDestroyTextureObject(tex);
-  if (atlas) cudaFreeArray(atlas);
-}
-
-// Block-linear, gather-enabled copy of the distance fields: ONE 2-D CUDA array holding all views tiled in a
-// grid (view i at texel offset ((i % cols) W, (i / cols) H)) behind one texture object.  The fused kernel
-// fetches the 2x2 bilinear footprint with ONE tld4 (tex2Dgather) and applies the exact fp32 weights itself;
-// the hardware's 8-bit-fraction filtering is never used.  A footprint never leaves its view (x0 <= W-2).
-epo_status epo_build_atlas(epo_ctx* ctx, const float* d_dtf, const __half* d_dtf_h, cudaArray_t* atlas_out,
-                           cudaTextureObject_t* tex_out, int* cols_out) {
-  const int N = ctx->N, W = ctx->W, H = ctx->H;
-  const bool half = d_dtf_h != nullptr;
-  int cols = 32768 / W; if (cols < 1) cols = 1; if (cols > N) cols = N;
-  const int rows = (N + cols - 1) / cols;
-  if ((int64_t)rows * H > 65536 || (int64_t)cols * W > 131072)
-    return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "%d views of %dx%d do not fit one 2-D texture atlas", N, W, H);
-  cudaChannelFormatDesc desc = half ? cudaCreateChannelDescHalf() : cudaCreateChannelDesc<float>();
-  const size_t esz = half ? sizeof(__half) : sizeof(float);
-  cudaArray_t arr = nullptr; cudaTextureObject_t t = 0;
-  cudaError_t e = cudaMallocArray(&arr, &desc, (size_t)cols * W, (size_t)rows * H, cudaArrayTextureGather);
-  for (int i = 0; i < N && e == cudaSuccess; ++i) {
-    const void* src = half ? (const void*)(d_dtf_h + (size_t)i * W * H) : (const void*)(d_dtf + (size_t)i * W * H);
-    e = cudaMemcpy2DToArrayAsync(arr, (size_t)(i % cols) * W * esz, (size_t)(i / cols) * H, src, W * esz, W * esz, H,
-                                 cudaMemcpyDeviceToDevice, ctx->stream);
-  }
-  if (e == cudaSuccess) {
-    cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
-    rd.resType = cudaResourceTypeArray; rd.res.array.array = arr;
-    cudaTextureDesc td; memset(&td, 0, sizeof(td));
-    td.addressMode[0] = td.addressMode[1] = cudaAddressModeClamp;
-    td.filterMode = cudaFilterModePoint; td.readMode = cudaReadModeElementType; td.normalizedCoords = 0;
-    e = cudaCreateTextureObject(&t, &rd, &td, nullptr);
-  }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-  if (e != cudaSuccess) {
-    epo_free_atlas(arr, t);
-    return epo_fail(ctx, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "distance-field atlas: %s",
-                    cudaGetErrorString(e));
-  }
-  *atlas_out = arr; *tex_out = t; *cols_out = cols;
   return EPO_OK;
 }
