@@ -182,6 +182,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   float4* pts = nullptr; cudaArray_t atlas = nullptr; cudaTextureObject_t tex = 0; int cols = 1;
   EpoDtfScratch scratch = {nullptr, 0};
   std::vector<int32_t> hoff;
+  bool subsampled = false;
   epo_status rc = EPO_OK;
   cudaError_t e = cudaMalloc(&d_depth, N * px * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&d_e, N * px);
@@ -202,9 +203,9 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
     if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
   }
   tr.mark("copy depth");
-  if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff);
+  if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff, &subsampled);
   tr.mark("edge lists");
-  if (rc == EPO_OK) rc = epo_build_points(c, d_small, off, rec, E, hoff, &pts);
+  if (rc == EPO_OK) rc = epo_build_points(c, d_small, off, rec, E, hoff, d_e, d_depth, subsampled, &pts);
   if (rc == EPO_OK) {
     // commit the small state on the stream, then drain it once
     e = cudaMemcpyAsync(c->d_K, d_small, N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, st);
@@ -256,7 +257,7 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   int32_t* d_user = nullptr;
   EPO_CUDA(c, cudaMalloc(&d_user, (size_t)P * 2 * sizeof(int32_t)));
   cudaError_t e = cudaMemcpyAsync(d_user, hp.data(), (size_t)P * 2 * sizeof(int32_t), cudaMemcpyHostToDevice, st);
-  int2 *canon = nullptr, *work = nullptr; int32_t *perm = nullptr, *toff = nullptr, *soff = nullptr, *sinc = nullptr, *woff = nullptr;
+  int2* canon = nullptr; int4* work = nullptr; int32_t *perm = nullptr, *toff = nullptr, *soff = nullptr, *sinc = nullptr, *woff = nullptr;
   int64_t n_work = 0;
   epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &woff, &n_work)
                                      : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));

@@ -23,7 +23,7 @@ constexpr int kAccStride = 8;
 // Edge pixels handled by one CTA of the fused kernel: kLgOuter passes of kLgThreads threads x kLgPerThread
 // (unrolled) samples.  The point list is padded by kLgChunk entries so that tail lanes may read past a list.
 #ifndef EPO_LG_THREADS
-#define EPO_LG_THREADS 256
+#define EPO_LG_THREADS 128
 #endif
 #ifndef EPO_LG_PER_THREAD
 #define EPO_LG_PER_THREAD 2
@@ -32,7 +32,7 @@ constexpr int kAccStride = 8;
 #define EPO_LG_OUTER 8
 #endif
 #ifndef EPO_LG_MINBLOCKS
-#define EPO_LG_MINBLOCKS 4
+#define EPO_LG_MINBLOCKS 8
 #endif
 constexpr int kLgThreads = EPO_LG_THREADS;
 constexpr int kLgPerThread = EPO_LG_PER_THREAD;
@@ -74,7 +74,7 @@ struct epo_ctx {
   int32_t* d_tgt_off;     // [N+1] CSR by target over canonical ids
   int32_t* d_src_off;     // [N+1]
   int32_t* d_src_inc;     // [P] canonical ids grouped by source, ascending
-  int2* d_work;           // [n_work] (canonical pair, first edge index of the chunk)
+  int4* d_work;           // [n_work] {source, target, first point of the chunk (absolute), samples left}, target-major
   int32_t* d_work_off;    // [P+1] first work item of each canonical pair
   std::vector<int32_t> h_pairs;   // user order, for reprojection counting
 
@@ -120,18 +120,19 @@ epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
 // preprocess.cu
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
                                 int32_t** out_off, EdgeRec** out_rec, int64_t* out_E,
-                                std::vector<int32_t>* h_off);
+                                std::vector<int32_t>* h_off, bool* out_subsampled);
 struct EpoDtfScratch { int32_t* g; cudaSurfaceObject_t surf; };   // alive until the EDT kernels have run
 epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArray_t* atlas, cudaTextureObject_t* tex,
                                int* cols, EpoDtfScratch* scratch);
 void epo_free_dtf_scratch(EpoDtfScratch* s);
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
-                            const std::vector<int32_t>& h_off, float4** out_pts);
+                            const std::vector<int32_t>& h_off, const uint8_t* d_edges_u8, const float* d_depth,
+                            bool subsampled, float4** out_pts);
 void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex);
 // pairs.cu
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
-                           int32_t** out_src_inc, int2** out_work, int32_t** out_work_off, int64_t* out_n_work);
+                           int32_t** out_src_inc, int4** out_work, int32_t** out_work_off, int64_t* out_n_work);
 // lossgrad.cu
 epo_status epo_launch_loss_grad(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)

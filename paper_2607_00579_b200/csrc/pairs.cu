@@ -90,21 +90,27 @@ __global__ void k_chunk_counts(const int2* __restrict__ canon, const int32_t* __
   cnt[p] = (n + chunk - 1) / chunk;
 }
 
-__global__ void k_fill_work(const int32_t* __restrict__ work_off, int64_t P, int chunk, int2* __restrict__ work) {
+// work item = {source, target, first point of the chunk (absolute index into the point list), samples of the
+// source's list from there on}: the fused kernel needs no other table before it can start loading points
+__global__ void k_fill_work(const int32_t* __restrict__ work_off, const int2* __restrict__ canon,
+                            const int32_t* __restrict__ edge_off, int64_t P, int chunk, int4* __restrict__ work) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
+  const int2 st = canon[p];
+  const int e0 = edge_off[st.x], n = edge_off[st.x + 1] - e0;
   int lo = work_off[p], hi = work_off[p + 1];
-  for (int w = lo; w < hi; ++w) work[w] = make_int2((int)p, (w - lo) * chunk);
+  for (int w = lo; w < hi; ++w) work[w] = make_int4(st.x, st.y, e0 + (w - lo) * chunk, n - (w - lo) * chunk);
 }
 
 }  // namespace
 
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2** out_pairs, int32_t** out_perm,
-                           int32_t** out_tgt_off, int32_t** out_src_off, int32_t** out_src_inc, int2** out_work,
+                           int32_t** out_tgt_off, int32_t** out_src_off, int32_t** out_src_inc, int4** out_work,
                            int32_t** out_work_off, int64_t* out_n_work) {
   const int N = ctx->N;
   cudaStream_t st = ctx->stream;
-  int2 *canon = nullptr, *work = nullptr;
+  int2* canon = nullptr;
+  int4* work = nullptr;
   int32_t *perm = nullptr, *tgt_off = nullptr, *src_off = nullptr, *src_inc = nullptr;
   int32_t *cnt = nullptr, *cursor = nullptr, *bucket = nullptr, *chunk_cnt = nullptr, *work_off = nullptr;
   auto free_all = [&]() {
@@ -153,8 +159,8 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
   int32_t n_work = 0;
   PR_CUDA(cudaMemcpyAsync(&n_work, work_off + P, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   PR_CUDA(cudaStreamSynchronize(st));
-  PR_CUDA(cudaMalloc(&work, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int2)));
-  k_fill_work<<<gridP, 256, 0, st>>>(work_off, P, kLgChunk, work);
+  PR_CUDA(cudaMalloc(&work, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int4)));
+  k_fill_work<<<gridP, 256, 0, st>>>(work_off, canon, ctx->d_edge_off, P, kLgChunk, work);
   ctx->launches += 1;
   PR_CUDA(cudaGetLastError());
   PR_CUDA(cudaStreamSynchronize(st));

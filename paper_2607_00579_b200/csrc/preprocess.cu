@@ -228,12 +228,71 @@ __global__ void k_make_points(const EdgeRec* __restrict__ rec, const int32_t* __
   }
 }
 
+// The same points in TILE-MAJOR order (the order the fused kernel consumes; the canonical raster list above is
+// what the API exposes).  Each view is cut into kTile x kTile pixel tiles, tiles in raster order, pixels in
+// raster order inside a tile: 32 consecutive points then follow one or two edge curves through a compact patch
+// of the source image, so the lanes of a warp gather from neighbouring texels of the target field (shared
+// sectors inside one tld4, a compact L1 working set) instead of from 32 unrelated places along an image row.
+// Only the summation order changes.  One warp per (view, tile): two tile rows (32 pixels) per step.
+#ifndef EPO_TILE
+#define EPO_TILE 16
+#endif
+constexpr int kTile = EPO_TILE;   // power of two, 4..32
+
+__device__ __forceinline__ bool tile_pixel(int W, int H, int tx, int ty, int step, int lane, int* u, int* v) {
+  *u = tx * kTile + (lane & (kTile - 1));
+  *v = ty * kTile + step * (32 / kTile) + lane / kTile;
+  return *u < W && *v < H;
+}
+
+__global__ void k_tile_count(const uint8_t* __restrict__ edges, const float* __restrict__ depth, int N, int W, int H,
+                             int tiles_x, int tiles_y, float z_min, int32_t* __restrict__ tile_cnt) {
+  const int lane = threadIdx.x & 31;
+  const int64_t wid = (int64_t)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int64_t per_view = (int64_t)tiles_x * tiles_y;
+  if (wid >= per_view * N) return;
+  const int view = (int)(wid / per_view), t = (int)(wid % per_view), tx = t % tiles_x, ty = t / tiles_x;
+  int cnt = 0;
+  for (int step = 0; step < kTile * kTile / 32; ++step) {
+    int u, v;
+    const bool f = tile_pixel(W, H, tx, ty, step, lane, &u, &v) &&
+                   edge_kept(edges, depth, ((int64_t)view * H + v) * W + u, z_min);
+    cnt += __popc(__ballot_sync(0xffffffffu, f));
+  }
+  if (lane == 0) tile_cnt[wid] = cnt;
+}
+
+__global__ void k_tile_points(const uint8_t* __restrict__ edges, const float* __restrict__ depth, int N, int W, int H,
+                              int tiles_x, int tiles_y, float z_min, const int32_t* __restrict__ tile_off,
+                              const float* __restrict__ K, float4* __restrict__ pts) {
+  const int lane = threadIdx.x & 31;
+  const int64_t wid = (int64_t)blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int64_t per_view = (int64_t)tiles_x * tiles_y;
+  if (wid >= per_view * N) return;
+  const int view = (int)(wid / per_view), t = (int)(wid % per_view), tx = t % tiles_x, ty = t / tiles_x;
+  const float ifx = 1.0f / K[4 * view], ify = 1.0f / K[4 * view + 1], cx = K[4 * view + 2], cy = K[4 * view + 3];
+  int32_t pos = tile_off[wid];
+  for (int step = 0; step < kTile * kTile / 32; ++step) {
+    int u, v;
+    const bool in = tile_pixel(W, H, tx, ty, step, lane, &u, &v);
+    const int64_t idx = ((int64_t)view * H + v) * W + u;
+    const bool f = in && edge_kept(edges, depth, idx, z_min);
+    const unsigned m = __ballot_sync(0xffffffffu, f);
+    if (f) {
+      const float z = depth[idx];
+      pts[pos + __popc(m & ((1u << lane) - 1u))] =
+          make_float4(z * (((float)u - cx) * ifx), z * (((float)v - cy) * ify), z, 0.f);
+    }
+    pos += __popc(m);
+  }
+}
+
 
 }  // namespace
 
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
                                 int32_t** out_off, EdgeRec** out_rec, int64_t* out_E,
-                                std::vector<int32_t>* h_off) {
+                                std::vector<int32_t>* h_off, bool* out_subsampled) {
   const int N = ctx->N, W = ctx->W, H = ctx->H;
   const int64_t rows = (int64_t)N * H;
   cudaStream_t st = ctx->stream;
@@ -273,6 +332,7 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
   bool need_sub = false;
   if (e_max > 0)
     for (int i = 0; i < N; ++i) need_sub |= (hfull[i + 1] - hfull[i]) > e_max;
+  *out_subsampled = need_sub;
   if (!need_sub) {
     *out_off = full_off; *out_rec = full; *out_E = Efull; *h_off = hfull;
     full_off = nullptr; full = nullptr;
@@ -372,18 +432,44 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArra
 }
 
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
-                            const std::vector<int32_t>& h_off, float4** out_pts) {
+                            const std::vector<int32_t>& h_off, const uint8_t* d_edges_u8, const float* d_depth,
+                            bool subsampled, float4** out_pts) {
   float4* pts = nullptr;
+  cudaStream_t st = ctx->stream;
   // padded by one chunk of zeros: the fused kernel's tail lanes read past the end of a list and discard
   EPO_CUDA(ctx, cudaMalloc(&pts, (size_t)(E + kLgChunk) * sizeof(float4)));
-  EPO_CUDA(ctx, cudaMemsetAsync(pts + E, 0, (size_t)kLgChunk * sizeof(float4), ctx->stream));
-  int max_n = 1;
-  for (int i = 0; i < ctx->N; ++i) max_n = h_off[i + 1] - h_off[i] > max_n ? h_off[i + 1] - h_off[i] : max_n;
-  dim3 grid((max_n + 255) / 256, ctx->N);
-  k_make_points<<<grid, 256, 0, ctx->stream>>>(d_rec, d_off, d_K, pts);
-  ctx->launches += 1;
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) { cudaFree(pts); return epo_fail(ctx, EPO_ERR_CUDA, "k_make_points: %s", cudaGetErrorString(e)); }
+  EPO_CUDA(ctx, cudaMemsetAsync(pts + E, 0, (size_t)kLgChunk * sizeof(float4), st));
+  cudaError_t e = cudaSuccess;
+  if (subsampled) {
+    // an E_max sub-sample is defined on the raster list (reading S6): keep its order
+    int max_n = 1;
+    for (int i = 0; i < ctx->N; ++i) max_n = h_off[i + 1] - h_off[i] > max_n ? h_off[i + 1] - h_off[i] : max_n;
+    dim3 grid((max_n + 255) / 256, ctx->N);
+    k_make_points<<<grid, 256, 0, st>>>(d_rec, d_off, d_K, pts);
+    ctx->launches += 1;
+    e = cudaGetLastError();
+  } else {
+    // tile-major: per-(view, tile) counts -> scan -> ordered scatter.  The per-view totals equal the raster
+    // list's (same keep rule), so view i's points occupy [off[i], off[i+1]) in both orders.
+    const int N = ctx->N, W = ctx->W, H = ctx->H;
+    const int tiles_x = (W + kTile - 1) / kTile, tiles_y = (H + kTile - 1) / kTile;
+    const int64_t n_tiles = (int64_t)N * tiles_x * tiles_y;
+    int32_t *tile_cnt = nullptr, *tile_off = nullptr;
+    e = cudaMalloc(&tile_cnt, (size_t)(n_tiles + 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&tile_off, (size_t)(n_tiles + 1) * sizeof(int32_t));
+    if (e == cudaSuccess) {
+      const int grid = (int)((n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock);
+      k_tile_count<<<grid, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, d_depth, N, W, H, tiles_x, tiles_y, ctx->cfg.z_min, tile_cnt);
+      k_exclusive_scan<<<1, 1024, 0, st>>>(tile_cnt, tile_off, n_tiles, 0);
+      k_tile_points<<<grid, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, d_depth, N, W, H, tiles_x, tiles_y, ctx->cfg.z_min,
+                                                          tile_off, d_K, pts);
+      ctx->launches += 3;
+      e = cudaGetLastError();
+      if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // the scratch below is freed on return
+    }
+    cudaFree(tile_cnt); cudaFree(tile_off);
+  }
+  if (e != cudaSuccess) { cudaFree(pts); return epo_fail(ctx, EPO_ERR_CUDA, "point list: %s", cudaGetErrorString(e)); }
   *out_pts = pts;
   return EPO_OK;
 }
