@@ -124,6 +124,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   const size_t N = (size_t)c->N;
   if (e == cudaSuccess) e = cudaMalloc(&c->d_K, N * 4 * sizeof(float));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_poses, N * 12 * sizeof(double));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_poses_next, N * 12 * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_poses_init, N * 12 * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_grad, N * 6 * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_loss_part, N * sizeof(double));
@@ -149,7 +150,7 @@ void epo_destroy(epo_ctx* c) {
   cudaSetDevice(c->cfg.device);
   cudaStreamSynchronize(c->stream);
   free_pairs(c); free_views(c);
-  cudaFree(c->d_K); cudaFree(c->d_poses); cudaFree(c->d_poses_init); cudaFree(c->d_grad); cudaFree(c->d_loss_part);
+  cudaFree(c->d_K); cudaFree(c->d_poses); cudaFree(c->d_poses_next); cudaFree(c->d_poses_init); cudaFree(c->d_grad); cudaFree(c->d_loss_part);
   cudaFree(c->d_m); cudaFree(c->d_v); cudaFree(c->d_dR); cudaFree(c->d_dt); cudaFree(c->d_state);
   cudaFree(c->d_theta); cudaFree(c->d_loss_trace);
   cudaGetLastError();
@@ -297,7 +298,8 @@ epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss
   if (!loss || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_loss_grad: NULL loss or negative lambda");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
-  EPO_TRY(epo_launch_loss_grad(c, lambda, false));
+  EPO_TRY(epo_launch_fused(c, lambda, false));
+  EPO_TRY(epo_launch_finish(c, false, false, false));
   bool sync = false;
   // loss: DevState.loss (double) -> float
   epo_launch_f64_to_f32(st, &c->d_state->loss, c->d_out_f, 1);
@@ -329,10 +331,10 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
   if (n_iters < 0) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_step: negative iteration count");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
-  EPO_TRY(epo_launch_begin_step_call(c));
+  if (n_iters == 0) EPO_TRY(epo_launch_begin_step_call(c));
   for (int i = 0; i < n_iters; ++i) {
-    EPO_TRY(epo_launch_loss_grad(c, -1.0f, true));
-    EPO_TRY(epo_launch_update(c));
+    EPO_TRY(epo_launch_fused(c, -1.0f, true));
+    EPO_TRY(epo_launch_finish(c, true, true, i == 0));
   }
   bool sync = false;
   if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));

@@ -46,6 +46,8 @@ struct DevState {
   int32_t phase;       // 0, 1, 2 (Alg. 2 l.13-17)
   int32_t stopped;     // step >= max_steps, or early_stop && phase == 2
   int32_t iters_done;  // iterations executed since the last epo_step began
+  int32_t ticket;      // CTAs of k_finish that have finished (the last one runs the serial tail and re-zeroes it)
+  int32_t pad_;
   double loss;         // loss of the last evaluation
 };
 
@@ -59,6 +61,7 @@ struct epo_ctx {
   // views
   float* d_K;             // [N][4]
   double* d_poses;        // [N][12] current (fp64: T_ts is formed without fp32 cancellation)
+  double* d_poses_next;   // [N][12] poses after the update in flight (published by the last CTA of k_finish)
   double* d_poses_init;   // [N][12] as given to epo_set_views / epo_reset
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
@@ -99,6 +102,22 @@ struct epo_ctx {
   char err[512];
 };
 
+// relative pose T_ts = T_t T_s^-1 in fp64 (row a-1): entry k of the 3x4 [R_ts | t_ts], R_ts = R_t R_s^T,
+// t_ts = t_t - R_ts t_s  (reading P2: formed in double, rounded once where fp32 is wanted)
+#ifdef __CUDACC__
+__device__ __forceinline__ double rel_pose_entry(const double* Ts, const double* Tt, int k) {
+  int i = k >> 2, j = k & 3;
+  if (j < 3) return Tt[4 * i] * Ts[4 * j] + Tt[4 * i + 1] * Ts[4 * j + 1] + Tt[4 * i + 2] * Ts[4 * j + 2];
+  double r = Tt[4 * i + 3];
+#pragma unroll
+  for (int m = 0; m < 3; ++m) {
+    double Rim = Tt[4 * i] * Ts[4 * m] + Tt[4 * i + 1] * Ts[4 * m + 1] + Tt[4 * i + 2] * Ts[4 * m + 2];
+    r -= Rim * Ts[4 * m + 3];
+  }
+  return r;
+}
+#endif
+
 // ---- error plumbing ---------------------------------------------------------------------------
 epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
 
@@ -134,11 +153,11 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
                            int32_t** out_src_inc, int4** out_work, int32_t** out_work_off, int64_t* out_n_work);
 // lossgrad.cu
-epo_status epo_launch_loss_grad(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
+epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)
-// update.cu
-epo_status epo_launch_update(epo_ctx* ctx);
-epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done, recompute `stopped`
+// update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first);
+epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done (an epo_step call of zero iterations)
 void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n);
 void epo_launch_f32_to_f64(cudaStream_t st, const float* in, double* out, int64_t n);
 void epo_launch_scatter_pair_outputs(cudaStream_t st, const float* pl, const int32_t* pv, const int32_t* perm,

@@ -1,4 +1,5 @@
-// Optimiser side of one iteration (DESIGN.md rows a-10..a-12), one CTA, fp64 (N is a few hundred):
+// Everything of one iteration after the fused kernel (DESIGN.md rows a-9..a-12), one launch, fp64:
+//   PAPER.md:485-486   per-direction mean  sum rho / sum valid;  PAPER.md:91 Eq. 6 mean over pairs
 //   PAPER.md:121       Adam(W) beta=(0.9, 0.999); linear warm-up 0 -> 3e-3 over 25 steps, cosine decay to 2000
 //   PAPER.md:429       OptimizerAndSchedulerStep
 //   PAPER.md:104-110   Eq. 9 / Eq. 10 pose change in degrees, 95th percentiles, theta95 = max
@@ -11,19 +12,40 @@
 namespace {
 
 constexpr double kPi = 3.14159265358979323846;
-constexpr int kUpdThreads = 256;
+constexpr int kFinThreads = 128;
 
-struct UpdParams {
-  double* poses;
-  const double* grad;
-  const double* loss_part;
+struct FinParams {
+  // a-9 inputs: pair lists and the fused kernel's per-CTA partial sums
+  const int2* pairs;
+  const int32_t *tgt_off, *src_off, *src_inc, *work_off;
+  const double* part;
+  float* pair_loss;
+  int32_t* pair_valid;
+  double *grad, *loss_part;
+  // optimiser state
+  double *poses, *poses_next;
   double *m, *v, *dR, *dt, *theta, *loss_trace;
   DevState* state;
   int N;
   int64_t P;
   double lr_max, beta1, beta2, adam_eps, eps1, eps2;
   int warmup, max_steps, w1, w2, smooth, early_stop;
+  int gated, step_mode, call_first;
 };
+
+// sum over the CTA in a fixed order (xor tree inside each warp, then the warps in index order); every thread
+// gets the total.  `scratch` holds kFinThreads / 32 doubles.
+__device__ double block_sum(double v, double* scratch) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();                                  // scratch may still be in use
+  if ((threadIdx.x & 31) == 0) scratch[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double t = 0.0;
+#pragma unroll
+  for (int w = 0; w < kFinThreads / 32; ++w) t += scratch[w];
+  return t;
+}
 
 __device__ double lr_of_step(int s, double lr_max, int warmup, int max_steps) {
   if (s < warmup) return lr_max * (double)(s + 1) / (double)warmup;
@@ -60,7 +82,20 @@ __device__ void se3_exp(const double* e, double* T) {
 
 __device__ __forceinline__ double clip1(double c) { return c > 1.0 ? 1.0 : (c < -1.0 ? -1.0 : c); }
 
-// value of rank k (0-based, ties broken by index) among x[0..n): every thread scans all of x
+// per-pair sums = the pair's per-CTA partials of the fused kernel added in a fixed order: lane l adds value
+// (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... then the four chunk classes are combined by two xor-shuffles.
+// All 32 loads of a step are independent (one L2 round trip per four chunks instead of one per value).
+// Every lane returns the total of value (lane & 7).
+__device__ __forceinline__ double pair_value(const FinParams& p, int q, int lane) {
+  const int w1 = p.work_off[q + 1];
+  double s = 0.0;
+  for (int w = p.work_off[q] + (lane >> 3); w < w1; w += 4) s += __ldcg(p.part + (size_t)w * kAccStride + (lane & 7));
+  s += __shfl_xor_sync(0xffffffffu, s, 8);
+  s += __shfl_xor_sync(0xffffffffu, s, 16);
+  return s;
+}
+
+// value of ranks k and k+1 (0-based, ties broken by index) among x[0..n): every thread scans all of x
 __device__ void select_two(const double* x, int n, int k, double* lo, double* hi) {
   for (int i = threadIdx.x; i < n; i += blockDim.x) {
     const double xi = x[i];
@@ -71,94 +106,176 @@ __device__ void select_two(const double* x, int n, int k, double* lo, double* hi
   }
 }
 
-// Converged(theta_{0..s}; w, eps)  (smooth: PAPER.md:357; raw: PAPER.md:114)
-__device__ bool converged(const double* theta, int s, int w, double eps, int smooth) {
-  if (smooth) {
-    if (s < 2 * w - 2) return false;
-    for (int k = s - w + 1; k <= s; ++k) {
+// Converged(theta_{0..s}; w, eps)  (smooth: PAPER.md:357; raw: PAPER.md:114), evaluated by the whole CTA:
+// thread k < w tests the window ending at step s - k (its mean is summed in time order).
+__device__ bool converged(const double* theta, double theta_s, int s, int w, double eps, int smooth) {
+  const int need = smooth ? 2 * w - 2 : w - 1;
+  if (s < need) return false;                       // uniform
+  bool ok = true;
+  const int k = threadIdx.x;
+  if (k < w) {
+    auto th = [&](int j) { return j == s ? theta_s : __ldcg(theta + j); };
+    if (smooth) {
       double m = 0.0;
-      for (int j = k - w + 1; j <= k; ++j) m += theta[j];
-      if (!(m / w < eps)) return false;
+      for (int j = s - k - w + 1; j <= s - k; ++j) m += th(j);
+      ok = m / w < eps;
+    } else {
+      ok = th(s - k) < eps;
     }
-    return true;
   }
-  if (s < w - 1) return false;
-  for (int k = s - w + 1; k <= s; ++k) if (!(theta[k] < eps)) return false;
-  return true;
+  return __syncthreads_and(ok) != 0;
 }
 
-__global__ void __launch_bounds__(kUpdThreads) k_update(const UpdParams p) {
+// ---------------------------------------------------------------------------------------------------------
+// k_finish: everything of one iteration after the fused kernel, in ONE launch of N CTAs (one per camera c).
+//  a-9   g_c = (1/P) [ sum_{p: t=c} [A; M]_p / n_p  -  sum_{p: s=c} Ad_{T_ts}^T [A; M]_p / n_p ]   (identity I1:
+//        G_src = [-R^T A ; -R^T (M - t x A)]), L_p = S_p / n_p, per-target loss sums.  One warp per pair.
+//  a-10  (step mode) Adam on the six coordinates (lanes 2..7 of warp 0), SE(3) exponential and T_c <- Exp(eps) T_c
+//        by one thread, written to the NEXT pose buffer: other CTAs still read the current poses.
+//  a-11  per-camera pose change; then the LAST CTA to finish (atomic ticket) publishes the new poses, takes the
+//  a-12  two 95th percentiles, runs the windowed two-phase test and advances the device control block.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   DevState* st = p.state;
-  if (st->stopped) return;
-  __shared__ double sred[kUpdThreads];
-  __shared__ double sel[4];
-  const int tid = threadIdx.x, s = st->step, N = p.N;
-  // total loss of this evaluation (fixed-order tree)
-  double lv = 0.0;
-  for (int i = tid; i < N; i += kUpdThreads) lv += p.loss_part[i];
-  sred[tid] = lv;
-  __syncthreads();
-  for (int o = kUpdThreads / 2; o > 0; o >>= 1) { if (tid < o) sred[tid] += sred[tid + o]; __syncthreads(); }
-  const double loss = sred[0] / (double)p.P;
-  // a-10 Adam + retraction, a-11 per-camera pose change
-  const double lr = lr_of_step(s, p.lr_max, p.warmup, p.max_steps);
-  const double c1 = 1.0 - pow(p.beta1, (double)(s + 1)), c2 = 1.0 - pow(p.beta2, (double)(s + 1));
-  for (int c = tid; c < N; c += kUpdThreads) {
-    double eps[6], E[12], T[12], Tn[12];
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-      const double g = p.grad[6 * c + k];
-      const double m = p.beta1 * p.m[6 * c + k] + (1.0 - p.beta1) * g;
-      const double v = p.beta2 * p.v[6 * c + k] + (1.0 - p.beta2) * g * g;
-      p.m[6 * c + k] = m; p.v[6 * c + k] = v;
-      eps[k] = -lr * (m / c1) / (sqrt(v / c2) + p.adam_eps);
-    }
-    se3_exp(eps, E);
-#pragma unroll
-    for (int k = 0; k < 12; ++k) T[k] = p.poses[12 * c + k];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) Tn[4 * i + j] = E[4 * i] * T[j] + E[4 * i + 1] * T[4 + j] + E[4 * i + 2] * T[8 + j];
-      Tn[4 * i + 3] += E[4 * i + 3];
-    }
-    double tr = 0.0;   // Eq. 9: tr(R^s (R^{s-1})^T)
-#pragma unroll
-    for (int i = 0; i < 3; ++i)
-#pragma unroll
-      for (int j = 0; j < 3; ++j) tr += Tn[4 * i + j] * T[4 * i + j];
-    p.dR[c] = (180.0 / kPi) * acos(clip1((tr - 1.0) / 2.0));
-    const double na = sqrt(Tn[3] * Tn[3] + Tn[7] * Tn[7] + Tn[11] * Tn[11]);
-    const double nb = sqrt(T[3] * T[3] + T[7] * T[7] + T[11] * T[11]);
-    double dtc = 0.0;  // Eq. 10; 0 if either norm < 1e-12 (reading S13)
-    if (na >= 1e-12 && nb >= 1e-12)
-      dtc = (180.0 / kPi) * acos(clip1((Tn[3] / na) * (T[3] / nb) + (Tn[7] / na) * (T[7] / nb) + (Tn[11] / na) * (T[11] / nb)));
-    p.dt[c] = dtc;
-#pragma unroll
-    for (int k = 0; k < 12; ++k) p.poses[12 * c + k] = Tn[k];
+  if (p.gated && st->stopped) {
+    if (p.call_first && blockIdx.x == 0 && threadIdx.x == 0) st->iters_done = 0;
+    return;
   }
-  __syncthreads();   // dR/dt written by this CTA are visible to it after the barrier
+  extern __shared__ double sdyn[];                 // last CTA: dR[N], dt[N]
+  __shared__ double sg[kFinThreads / 32][8];
+  __shared__ double sel[4];
+  __shared__ int s_last;
+  const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = p.N;
+  const double* Pc = p.poses + 12 * (size_t)c;
+  // ---- a-9: lane 0 accumulates the loss sum, lanes 2..7 the six gradient coordinates
+  double acc = 0.0;
+  for (int q = p.tgt_off[c] + warp; q < p.tgt_off[c + 1]; q += kFinThreads / 32) {
+    const double v = pair_value(p, q, lane);
+    const double S = __shfl_sync(0xffffffffu, v, 0), n = __shfl_sync(0xffffffffu, v, 1);
+    const double L = n > 0.0 ? S / n : 0.0;
+    if (lane == 0) { p.pair_loss[q] = (float)L; p.pair_valid[q] = (int32_t)n; acc += L; }
+    else if (lane >= 2 && lane < 8 && n > 0.0) acc += v / n;
+  }
+  for (int j = p.src_off[c] + warp; j < p.src_off[c + 1]; j += kFinThreads / 32) {
+    const int q = p.src_inc[j];
+    const double v = pair_value(p, q, lane);
+    const double n = __shfl_sync(0xffffffffu, v, 1);
+    const double A0 = __shfl_sync(0xffffffffu, v, 2), A1 = __shfl_sync(0xffffffffu, v, 3), A2 = __shfl_sync(0xffffffffu, v, 4);
+    double m0 = __shfl_sync(0xffffffffu, v, 5), m1 = __shfl_sync(0xffffffffu, v, 6), m2 = __shfl_sync(0xffffffffu, v, 7);
+    if (lane >= 2 && lane < 8 && n > 0.0) {
+      const double* Pt = p.poses + 12 * (size_t)p.pairs[q].y;
+      const int i = (lane - 2) % 3;
+      const double r0 = rel_pose_entry(Pc, Pt, i), r1 = rel_pose_entry(Pc, Pt, 4 + i), r2 = rel_pose_entry(Pc, Pt, 8 + i);
+      if (lane < 5) {
+        acc -= (r0 * A0 + r1 * A1 + r2 * A2) / n;                      // R^T A
+      } else {
+        const double t0 = rel_pose_entry(Pc, Pt, 3), t1 = rel_pose_entry(Pc, Pt, 7), t2 = rel_pose_entry(Pc, Pt, 11);
+        m0 -= t1 * A2 - t2 * A1; m1 -= t2 * A0 - t0 * A2; m2 -= t0 * A1 - t1 * A0;   // M' = M - t_ts x A
+        acc -= (r0 * m0 + r1 * m1 + r2 * m2) / n;                      // R^T M'
+      }
+    }
+  }
+  if (lane < 8) sg[warp][lane] = acc;
+  __syncthreads();
+  double g = 0.0;                                    // warp 0, lane k < 8: sum over warps in a fixed order
+  if (tid < 8) {
+#pragma unroll
+    for (int w = 0; w < kFinThreads / 32; ++w) g += sg[w][tid];
+    if (tid == 0) p.loss_part[c] = g;
+    else if (tid >= 2) { g /= (double)p.P; p.grad[6 * (size_t)c + tid - 2] = g; }
+  }
+  if (!p.step_mode) {
+    // evaluation only (epo_loss_grad): the last CTA adds the per-target loss sums
+    if (tid == 0) { __threadfence(); s_last = atomicAdd(&st->ticket, 1) == N - 1; }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double lv = 0.0;
+    for (int i = tid; i < N; i += kFinThreads) lv += __ldcg(p.loss_part + i);
+    const double tot = block_sum(lv, &sg[0][0]);
+    if (tid == 0) { st->loss = tot / (double)p.P; st->ticket = 0; }
+    return;
+  }
+  // ---- a-10 Adam (lanes 2..7 of warp 0), a-12 learning rate
+  const int s = st->step;
+  if (warp == 0) {
+    double eps = 0.0;
+    if (lane >= 2 && lane < 8) {
+      const size_t k = 6 * (size_t)c + lane - 2;
+      const double lr = lr_of_step(s, p.lr_max, p.warmup, p.max_steps);
+      const double c1 = 1.0 - pow(p.beta1, (double)(s + 1)), c2 = 1.0 - pow(p.beta2, (double)(s + 1));
+      const double m = p.beta1 * p.m[k] + (1.0 - p.beta1) * g;
+      const double v = p.beta2 * p.v[k] + (1.0 - p.beta2) * g * g;
+      p.m[k] = m; p.v[k] = v;
+      eps = -lr * (m / c1) / (sqrt(v / c2) + p.adam_eps);
+    }
+    double e[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) e[k] = __shfl_sync(0xffffffffu, eps, 2 + k);
+    if (lane == 0) {
+      // retraction T_c <- Exp(eps) T_c and a-11 pose change of this camera
+      double E[12], T[12], Tn[12];
+      se3_exp(e, E);
+#pragma unroll
+      for (int k = 0; k < 12; ++k) T[k] = Pc[k];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) Tn[4 * i + j] = E[4 * i] * T[j] + E[4 * i + 1] * T[4 + j] + E[4 * i + 2] * T[8 + j];
+        Tn[4 * i + 3] += E[4 * i + 3];
+      }
+      double tr = 0.0;   // Eq. 9: tr(R^s (R^{s-1})^T)
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) tr += Tn[4 * i + j] * T[4 * i + j];
+      p.dR[c] = (180.0 / kPi) * acos(clip1((tr - 1.0) / 2.0));
+      const double na = sqrt(Tn[3] * Tn[3] + Tn[7] * Tn[7] + Tn[11] * Tn[11]);
+      const double nb = sqrt(T[3] * T[3] + T[7] * T[7] + T[11] * T[11]);
+      double dtc = 0.0;  // Eq. 10; 0 if either norm < 1e-12 (reading S13)
+      if (na >= 1e-12 && nb >= 1e-12)
+        dtc = (180.0 / kPi) * acos(clip1((Tn[3] / na) * (T[3] / nb) + (Tn[7] / na) * (T[7] / nb) + (Tn[11] / na) * (T[11] / nb)));
+      p.dt[c] = dtc;
+#pragma unroll
+      for (int k = 0; k < 12; ++k) p.poses_next[12 * (size_t)c + k] = Tn[k];
+      __threadfence();                               // this camera's outputs before its ticket
+      s_last = atomicAdd(&st->ticket, 1) == N - 1;
+    }
+  }
+  __syncthreads();
+  if (!s_last) return;
+  // ---- last CTA: every camera has been reduced and stepped; nobody reads the current poses any more
+  __threadfence();
+  double* sdR = sdyn; double* sdt = sdyn + N;
+  double lv = 0.0;
+  for (int i = tid; i < N; i += kFinThreads) {
+    sdR[i] = __ldcg(p.dR + i); sdt[i] = __ldcg(p.dt + i);
+    lv += __ldcg(p.loss_part + i);
+  }
+  for (int i = tid; i < 12 * N; i += kFinThreads) p.poses[i] = __ldcg(p.poses_next + i);
+  const double loss = block_sum(lv, &sg[0][0]) / (double)p.P;     // (contains the barrier that publishes sdR / sdt)
   // 95th percentiles, linear interpolation at rank 0.95 (N-1) (reading S12)
   const double rank = 95.0 / 100.0 * (double)(N - 1);
   const int k0 = (int)floor(rank);
   const double fr = rank - (double)k0;
-  select_two(p.dR, N, k0, &sel[0], &sel[1]);
-  select_two(p.dt, N, k0, &sel[2], &sel[3]);
+  select_two(sdR, N, k0, &sel[0], &sel[1]);
+  select_two(sdt, N, k0, &sel[2], &sel[3]);
   __syncthreads();
+  const double r95 = (k0 + 1 < N) ? sel[0] + fr * (sel[1] - sel[0]) : sel[0];
+  const double t95 = (k0 + 1 < N) ? sel[2] + fr * (sel[3] - sel[2]) : sel[2];
+  const double th = r95 > t95 ? r95 : t95;
+  int phase = st->phase;
+  if (phase == 0) { if (converged(p.theta, th, s, p.w1, p.eps1, p.smooth)) phase = 1; }
+  else if (phase == 1) { if (converged(p.theta, th, s, p.w2, p.eps2, p.smooth)) phase = 2; }
   if (tid == 0) {
-    const double r95 = (k0 + 1 < N) ? sel[0] + fr * (sel[1] - sel[0]) : sel[0];
-    const double t95 = (k0 + 1 < N) ? sel[2] + fr * (sel[3] - sel[2]) : sel[2];
-    const double th = r95 > t95 ? r95 : t95;
     p.theta[s] = th;
     p.loss_trace[s] = loss;
     st->loss = loss;
-    int phase = st->phase;
-    if (phase == 0) { if (converged(p.theta, s, p.w1, p.eps1, p.smooth)) phase = 1; }
-    else if (phase == 1) { if (converged(p.theta, s, p.w2, p.eps2, p.smooth)) phase = 2; }
     st->phase = phase;
     st->step = s + 1;
-    st->iters_done += 1;
+    st->iters_done = p.call_first ? 1 : st->iters_done + 1;
     st->stopped = (s + 1 >= p.max_steps) || (p.early_stop && phase == 2);
+    st->ticket = 0;
   }
 }
 
@@ -178,15 +295,23 @@ __global__ void k_f32_to_f64(const float* __restrict__ in, double* __restrict__ 
 
 }  // namespace
 
-epo_status epo_launch_update(epo_ctx* ctx) {
-  UpdParams p;
-  p.poses = ctx->d_poses; p.grad = ctx->d_grad; p.loss_part = ctx->d_loss_part; p.m = ctx->d_m; p.v = ctx->d_v;
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first) {
+  FinParams p;
+  p.pairs = ctx->d_pairs; p.tgt_off = ctx->d_tgt_off; p.src_off = ctx->d_src_off; p.src_inc = ctx->d_src_inc;
+  p.work_off = ctx->d_work_off; p.part = ctx->d_part; p.pair_loss = ctx->d_pair_loss; p.pair_valid = ctx->d_pair_valid;
+  p.grad = ctx->d_grad; p.loss_part = ctx->d_loss_part;
+  p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.m = ctx->d_m; p.v = ctx->d_v;
   p.dR = ctx->d_dR; p.dt = ctx->d_dt; p.theta = ctx->d_theta; p.loss_trace = ctx->d_loss_trace;
   p.state = ctx->d_state; p.N = ctx->N; p.P = ctx->P;
   p.lr_max = ctx->cfg.lr_max; p.beta1 = ctx->cfg.beta1; p.beta2 = ctx->cfg.beta2; p.adam_eps = ctx->cfg.adam_eps;
   p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.warmup = ctx->cfg.warmup_steps; p.max_steps = ctx->cfg.max_steps;
   p.w1 = ctx->cfg.w1; p.w2 = ctx->cfg.w2; p.smooth = ctx->cfg.smooth_window; p.early_stop = ctx->cfg.early_stop;
-  k_update<<<1, kUpdThreads, 0, ctx->stream>>>(p);
+  p.gated = gated ? 1 : 0; p.step_mode = step_mode ? 1 : 0; p.call_first = call_first ? 1 : 0;
+  const size_t smem = (size_t)2 * ctx->N * sizeof(double);   // the last CTA's copy of dR, dt
+  if (smem > 200 * 1024) return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "more than %d views", 200 * 1024 / 16);
+  if (smem > 48 * 1024)
+    EPO_CUDA(ctx, cudaFuncSetAttribute(k_finish, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_finish<<<ctx->N, kFinThreads, smem, ctx->stream>>>(p);
   ctx->launches += 1;
   EPO_CUDA(ctx, cudaGetLastError());
   return EPO_OK;
