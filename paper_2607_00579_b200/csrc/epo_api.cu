@@ -120,6 +120,8 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   c->N = cfg->n_views; c->W = cfg->width; c->H = cfg->height;
   c->have_views = c->have_pairs = false; c->P = c->E = c->n_work = c->reproj_per_eval = c->launches = 0;
   c->err[0] = 0;
+  { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
+  c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
   const size_t N = (size_t)c->N;
   if (e == cudaSuccess) e = cudaMalloc(&c->d_K, N * 4 * sizeof(float));
@@ -234,7 +236,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   free_pairs(c); free_views(c);
   c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff;
   c->d_pts = pts; c->dtf_atlas = atlas; c->dtf_tex = tex; c->atlas_cols = cols;
-  c->have_views = true;
+  c->have_views = true; c->static_dirty = true;
   tr.mark("free temporaries");
   return EPO_OK;
 }
@@ -286,7 +288,7 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   c->d_pairs = canon; c->d_perm = perm; c->d_tgt_off = toff; c->d_src_off = soff; c->d_src_inc = sinc; c->d_work = work;
   c->d_work_off = woff; c->n_work = n_work; c->P = P; c->d_part = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
   c->h_pairs.swap(hp); c->reproj_per_eval = reproj;
-  c->have_pairs = true;
+  c->have_pairs = true; c->static_dirty = true;
   EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, (size_t)c->N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
   EPO_TRY(reset_optimiser(c));
   return EPO_OK;

@@ -56,6 +56,8 @@ struct epo_ctx {
   cudaStream_t stream;
   int N, W, H;
   bool have_views, have_pairs;
+  bool pdl;            // programmatic dependent launch between the kernels of the loop (EPO_NO_PDL=1 turns it off)
+  bool static_dirty;   // work list / points / fields were (re)built since the last fused launch: launch it serialised
   int64_t P, E, n_work, reproj_per_eval, launches;
 
   // views

@@ -12,7 +12,7 @@
 namespace {
 
 constexpr double kPi = 3.14159265358979323846;
-constexpr int kFinThreads = 128;
+constexpr int kFinThreads = 256;
 
 struct FinParams {
   // a-9 inputs: pair lists and the fused kernel's per-CTA partial sums
@@ -82,19 +82,6 @@ __device__ void se3_exp(const double* e, double* T) {
 
 __device__ __forceinline__ double clip1(double c) { return c > 1.0 ? 1.0 : (c < -1.0 ? -1.0 : c); }
 
-// per-pair sums = the pair's per-CTA partials of the fused kernel added in a fixed order: lane l adds value
-// (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... then the four chunk classes are combined by two xor-shuffles.
-// All 32 loads of a step are independent (one L2 round trip per four chunks instead of one per value).
-// Every lane returns the total of value (lane & 7).
-__device__ __forceinline__ double pair_value(const FinParams& p, int q, int lane) {
-  const int w1 = p.work_off[q + 1];
-  double s = 0.0;
-  for (int w = p.work_off[q] + (lane >> 3); w < w1; w += 4) s += __ldcg(p.part + (size_t)w * kAccStride + (lane & 7));
-  s += __shfl_xor_sync(0xffffffffu, s, 8);
-  s += __shfl_xor_sync(0xffffffffu, s, 16);
-  return s;
-}
-
 // value of ranks k and k+1 (0-based, ties broken by index) among x[0..n): every thread scans all of x
 __device__ void select_two(const double* x, int n, int k, double* lo, double* hi) {
   for (int i = threadIdx.x; i < n; i += blockDim.x) {
@@ -137,41 +124,59 @@ __device__ bool converged(const double* theta, double theta_s, int s, int w, dou
 // ---------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   DevState* st = p.state;
-  if (p.gated && st->stopped) {
-    if (p.call_first && blockIdx.x == 0 && threadIdx.x == 0) st->iters_done = 0;
-    return;
-  }
   extern __shared__ double sdyn[];                 // last CTA: dR[N], dt[N]
   __shared__ double sg[kFinThreads / 32][8];
   __shared__ double sel[4];
   __shared__ int s_last;
   const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = p.N;
-  const double* Pc = p.poses + 12 * (size_t)c;
-  // ---- a-9: lane 0 accumulates the loss sum, lanes 2..7 the six gradient coordinates
-  double acc = 0.0;
-  for (int q = p.tgt_off[c] + warp; q < p.tgt_off[c + 1]; q += kFinThreads / 32) {
-    const double v = pair_value(p, q, lane);
-    const double S = __shfl_sync(0xffffffffu, v, 0), n = __shfl_sync(0xffffffffu, v, 1);
-    const double L = n > 0.0 ? S / n : 0.0;
-    if (lane == 0) { p.pair_loss[q] = (float)L; p.pair_valid[q] = (int32_t)n; acc += L; }
-    else if (lane >= 2 && lane < 8 && n > 0.0) acc += v / n;
+  constexpr int kWarps = kFinThreads / 32;
+  // The pair lists are static: read this camera's ranges and this warp's first pair before waiting for the
+  // fused kernel (programmatic dependent launch: this prologue overlaps the fused kernel's tail).
+  const int t0 = p.tgt_off[c], nt = p.tgt_off[c + 1] - t0, s0 = p.src_off[c], n_inc = nt + p.src_off[c + 1] - s0;
+  auto pair_of = [&](int j) { return j < nt ? t0 + j : p.src_inc[s0 + j - nt]; };
+  int j = warp, q = 0, w0 = 0, w1 = 0;
+  if (j < n_inc) { q = pair_of(j); w0 = p.work_off[q]; w1 = p.work_off[q + 1]; }
+  cudaTriggerProgrammaticLaunchCompletion();       // the next fused kernel may start its own static prologue
+  cudaGridDependencySynchronize();                 // partial sums, poses and the control block are final now
+  if (p.gated && st->stopped) {
+    if (p.call_first && blockIdx.x == 0 && threadIdx.x == 0) st->iters_done = 0;
+    return;
   }
-  for (int j = p.src_off[c] + warp; j < p.src_off[c + 1]; j += kFinThreads / 32) {
-    const int q = p.src_inc[j];
-    const double v = pair_value(p, q, lane);
+  const double* Pc = p.poses + 12 * (size_t)c;
+  // ---- a-9: one warp per incident pair (first the pairs with target c, then those with source c); lane 0
+  // accumulates the loss sum, lanes 2..7 the six gradient coordinates
+  double acc = 0.0;
+  while (j < n_inc) {
+    // per-pair sums: lane l adds value (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... (independent loads), then
+    // the four chunk classes are combined by two xor-shuffles: a fixed order
+    double v = 0.0;
+    for (int w = w0 + (lane >> 3); w < w1; w += 4) v += __ldcg(p.part + (size_t)w * kAccStride + (lane & 7));
+    const bool tgt = j < nt;
+    const int qc = q;
+    j += kWarps;
+    if (j < n_inc) { q = pair_of(j); w0 = p.work_off[q]; w1 = p.work_off[q + 1]; }   // next pair's range, in flight
+    v += __shfl_xor_sync(0xffffffffu, v, 8);
+    v += __shfl_xor_sync(0xffffffffu, v, 16);
     const double n = __shfl_sync(0xffffffffu, v, 1);
-    const double A0 = __shfl_sync(0xffffffffu, v, 2), A1 = __shfl_sync(0xffffffffu, v, 3), A2 = __shfl_sync(0xffffffffu, v, 4);
-    double m0 = __shfl_sync(0xffffffffu, v, 5), m1 = __shfl_sync(0xffffffffu, v, 6), m2 = __shfl_sync(0xffffffffu, v, 7);
-    if (lane >= 2 && lane < 8 && n > 0.0) {
-      const double* Pt = p.poses + 12 * (size_t)p.pairs[q].y;
-      const int i = (lane - 2) % 3;
-      const double r0 = rel_pose_entry(Pc, Pt, i), r1 = rel_pose_entry(Pc, Pt, 4 + i), r2 = rel_pose_entry(Pc, Pt, 8 + i);
-      if (lane < 5) {
-        acc -= (r0 * A0 + r1 * A1 + r2 * A2) / n;                      // R^T A
-      } else {
-        const double t0 = rel_pose_entry(Pc, Pt, 3), t1 = rel_pose_entry(Pc, Pt, 7), t2 = rel_pose_entry(Pc, Pt, 11);
-        m0 -= t1 * A2 - t2 * A1; m1 -= t2 * A0 - t0 * A2; m2 -= t0 * A1 - t1 * A0;   // M' = M - t_ts x A
-        acc -= (r0 * m0 + r1 * m1 + r2 * m2) / n;                      // R^T M'
+    if (tgt) {
+      const double S = __shfl_sync(0xffffffffu, v, 0);
+      const double L = n > 0.0 ? S / n : 0.0;
+      if (lane == 0) { p.pair_loss[qc] = (float)L; p.pair_valid[qc] = (int32_t)n; acc += L; }
+      else if (lane >= 2 && lane < 8 && n > 0.0) acc += v / n;
+    } else {
+      const double A0 = __shfl_sync(0xffffffffu, v, 2), A1 = __shfl_sync(0xffffffffu, v, 3), A2 = __shfl_sync(0xffffffffu, v, 4);
+      double m0 = __shfl_sync(0xffffffffu, v, 5), m1 = __shfl_sync(0xffffffffu, v, 6), m2 = __shfl_sync(0xffffffffu, v, 7);
+      if (lane >= 2 && lane < 8 && n > 0.0) {
+        const double* Pt = p.poses + 12 * (size_t)p.pairs[qc].y;
+        const int i = (lane - 2) % 3;
+        const double r0 = rel_pose_entry(Pc, Pt, i), r1 = rel_pose_entry(Pc, Pt, 4 + i), r2 = rel_pose_entry(Pc, Pt, 8 + i);
+        if (lane < 5) {
+          acc -= (r0 * A0 + r1 * A1 + r2 * A2) / n;                      // R^T A
+        } else {
+          const double t0 = rel_pose_entry(Pc, Pt, 3), t1 = rel_pose_entry(Pc, Pt, 7), t2 = rel_pose_entry(Pc, Pt, 11);
+          m0 -= t1 * A2 - t2 * A1; m1 -= t2 * A0 - t0 * A2; m2 -= t0 * A1 - t1 * A0;   // M' = M - t_ts x A
+          acc -= (r0 * m0 + r1 * m1 + r2 * m2) / n;                      // R^T M'
+        }
       }
     }
   }
@@ -311,7 +316,14 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   if (smem > 200 * 1024) return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "more than %d views", 200 * 1024 / 16);
   if (smem > 48 * 1024)
     EPO_CUDA(ctx, cudaFuncSetAttribute(k_finish, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_finish<<<ctx->N, kFinThreads, smem, ctx->stream>>>(p);
+  // programmatic dependent launch: the CTAs may become resident while the fused kernel drains; they wait in
+  // cudaGridDependencySynchronize() before touching anything it (or an earlier kernel) wrote
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3((unsigned)ctx->N); lc.blockDim = dim3(kFinThreads); lc.dynamicSmemBytes = smem; lc.stream = ctx->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = ctx->pdl ? 1 : 0;
+  EPO_CUDA(ctx, cudaLaunchKernelEx(&lc, k_finish, p));
   ctx->launches += 1;
   EPO_CUDA(ctx, cudaGetLastError());
   return EPO_OK;
