@@ -59,9 +59,8 @@ cudaError_t copy_out(void* dst, const void* src, size_t bytes, cudaStream_t st, 
 
 void free_views(epo_ctx* c) {
   cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_pts);
-  epo_free_atlas(c->dtf_atlas, c->dtf_tex);
+  epo_free_atlas(&c->atlas);
   c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_pts = nullptr;
-  c->dtf_atlas = nullptr; c->dtf_tex = 0;
   c->have_views = false;
 }
 void free_pairs(epo_ctx* c) {
@@ -120,6 +119,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   c->N = cfg->n_views; c->W = cfg->width; c->H = cfg->height;
   c->have_views = c->have_pairs = false; c->P = c->E = c->n_work = c->reproj_per_eval = c->launches = 0;
   c->err[0] = 0;
+  c->atlas = EpoAtlas{nullptr, nullptr, 0, 0, 1};
   { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
   c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
@@ -182,8 +182,8 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   PhaseTrace tr(st, "epo_set_views");
   float* d_depth = nullptr; uint8_t* d_e = nullptr; float* d_small = nullptr;
   int32_t* off = nullptr; EdgeRec* rec = nullptr; int64_t E = 0;
-  float4* pts = nullptr; cudaArray_t atlas = nullptr; cudaTextureObject_t tex = 0; int cols = 1;
-  EpoDtfScratch scratch = {nullptr, 0};
+  float4* pts = nullptr; EpoAtlas atlas = {nullptr, nullptr, 0, 0, 1};
+  EpoDtfScratch scratch = {nullptr, 0, 0};
   std::vector<int32_t> hoff;
   bool subsampled = false;
   epo_status rc = EPO_OK;
@@ -199,7 +199,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
     rc = epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_set_views: %s",
                   cudaGetErrorString(e));
   tr.mark("copy edges");
-  if (rc == EPO_OK) rc = epo_build_dtf_atlas(c, d_e, &atlas, &tex, &cols, &scratch);
+  if (rc == EPO_OK) rc = epo_build_dtf_atlas(c, d_e, &atlas, &scratch);
   tr.mark("distance fields");
   if (rc == EPO_OK) {
     e = copy_in(d_depth, depth, N * px * sizeof(float), st);
@@ -230,12 +230,12 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
     // d_K / d_poses may have been overwritten only if every build step succeeded and the final drain failed
     // (a sticky CUDA error: the context is unusable anyway)
     cudaGetLastError();
-    cudaFree(off); cudaFree(rec); cudaFree(pts); epo_free_atlas(atlas, tex);
+    cudaFree(off); cudaFree(rec); cudaFree(pts); epo_free_atlas(&atlas);
     return rc;
   }
   free_pairs(c); free_views(c);
   c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff;
-  c->d_pts = pts; c->dtf_atlas = atlas; c->dtf_tex = tex; c->atlas_cols = cols;
+  c->d_pts = pts; c->atlas = atlas;
   c->have_views = true; c->static_dirty = true;
   tr.mark("free temporaries");
   return EPO_OK;
@@ -441,10 +441,10 @@ epo_status epo_get_dtf(epo_ctx* c, int32_t view, float* dtf) {
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   // the field lives only in the atlas the kernel samples: read view's tile back (fp16 fields are widened)
   const size_t W = (size_t)c->W, H = (size_t)c->H;
-  const size_t ax = (size_t)(view % c->atlas_cols) * W, ay = (size_t)(view / c->atlas_cols) * H;
+  const size_t ax = (size_t)(view % c->atlas.cols) * W, ay = (size_t)(view / c->atlas.cols) * H;
   if (c->cfg.dtf_format == 1) {
     std::vector<__half> h(W * H);
-    EPO_CUDA(c, cudaMemcpy2DFromArrayAsync(h.data(), W * sizeof(__half), c->dtf_atlas, ax * sizeof(__half), ay,
+    EPO_CUDA(c, cudaMemcpy2DFromArrayAsync(h.data(), W * sizeof(__half), c->atlas.arr, ax * sizeof(__half), ay,
                                            W * sizeof(__half), H, cudaMemcpyDeviceToHost, c->stream));
     EPO_CUDA(c, cudaStreamSynchronize(c->stream));
     std::vector<float> f(W * H);
@@ -454,7 +454,7 @@ epo_status epo_get_dtf(epo_ctx* c, int32_t view, float* dtf) {
     return EPO_OK;
   }
   const bool dev = is_device_ptr(dtf);
-  EPO_CUDA(c, cudaMemcpy2DFromArrayAsync(dtf, W * sizeof(float), c->dtf_atlas, ax * sizeof(float), ay, W * sizeof(float), H,
+  EPO_CUDA(c, cudaMemcpy2DFromArrayAsync(dtf, W * sizeof(float), c->atlas.arr, ax * sizeof(float), ay, W * sizeof(float), H,
                                          dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
   if (!dev) EPO_CUDA(c, cudaStreamSynchronize(c->stream));
   return EPO_OK;

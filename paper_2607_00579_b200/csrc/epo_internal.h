@@ -51,6 +51,22 @@ struct DevState {
   double loss;         // loss of the last evaluation
 };
 
+// All distance fields in block-linear, gather-enabled 2-D CUDA arrays, views tiled in a grid: view i sits at
+// texel offset ((i % cols) W, (i / cols) H).
+//   arr / tex    the field itself, fp32 (or fp16 when dtf_format = 1): what epo_get_dtf returns
+//   arr8 / tex8  (fp32 format only) the exact integer SQUARED distance, saturated at 255, one byte per texel.
+//                The fused kernel samples this one whenever lambda <= kU8LambdaMax and takes the correctly rounded
+//                square root from a 256-entry table: the same fp32 tap values from a quarter of the bytes.  A
+//                saturated tap (distance >= sqrt(255) = 15.97) can only occur in a footprint whose four taps all
+//                exceed 15.97 - sqrt(2) = 14.55 (the exact EDT is 1-Lipschitz), where d > lambda clamps the sample to
+//                rho = H(lambda), rho' = 0 whatever the taps are.
+struct EpoAtlas {
+  cudaArray_t arr, arr8;
+  cudaTextureObject_t tex, tex8;
+  int cols;
+};
+constexpr float kU8LambdaMax = 14.5f;
+
 struct epo_ctx {
   epo_config cfg;
   cudaStream_t stream;
@@ -68,9 +84,7 @@ struct epo_ctx {
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
   float4* d_pts;          // [E] camera-frame points (x_s, y_s, z_s, 0): K and Z are fixed, so row a-2 is hoisted
-  cudaArray_t dtf_atlas;                      // block-linear, gather-enabled array of all fields (fp32 or fp16): views tiled in a grid
-  cudaTextureObject_t dtf_tex;                // texture object on the atlas (what the fused kernel samples)
-  int atlas_cols;                             // view i sits at texel offset ((i % cols) W, (i / cols) H)
+  EpoAtlas atlas;         // the distance fields as the fused kernel samples them (see EpoAtlas)
   std::vector<int32_t> h_edge_off;
 
   // pairs
@@ -142,14 +156,13 @@ epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
                                 int32_t** out_off, EdgeRec** out_rec, int64_t* out_E,
                                 std::vector<int32_t>* h_off, bool* out_subsampled);
-struct EpoDtfScratch { int32_t* g; cudaSurfaceObject_t surf; };   // alive until the EDT kernels have run
-epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArray_t* atlas, cudaTextureObject_t* tex,
-                               int* cols, EpoDtfScratch* scratch);
+struct EpoDtfScratch { int32_t* g; cudaSurfaceObject_t surf, surf8; };   // alive until the EDT kernels have run
+epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, EpoAtlas* atlas, EpoDtfScratch* scratch);
 void epo_free_dtf_scratch(EpoDtfScratch* s);
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
                             const std::vector<int32_t>& h_off, const uint8_t* d_edges_u8, const float* d_depth,
                             bool subsampled, float4** out_pts);
-void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex);
+void epo_free_atlas(EpoAtlas* atlas);
 // pairs.cu
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,

@@ -173,13 +173,15 @@ __global__ void k_edt_rows(const uint8_t* __restrict__ edges, int64_t rows, int 
 // stays converged.  An out-of-range row is clamped to the border row: its candidate only over-estimates
 // that row's true candidate, so the minimum is unchanged and the loop is branch-free.
 // DTF = correctly rounded fp32 sqrt of d2 (d2 < 2^24 is exact in fp32; else via fp64 sqrt), written
-// straight into the block-linear atlas the fused kernel samples (surface store; fp16 = RNE of the fp32).
+// straight into the block-linear atlas (surface store; fp16 = RNE of the fp32), and -- fp32 format -- d2 itself,
+// saturated at 255, into the one-byte atlas the fused kernel samples (see EpoAtlas).
 // ---------------------------------------------------------------------------------------------
 constexpr int kEdtStrip = 32, kEdtWarps = 8;
 
 template <typename I, bool kStage>
 __global__ void __launch_bounds__(kEdtStrip * kEdtWarps)
-k_edt_cols(const int32_t* __restrict__ g, int W, int H, cudaSurfaceObject_t atlas, int atlas_cols, int half) {
+k_edt_cols(const int32_t* __restrict__ g, int W, int H, cudaSurfaceObject_t atlas, cudaSurfaceObject_t atlas8,
+           int atlas_cols, int half) {
   extern __shared__ int32_t sg[];             // [H][32] when kStage
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int view = blockIdx.y, x = blockIdx.x * kEdtStrip + lane;
@@ -206,7 +208,10 @@ k_edt_cols(const int32_t* __restrict__ g, int W, int H, cudaSurfaceObject_t atla
     if (in) {
       const float r = (best < (I)(1 << 24)) ? __fsqrt_rn((float)best) : (float)sqrt((double)best);
       if (half) surf2Dwrite(__half_as_ushort(__float2half_rn(r)), atlas, ox * 2, oy + y);
-      else surf2Dwrite(r, atlas, ox * 4, oy + y);
+      else {
+        surf2Dwrite(r, atlas, ox * 4, oy + y);
+        surf2Dwrite((unsigned char)(best < (I)255 ? best : (I)255), atlas8, ox, oy + y);   // exact d^2, saturated
+      }
     }
   }
 }
@@ -357,9 +362,12 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
   return EPO_OK;
 }
 
-void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex) {
-  if (tex) cudaDestroyTextureObject(tex);
-  if (atlas) cudaFreeArray(atlas);
+void epo_free_atlas(EpoAtlas* a) {
+  if (a->tex) cudaDestroyTextureObject(a->tex);
+  if (a->tex8) cudaDestroyTextureObject(a->tex8);
+  if (a->arr) cudaFreeArray(a->arr);
+  if (a->arr8) cudaFreeArray(a->arr8);
+  a->tex = a->tex8 = 0; a->arr = a->arr8 = nullptr;
 }
 
 // Distance fields of all views (rows a-P2, a-P3), written straight into ONE block-linear, gather-enabled 2-D
@@ -371,12 +379,12 @@ void epo_free_atlas(cudaArray_t atlas, cudaTextureObject_t tex) {
 // has drained.
 void epo_free_dtf_scratch(EpoDtfScratch* s) {
   if (s->surf) cudaDestroySurfaceObject(s->surf);
+  if (s->surf8) cudaDestroySurfaceObject(s->surf8);
   cudaFree(s->g);
-  s->surf = 0; s->g = nullptr;
+  s->surf = s->surf8 = 0; s->g = nullptr;
 }
 
-epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArray_t* atlas_out,
-                               cudaTextureObject_t* tex_out, int* cols_out, EpoDtfScratch* scratch_out) {
+epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, EpoAtlas* out, EpoDtfScratch* scratch_out) {
   const int N = ctx->N, W = ctx->W, H = ctx->H;
   const int64_t rows = (int64_t)N * H;
   cudaStream_t st = ctx->stream;
@@ -385,13 +393,18 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArra
   const int arows = (N + cols - 1) / cols;
   if ((int64_t)arows * H > 65536 || (int64_t)cols * W > 131072)
     return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "%d views of %dx%d do not fit one 2-D texture atlas", N, W, H);
+  EpoAtlas a = {nullptr, nullptr, 0, 0, cols};
+  cudaSurfaceObject_t surf = 0, surf8 = 0; int32_t* g = nullptr;
   cudaChannelFormatDesc desc = half ? cudaCreateChannelDescHalf() : cudaCreateChannelDesc<float>();
-  cudaArray_t arr = nullptr; cudaTextureObject_t t = 0; cudaSurfaceObject_t surf = 0; int32_t* g = nullptr;
-  cudaError_t e = cudaMallocArray(&arr, &desc, (size_t)cols * W, (size_t)arows * H,
-                                  cudaArrayTextureGather | cudaArraySurfaceLoadStore);
+  cudaChannelFormatDesc desc8 = cudaCreateChannelDesc<unsigned char>();
+  const unsigned flags = cudaArrayTextureGather | cudaArraySurfaceLoadStore;
+  cudaError_t e = cudaMallocArray(&a.arr, &desc, (size_t)cols * W, (size_t)arows * H, flags);
+  if (e == cudaSuccess && !half) e = cudaMallocArray(&a.arr8, &desc8, (size_t)cols * W, (size_t)arows * H, flags);
   cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
-  rd.resType = cudaResourceTypeArray; rd.res.array.array = arr;
+  rd.resType = cudaResourceTypeArray; rd.res.array.array = a.arr;
+  cudaResourceDesc rd8 = rd; rd8.res.array.array = a.arr8;
   if (e == cudaSuccess) e = cudaCreateSurfaceObject(&surf, &rd);
+  if (e == cudaSuccess && !half) e = cudaCreateSurfaceObject(&surf8, &rd8);
   if (e == cudaSuccess) e = cudaMalloc(&g, (size_t)rows * W * sizeof(int32_t));
   if (e == cudaSuccess) {
     const int grid_rows = (int)((rows + kWarpsPerBlock - 1) / kWarpsPerBlock);
@@ -405,7 +418,7 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArra
 #define EDT_LAUNCH(I, S)                                                                                       \
     do {                                                                                                        \
       if (S) e = cudaFuncSetAttribute(k_edt_cols<I, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-      if (e == cudaSuccess) k_edt_cols<I, S><<<grid, thr, (S) ? smem : 0, st>>>(g, W, H, surf, cols, half ? 1 : 0); \
+      if (e == cudaSuccess) k_edt_cols<I, S><<<grid, thr, (S) ? smem : 0, st>>>(g, W, H, surf, surf8, cols, half ? 1 : 0); \
     } while (0)
     if (wide) { if (stage) EDT_LAUNCH(long long, true); else EDT_LAUNCH(long long, false); }
     else      { if (stage) EDT_LAUNCH(int, true);       else EDT_LAUNCH(int, false); }
@@ -417,17 +430,19 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, cudaArra
     cudaTextureDesc td; memset(&td, 0, sizeof(td));
     td.addressMode[0] = td.addressMode[1] = cudaAddressModeClamp;
     td.filterMode = cudaFilterModePoint; td.readMode = cudaReadModeElementType; td.normalizedCoords = 0;
-    e = cudaCreateTextureObject(&t, &rd, &td, nullptr);
+    e = cudaCreateTextureObject(&a.tex, &rd, &td, nullptr);
+    if (e == cudaSuccess && !half) e = cudaCreateTextureObject(&a.tex8, &rd8, &td, nullptr);
   }
   if (e != cudaSuccess) {
     cudaStreamSynchronize(st);
     if (surf) cudaDestroySurfaceObject(surf);
+    if (surf8) cudaDestroySurfaceObject(surf8);
     cudaFree(g);
-    epo_free_atlas(arr, t);
+    epo_free_atlas(&a);
     return epo_fail(ctx, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "distance fields: %s",
                     cudaGetErrorString(e));
   }
-  *atlas_out = arr; *tex_out = t; *cols_out = cols; scratch_out->g = g; scratch_out->surf = surf;
+  *out = a; scratch_out->g = g; scratch_out->surf = surf; scratch_out->surf8 = surf8;
   return EPO_OK;
 }
 
