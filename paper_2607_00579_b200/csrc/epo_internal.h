@@ -32,7 +32,7 @@ constexpr int kAccStride = 8;
 #define EPO_LG_OUTER 8
 #endif
 #ifndef EPO_LG_MINBLOCKS
-#define EPO_LG_MINBLOCKS 8
+#define EPO_LG_MINBLOCKS 7
 #endif
 constexpr int kLgThreads = EPO_LG_THREADS;
 constexpr int kLgPerThread = EPO_LG_PER_THREAD;
