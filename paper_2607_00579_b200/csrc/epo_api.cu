@@ -73,6 +73,23 @@ void free_pairs(epo_ctx* c) {
   c->have_pairs = false; c->P = 0; c->n_work = 0;
 }
 
+// Samples per work item (= per CTA) of the fused kernel, a multiple of kLgPass.  Every CTA pays a fixed price
+// (scheduling, the pose prologue, the block reduction: measured ~1.4 ns of GPU time each at config 3), so items are
+// made as long as possible -- up to kLgOuter passes -- while the grid still has about two waves of CTAs to
+// balance the SMs.  EPO_LG_PASSES in the environment overrides the choice (tuning).
+int choose_chunk(const epo_ctx* c, const std::vector<int32_t>& pairs, int64_t P) {
+  int64_t samples = 0;
+  for (int64_t k = 0; k < P; ++k) samples += c->h_edge_off[pairs[2 * k] + 1] - c->h_edge_off[pairs[2 * k]];
+  int sms = 148;
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->cfg.device);
+  const int64_t slots = (int64_t)sms * EPO_LG_MINBLOCKS;
+  int64_t passes = samples / (2 * slots * kLgPass);
+  if (passes < 4) passes = 4;
+  if (passes > kLgOuter) passes = kLgOuter;
+  if (const char* v = std::getenv("EPO_LG_PASSES")) { int k = std::atoi(v); if (k >= 1 && k <= kLgMaxOuter) passes = k; }
+  return (int)passes * kLgPass;
+}
+
 epo_status reset_optimiser(epo_ctx* c) {
   cudaStream_t st = c->stream;
   EPO_CUDA(c, cudaMemsetAsync(c->d_m, 0, (size_t)c->N * 6 * sizeof(double), st));
@@ -117,7 +134,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   if (!c) return EPO_ERR_OUT_OF_MEMORY;
   c->cfg = *cfg; c->stream = (cudaStream_t)cfg->stream;
   c->N = cfg->n_views; c->W = cfg->width; c->H = cfg->height;
-  c->have_views = c->have_pairs = false; c->P = c->E = c->n_work = c->reproj_per_eval = c->launches = 0;
+  c->have_views = c->have_pairs = false; c->P = c->E = c->n_work = c->reproj_per_eval = c->launches = 0; c->lg_chunk = kLgOuter * kLgPass;
   c->err[0] = 0;
   c->atlas = EpoAtlas{nullptr, nullptr, 0, 0, 1};
   { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
@@ -262,7 +279,8 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   cudaError_t e = cudaMemcpyAsync(d_user, hp.data(), (size_t)P * 2 * sizeof(int32_t), cudaMemcpyHostToDevice, st);
   int2* canon = nullptr; int4* work = nullptr; int32_t *perm = nullptr, *toff = nullptr, *soff = nullptr, *sinc = nullptr, *woff = nullptr;
   int64_t n_work = 0;
-  epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &woff, &n_work)
+  const int chunk = choose_chunk(c, hp, P);
+  epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &woff, &n_work, chunk)
                                      : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
   cudaFree(d_user);
   double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
@@ -287,7 +305,7 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   free_pairs(c);
   c->d_pairs = canon; c->d_perm = perm; c->d_tgt_off = toff; c->d_src_off = soff; c->d_src_inc = sinc; c->d_work = work;
   c->d_work_off = woff; c->n_work = n_work; c->P = P; c->d_part = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
-  c->h_pairs.swap(hp); c->reproj_per_eval = reproj;
+  c->h_pairs.swap(hp); c->reproj_per_eval = reproj; c->lg_chunk = chunk;
   c->have_pairs = true; c->static_dirty = true;
   EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, (size_t)c->N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
   EPO_TRY(reset_optimiser(c));

@@ -29,15 +29,17 @@ constexpr int kAccStride = 8;
 #define EPO_LG_PER_THREAD 2
 #endif
 #ifndef EPO_LG_OUTER
-#define EPO_LG_OUTER 8
+#define EPO_LG_OUTER 16
 #endif
 #ifndef EPO_LG_MINBLOCKS
 #define EPO_LG_MINBLOCKS 7
 #endif
 constexpr int kLgThreads = EPO_LG_THREADS;
 constexpr int kLgPerThread = EPO_LG_PER_THREAD;
-constexpr int kLgOuter = EPO_LG_OUTER;
-constexpr int kLgChunk = kLgThreads * kLgPerThread * kLgOuter;
+constexpr int kLgOuter = EPO_LG_OUTER;        // most passes per work item (epo_ctx::lg_chunk is what runs)
+constexpr int kLgPass = kLgThreads * kLgPerThread;     // samples of one pass of a CTA
+constexpr int kLgMaxOuter = 32;
+constexpr int kLgPad = kLgPass * kLgMaxOuter;  // zero points appended to the list: tail lanes / prefetches read past a list
 
 // Device-resident control block of the optimisation loop (rows a-10..a-12): lets epo_step enqueue
 // n iterations without any host synchronisation; every kernel of an iteration checks `stopped`.
@@ -75,6 +77,7 @@ struct epo_ctx {
   bool pdl;            // programmatic dependent launch between the kernels of the loop (EPO_NO_PDL=1 turns it off)
   bool static_dirty;   // work list / points / fields were (re)built since the last fused launch: launch it serialised
   int64_t P, E, n_work, reproj_per_eval, launches;
+  int lg_chunk;        // samples per work item of the fused kernel (a multiple of kLgPass), chosen in epo_set_pairs
 
   // views
   float* d_K;             // [N][4]
@@ -166,7 +169,8 @@ void epo_free_atlas(EpoAtlas* atlas);
 // pairs.cu
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
-                           int32_t** out_src_inc, int4** out_work, int32_t** out_work_off, int64_t* out_n_work);
+                           int32_t** out_src_inc, int4** out_work, int32_t** out_work_off, int64_t* out_n_work,
+                           int chunk);
 // lossgrad.cu
 epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)

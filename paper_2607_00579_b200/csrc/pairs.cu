@@ -106,7 +106,7 @@ __global__ void k_fill_work(const int32_t* __restrict__ work_off, const int2* __
 
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2** out_pairs, int32_t** out_perm,
                            int32_t** out_tgt_off, int32_t** out_src_off, int32_t** out_src_inc, int4** out_work,
-                           int32_t** out_work_off, int64_t* out_n_work) {
+                           int32_t** out_work_off, int64_t* out_n_work, int chunk) {
   const int N = ctx->N;
   cudaStream_t st = ctx->stream;
   int2* canon = nullptr;
@@ -153,14 +153,14 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
   k_bucket<<<gridP, 256, 0, st>>>(reinterpret_cast<const int32_t*>(canon), P, 2, src_off, cursor, bucket);
   k_rank_sources<<<gridP, 256, 0, st>>>(canon, src_off, bucket, P, src_inc);
   // work list of the fused kernel: (pair, first edge of the chunk), target-major
-  k_chunk_counts<<<gridP, 256, 0, st>>>(canon, ctx->d_edge_off, P, kLgChunk, chunk_cnt);
+  k_chunk_counts<<<gridP, 256, 0, st>>>(canon, ctx->d_edge_off, P, chunk, chunk_cnt);
   k_scan_small<<<1, 1024, 0, st>>>(chunk_cnt, work_off, P);
   ctx->launches += 10;
   int32_t n_work = 0;
   PR_CUDA(cudaMemcpyAsync(&n_work, work_off + P, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   PR_CUDA(cudaStreamSynchronize(st));
   PR_CUDA(cudaMalloc(&work, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int4)));
-  k_fill_work<<<gridP, 256, 0, st>>>(work_off, canon, ctx->d_edge_off, P, kLgChunk, work);
+  k_fill_work<<<gridP, 256, 0, st>>>(work_off, canon, ctx->d_edge_off, P, chunk, work);
   ctx->launches += 1;
   PR_CUDA(cudaGetLastError());
   PR_CUDA(cudaStreamSynchronize(st));

@@ -452,8 +452,8 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
   float4* pts = nullptr;
   cudaStream_t st = ctx->stream;
   // padded by one chunk of zeros: the fused kernel's tail lanes read past the end of a list and discard
-  EPO_CUDA(ctx, cudaMalloc(&pts, (size_t)(E + kLgChunk) * sizeof(float4)));
-  EPO_CUDA(ctx, cudaMemsetAsync(pts + E, 0, (size_t)kLgChunk * sizeof(float4), st));
+  EPO_CUDA(ctx, cudaMalloc(&pts, (size_t)(E + kLgPad) * sizeof(float4)));
+  EPO_CUDA(ctx, cudaMemsetAsync(pts + E, 0, (size_t)kLgPad * sizeof(float4), st));
   cudaError_t e = cudaSuccess;
   if (subsampled) {
     // an E_max sub-sample is defined on the raster list (reading S6): keep its order

@@ -105,7 +105,7 @@ def test_fp16_field_is_rne_of_fp32_field():
 
 # ---------------------------------------------------------------------------------- loss + gradient
 @pytest.mark.parametrize("name", list(SMALL))
-@pytest.mark.parametrize("lam", [10.0, 6.0])
+@pytest.mark.parametrize("lam", [10.0, 6.0, 14.5, 20.0])
 def test_loss_and_gradient_parity(name, lam):
     """Per-pair loss 1e-5 and per-camera gradient 1e-4 (relative) on the same seeded inputs.
     Two oracles: the all-double one (default) and the one that decides the projected position in fp32 as
@@ -132,6 +132,29 @@ def test_loss_and_gradient_parity(name, lam):
     again = e.loss_grad(lam)
     assert abs(again["loss"] - got["loss"]) <= 1e-6 * abs(got["loss"])
     e.destroy()
+
+
+def test_byte_atlas_and_fp32_atlas_take_the_same_taps():
+    """The fused kernel samples the one-byte squared-distance atlas for lambda <= 14.5 and the fp32 field above
+    (EpoAtlas in epo_internal.h).  With lambda beyond every field value the clamp never acts, so the per-pair
+    valid counts must be identical on both sides of the switch, and just across it (14.5 vs 14.5 + 1 ulp) the two
+    paths must return the same pair losses: every tap that can matter is the same fp32 number."""
+    sc = scene("orbit8")
+    e = make_ctx(sc)
+    lo = e.loss_grad(14.5)
+    hi = e.loss_grad(float(np.nextafter(np.float32(14.5), np.float32(15.0))))
+    assert np.array_equal(lo["pair_valid"], hi["pair_valid"])
+    assert np.allclose(lo["pair_loss"], hi["pair_loss"], rtol=2e-6, atol=0)
+    assert np.allclose(lo["grad"], hi["grad"], rtol=1e-4, atol=1e-7)
+    e.destroy()
+
+
+def test_wide_clamp_schedule_runs_on_the_fp32_atlas():
+    """A clamp schedule above 14.5 px switches the loop to the fp32 atlas: same lock-step parity."""
+    kw = dict(clamp_start=24.0, clamp_end=16.0, early_stop=0)
+    worst, _, n = _lockstep(scene("room6"), 12, kw, kw)
+    assert n == 12
+    assert worst["rot"] <= 1e-3 and worst["tr"] <= 1e-4 and worst["theta"] <= 1e-3 and worst["loss"] <= 1e-5
 
 
 def test_loss_and_gradient_parity_device_pointers():
@@ -294,6 +317,7 @@ def test_early_stop_parity():
     assert phase == 2 and opt.phase.value == 2 and done < 600
     assert abs(done - odone) <= max(2, int(0.05 * odone)), (done, odone)
     assert e.step(5) == (0, 2)
+    assert e.step(0) == (0, 2)
     e.reset()                                                           # back to the initial poses, state cleared
     done2, _ = e.step(done)
     assert done2 == done
