@@ -152,6 +152,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   if (e == cudaSuccess) e = cudaMalloc(&c->d_dR, N * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_dt, N * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_state, sizeof(DevState));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, (size_t)cfg->max_steps * 4 * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_theta, (size_t)cfg->max_steps * sizeof(double));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_loss_trace, (size_t)cfg->max_steps * sizeof(double));
   if (e != cudaSuccess) {
@@ -160,6 +161,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
     epo_destroy(c);
     return st;
   }
+  if (epo_launch_fill_schedule(c) != EPO_OK) { epo_destroy(c); return EPO_ERR_CUDA; }
   *out = c;
   return EPO_OK;
 }
@@ -171,7 +173,7 @@ void epo_destroy(epo_ctx* c) {
   free_pairs(c); free_views(c);
   cudaFree(c->d_K); cudaFree(c->d_poses); cudaFree(c->d_poses_next); cudaFree(c->d_poses_init); cudaFree(c->d_grad); cudaFree(c->d_loss_part);
   cudaFree(c->d_m); cudaFree(c->d_v); cudaFree(c->d_dR); cudaFree(c->d_dt); cudaFree(c->d_state);
-  cudaFree(c->d_theta); cudaFree(c->d_loss_trace);
+  cudaFree(c->d_sched); cudaFree(c->d_theta); cudaFree(c->d_loss_trace);
   cudaGetLastError();
   delete c;
 }

@@ -111,6 +111,7 @@ struct epo_ctx {
   double *d_m, *d_v;      // [N][6]
   double *d_dR, *d_dt;    // [N] per-camera pose change (degrees)
   DevState* d_state;
+  double* d_sched;        // [max_steps][4] {lr_s, 1 - beta1^(s+1), 1 - beta2^(s+1), lambda_s}: row a-12, tabulated at create
   double* d_theta;        // [max_steps]
   double* d_loss_trace;   // [max_steps]
 
@@ -176,6 +177,7 @@ epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device s
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
 epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first);
+epo_status epo_launch_fill_schedule(epo_ctx* ctx);     // d_sched from the configuration (once, in epo_create)
 epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done (an epo_step call of zero iterations)
 void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n);
 void epo_launch_f32_to_f64(cudaStream_t st, const float* in, double* out, int64_t n);

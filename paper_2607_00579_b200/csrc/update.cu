@@ -28,8 +28,9 @@ struct FinParams {
   DevState* state;
   int N;
   int64_t P;
-  double lr_max, beta1, beta2, adam_eps, eps1, eps2;
-  int warmup, max_steps, w1, w2, smooth, early_stop;
+  double beta1, beta2, adam_eps, eps1, eps2;
+  const double* sched;          // [max_steps][4] {lr_s, 1 - beta1^(s+1), 1 - beta2^(s+1), lambda_s}
+  int max_steps, w1, w2, smooth, early_stop;
   int gated, step_mode, call_first;
 };
 
@@ -55,10 +56,15 @@ __device__ double lr_of_step(int s, double lr_max, int warmup, int max_steps) {
 // Exp(v, w) = [Exp_SO3(w), V(w) v]; V = I + (1-cos th)/th^2 [w]x + (th - sin th)/th^3 [w]x^2
 __device__ void se3_exp(const double* e, double* T) {
   const double v0 = e[0], v1 = e[1], v2 = e[2], w0 = e[3], w1 = e[4], w2 = e[5];
-  const double th2 = w0 * w0 + w1 * w1 + w2 * w2, th = sqrt(th2);
+  const double th2 = w0 * w0 + w1 * w1 + w2 * w2;
   double A, B, C;
-  if (th < 1e-4) { A = 1.0 - th2 / 6.0; B = 0.5 - th2 / 24.0; C = 1.0 / 6.0 - th2 / 120.0; }
-  else { A = sin(th) / th; B = (1.0 - cos(th)) / th2; C = (th - sin(th)) / (th2 * th); }
+  if (th2 < 1e-2) {
+    // |w| < 0.1 (an Adam step is a few 1e-3): the three series in th^2, seven terms each (next term < 1e-26),
+    // by Horner -- no sin / cos / sqrt on the serial path of the iteration
+    A = 1.0 + th2 * (-1.0 / 6 + th2 * (1.0 / 120 + th2 * (-1.0 / 5040 + th2 * (1.0 / 362880 + th2 * (-1.0 / 39916800 + th2 * (1.0 / 6227020800.0))))));
+    B = 0.5 + th2 * (-1.0 / 24 + th2 * (1.0 / 720 + th2 * (-1.0 / 40320 + th2 * (1.0 / 3628800 + th2 * (-1.0 / 479001600 + th2 * (1.0 / 87178291200.0))))));
+    C = 1.0 / 6 + th2 * (-1.0 / 120 + th2 * (1.0 / 5040 + th2 * (-1.0 / 362880 + th2 * (1.0 / 39916800 + th2 * (-1.0 / 6227020800.0 + th2 * (1.0 / 1307674368000.0))))));
+  } else { const double th = sqrt(th2); A = sin(th) / th; B = (1.0 - cos(th)) / th2; C = (th - sin(th)) / (th2 * th); }
   const double Wx[9] = {0, -w2, w1, w2, 0, -w0, -w1, w0, 0};
   double W2[9];
 #pragma unroll
@@ -201,14 +207,14 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     if (tid == 0) { st->loss = tot / (double)p.P; st->ticket = 0; }
     return;
   }
-  // ---- a-10 Adam (lanes 2..7 of warp 0), a-12 learning rate
+  // ---- a-10 Adam (lanes 2..7 of warp 0); the step-dependent scalars come from the schedule table (a-12)
   const int s = st->step;
+  __shared__ double sT[24];                          // new pose, old pose
   if (warp == 0) {
     double eps = 0.0;
     if (lane >= 2 && lane < 8) {
       const size_t k = 6 * (size_t)c + lane - 2;
-      const double lr = lr_of_step(s, p.lr_max, p.warmup, p.max_steps);
-      const double c1 = 1.0 - pow(p.beta1, (double)(s + 1)), c2 = 1.0 - pow(p.beta2, (double)(s + 1));
+      const double lr = p.sched[4 * (size_t)s], c1 = p.sched[4 * (size_t)s + 1], c2 = p.sched[4 * (size_t)s + 2];
       const double m = p.beta1 * p.m[k] + (1.0 - p.beta1) * g;
       const double v = p.beta2 * p.v[k] + (1.0 - p.beta2) * g * g;
       p.m[k] = m; p.v[k] = v;
@@ -218,7 +224,7 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
 #pragma unroll
     for (int k = 0; k < 6; ++k) e[k] = __shfl_sync(0xffffffffu, eps, 2 + k);
     if (lane == 0) {
-      // retraction T_c <- Exp(eps) T_c and a-11 pose change of this camera
+      // retraction T_c <- Exp(eps) T_c
       double E[12], T[12], Tn[12];
       se3_exp(e, E);
 #pragma unroll
@@ -229,24 +235,34 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
         for (int j = 0; j < 4; ++j) Tn[4 * i + j] = E[4 * i] * T[j] + E[4 * i + 1] * T[4 + j] + E[4 * i + 2] * T[8 + j];
         Tn[4 * i + 3] += E[4 * i + 3];
       }
-      double tr = 0.0;   // Eq. 9: tr(R^s (R^{s-1})^T)
 #pragma unroll
-      for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int j = 0; j < 3; ++j) tr += Tn[4 * i + j] * T[4 * i + j];
-      p.dR[c] = (180.0 / kPi) * acos(clip1((tr - 1.0) / 2.0));
-      const double na = sqrt(Tn[3] * Tn[3] + Tn[7] * Tn[7] + Tn[11] * Tn[11]);
-      const double nb = sqrt(T[3] * T[3] + T[7] * T[7] + T[11] * T[11]);
-      double dtc = 0.0;  // Eq. 10; 0 if either norm < 1e-12 (reading S13)
-      if (na >= 1e-12 && nb >= 1e-12)
-        dtc = (180.0 / kPi) * acos(clip1((Tn[3] / na) * (T[3] / nb) + (Tn[7] / na) * (T[7] / nb) + (Tn[11] / na) * (T[11] / nb)));
-      p.dt[c] = dtc;
-#pragma unroll
-      for (int k = 0; k < 12; ++k) p.poses_next[12 * (size_t)c + k] = Tn[k];
-      __threadfence();                               // this camera's outputs before its ticket
-      s_last = atomicAdd(&st->ticket, 1) == N - 1;
+      for (int k = 0; k < 12; ++k) { sT[k] = Tn[k]; sT[12 + k] = T[k]; }
     }
   }
+  __syncthreads();
+  // ---- a-11 pose change of this camera: three warps side by side
+  if (tid == 0) {
+    double tr = 0.0;   // Eq. 9: tr(R^s (R^{s-1})^T)
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+      for (int j = 0; j < 3; ++j) tr += sT[4 * i + j] * sT[12 + 4 * i + j];
+    p.dR[c] = (180.0 / kPi) * acos(clip1((tr - 1.0) / 2.0));
+    __threadfence();
+  } else if (tid == 32) {
+    const double a0 = sT[3], a1 = sT[7], a2 = sT[11], b0 = sT[15], b1 = sT[19], b2 = sT[23];
+    const double na = sqrt(a0 * a0 + a1 * a1 + a2 * a2), nb = sqrt(b0 * b0 + b1 * b1 + b2 * b2);
+    double dtc = 0.0;  // Eq. 10; 0 if either norm < 1e-12 (reading S13)
+    if (na >= 1e-12 && nb >= 1e-12)
+      dtc = (180.0 / kPi) * acos(clip1((a0 / na) * (b0 / nb) + (a1 / na) * (b1 / nb) + (a2 / na) * (b2 / nb)));
+    p.dt[c] = dtc;
+    __threadfence();
+  } else if (tid >= 64 && tid < 76) {
+    p.poses_next[12 * (size_t)c + tid - 64] = sT[tid - 64];
+    __threadfence();
+  }
+  __syncthreads();
+  if (tid == 0) s_last = atomicAdd(&st->ticket, 1) == N - 1;   // this camera's outputs precede its ticket
   __syncthreads();
   if (!s_last) return;
   // ---- last CTA: every camera has been reduced and stepped; nobody reads the current poses any more
@@ -284,6 +300,20 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   }
 }
 
+// a-12 schedules, tabulated once per context (the configuration is immutable): row s = {lr_s, 1 - beta1^(s+1),
+// 1 - beta2^(s+1), lambda_s}.  lambda_s = clamp_start + (clamp_end - clamp_start) min(s, clamp_steps) / clamp_steps
+// (PAPER.md:462), rounded to fp32 as the fused kernel uses it.
+__global__ void k_fill_schedule(double* __restrict__ sched, int max_steps, double lr_max, int warmup, double beta1,
+                                double beta2, double clamp_start, double clamp_end, int clamp_steps) {
+  const int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= max_steps) return;
+  const int m = s < clamp_steps ? s : clamp_steps;
+  sched[4 * s] = lr_of_step(s, lr_max, warmup, max_steps);
+  sched[4 * s + 1] = 1.0 - pow(beta1, (double)(s + 1));
+  sched[4 * s + 2] = 1.0 - pow(beta2, (double)(s + 1));
+  sched[4 * s + 3] = (double)(float)(clamp_start + (clamp_end - clamp_start) * (double)m / (double)clamp_steps);
+}
+
 __global__ void k_begin_step_call(DevState* st, int max_steps, int early_stop) {
   st->iters_done = 0;
   st->stopped = (st->step >= max_steps) || (early_stop && st->phase == 2);
@@ -308,8 +338,8 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.m = ctx->d_m; p.v = ctx->d_v;
   p.dR = ctx->d_dR; p.dt = ctx->d_dt; p.theta = ctx->d_theta; p.loss_trace = ctx->d_loss_trace;
   p.state = ctx->d_state; p.N = ctx->N; p.P = ctx->P;
-  p.lr_max = ctx->cfg.lr_max; p.beta1 = ctx->cfg.beta1; p.beta2 = ctx->cfg.beta2; p.adam_eps = ctx->cfg.adam_eps;
-  p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.warmup = ctx->cfg.warmup_steps; p.max_steps = ctx->cfg.max_steps;
+  p.sched = ctx->d_sched; p.beta1 = ctx->cfg.beta1; p.beta2 = ctx->cfg.beta2; p.adam_eps = ctx->cfg.adam_eps;
+  p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.max_steps = ctx->cfg.max_steps;
   p.w1 = ctx->cfg.w1; p.w2 = ctx->cfg.w2; p.smooth = ctx->cfg.smooth_window; p.early_stop = ctx->cfg.early_stop;
   p.gated = gated ? 1 : 0; p.step_mode = step_mode ? 1 : 0; p.call_first = call_first ? 1 : 0;
   const size_t smem = (size_t)2 * ctx->N * sizeof(double);   // the last CTA's copy of dR, dt
@@ -324,6 +354,15 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = ctx->pdl ? 1 : 0;
   EPO_CUDA(ctx, cudaLaunchKernelEx(&lc, k_finish, p));
+  ctx->launches += 1;
+  EPO_CUDA(ctx, cudaGetLastError());
+  return EPO_OK;
+}
+
+epo_status epo_launch_fill_schedule(epo_ctx* ctx) {
+  const epo_config& g = ctx->cfg;
+  k_fill_schedule<<<(g.max_steps + 127) / 128, 128, 0, ctx->stream>>>(ctx->d_sched, g.max_steps, g.lr_max, g.warmup_steps, g.beta1,
+                                                                      g.beta2, g.clamp_start, g.clamp_end, g.clamp_steps);
   ctx->launches += 1;
   EPO_CUDA(ctx, cudaGetLastError());
   return EPO_OK;
