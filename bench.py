@@ -63,19 +63,20 @@ def peaks():
 
 
 def ncu_traffic(config: int):
-    """dram read + write bytes per launch of the fused kernel from the committed ncu summary
-    (profiles/traffic.csv: config,kernel,dram_read_bytes,dram_write_bytes,source); None if not captured."""
+    """(dram read + write bytes, warp instructions) per launch of the fused kernel from the committed ncu summary
+    (profiles/traffic.csv: config,kernel,dram_read_bytes,dram_write_bytes,warp_instructions,source);
+    (None, None) if that config was not captured."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(p):
-        return None
-    best = None
+        return None, None
+    best = (None, None)
     for ln in open(p):
         c = [x.strip() for x in ln.split(",")]
         if ln.startswith("#") or len(c) < 4:
             continue
         try:
             if int(c[0]) == config and c[1] == "k_loss_grad":
-                best = float(c[2]) + float(c[3])
+                best = (float(c[2]) + float(c[3]), float(c[4]))
         except ValueError:
             continue
     return best
@@ -336,7 +337,7 @@ def main():
                     edge_pixels=int(edge_off[-1]), parallelism="replicas only" if world > 1 else "1 GPU"),
         clocks=clocks, gpu_launches=int(k1 - k0),
         roofline=dict(bound="hbm", achieved=ach, peak=peak, unit="GB/s", frac=ach / peak, traffic=None,
-                      kernel="k_loss_grad<float>", kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
+                      kernel="k_loss_grad<u8>", kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
                       algorithmic_bytes=alg_bytes, peak_source=peak_src,
                       note="algorithmic bytes = 8 B x attempted + 16 B x valid reprojections (DESIGN.md)"),
         warm_l2=dict(ms_per_step=warm_ms, value=world * reproj / (warm_ms / 1e3)),
@@ -347,7 +348,16 @@ def main():
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = cpu_baseline(sc)
-    line["roofline"]["traffic"] = ncu_traffic(args.config)
+    traffic, warp_inst = ncu_traffic(args.config)
+    line["roofline"]["traffic"] = traffic
+    if warp_inst:
+        # the ceiling that binds in steady state: one warp instruction per scheduler per clock
+        import torch as _t
+        sms = _t.cuda.get_device_properties(local).multi_processor_count
+        mhz = clocks.get("sm_mhz") or 1965.0
+        t_issue = warp_inst / (sms * 4 * mhz * 1e6)
+        line["roofline"].update(issue_frac=t_issue / (k_ms_cold / 1e3), warp_instructions=warp_inst,
+                                issue_note="warp instructions per launch (ncu) / (SMs x 4 schedulers x SM clock) / kernel time")
     print(json.dumps(line))
 
 
