@@ -109,6 +109,10 @@ def lib():
                               C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
                               C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                               C.POINTER(C.c_double)]
+        L.orc_subset_key.restype = C.c_uint64
+        L.orc_subset_key.argtypes = [C.c_uint64, C.c_int, C.c_int64]
+        L.orc_pair_subset.restype = C.c_int64
+        L.orc_pair_subset.argtypes = [C.c_uint64, C.c_int, C.c_int64, C.c_int64, C.c_void_p]
         L.orc_canonical_pairs.argtypes = [C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         _lib = L
     return _lib
@@ -267,6 +271,21 @@ def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair
 
 
 # ---------------------------------------------------------------------------------------------- O7
+def subset_key(seed: int, step: int, p: int) -> int:
+    """key(step, p) of the stochastic pair sub-sampling: a SplitMix64 output, see epo_oracle.c."""
+    return int(lib().orc_subset_key(C.c_uint64(seed & 0xFFFFFFFFFFFFFFFF), int(step), C.c_int64(p)))
+
+
+def pair_subset(seed: int, step: int, n_pairs: int, budget: int) -> np.ndarray:
+    """Boolean mask (caller's pair order) of the fresh uniform random subset S of step `step`, |S| = min(P, M)
+    (PAPER.md:465-474, 500)."""
+    flags = np.zeros(n_pairs, np.uint8)
+    n = lib().orc_pair_subset(C.c_uint64(seed & 0xFFFFFFFFFFFFFFFF), int(step), C.c_int64(n_pairs), C.c_int64(budget),
+                              flags.ctypes.data_as(C.c_void_p))
+    assert n == (n_pairs if budget <= 0 or n_pairs <= budget else budget)
+    return flags.astype(bool)
+
+
 def lam_schedule(s, cfg: Config = Config()):
     return lib().orc_lambda(s, cfg.clamp_start, cfg.clamp_end, cfg.clamp_steps)
 

@@ -410,6 +410,44 @@ void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, con
  * O7  Schedules, Adam, SE(3) exponential  (readings S4, S10, S11)
  * ================================================================================================= */
 /* clamp lambda: clamp_start -> clamp_end linearly over the first clamp_steps steps */
+/* ---------------------------------------------------------------------------------------------------------
+ * Stochastic viewgraph sub-sampling (Alg. 3 l.3-6; PAPER.md:500 A1.3): "at each iteration we
+ * evaluate the loss on a fresh uniform random subset S of E of size min(|E|, M)".
+ * The draw is a pure function of (seed, step, pair): pair p (0-based position in the caller's list) gets the key
+ *   key(step, p) = output number (step * 2^32 + p + 1) of the SplitMix64 generator seeded with `seed`
+ *                = mix(seed + 0x9E3779B97F4A7C15 * (step * 2^32 + p + 1)),
+ * and S = the M pairs with the smallest (key, p) -- a uniformly random M-subset (the keys induce a uniformly
+ * random order), without replacement, fresh for every step.  Written out as the definition: all keys, a full
+ * sort, the first M.  flags[p] = 1 iff pair p is in S; returns |S|.
+ * ------------------------------------------------------------------------------------------------------- */
+static uint64_t orc_splitmix_output(uint64_t seed, uint64_t n) {
+  uint64_t z = seed + 0x9E3779B97F4A7C15ULL * n;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+  return z ^ (z >> 31);
+}
+
+uint64_t orc_subset_key(uint64_t seed, int step, int64_t p) {
+  return orc_splitmix_output(seed, ((uint64_t)(uint32_t)step << 32) + (uint64_t)p + 1ULL);
+}
+
+typedef struct { uint64_t key; int64_t p; } orc_keyed;
+static int orc_keyed_cmp(const void* a, const void* b) {
+  const orc_keyed *x = (const orc_keyed*)a, *y = (const orc_keyed*)b;
+  if (x->key != y->key) return x->key < y->key ? -1 : 1;
+  return x->p < y->p ? -1 : (x->p > y->p ? 1 : 0);
+}
+
+int64_t orc_pair_subset(uint64_t seed, int step, int64_t P, int64_t M, uint8_t* flags) {
+  if (M <= 0 || P <= M) { for (int64_t p = 0; p < P; ++p) flags[p] = 1; return P; }   /* S = E (Alg. 3 l.5) */
+  orc_keyed* k = (orc_keyed*)malloc((size_t)P * sizeof(orc_keyed));
+  for (int64_t p = 0; p < P; ++p) { k[p].key = orc_subset_key(seed, step, p); k[p].p = p; flags[p] = 0; }
+  qsort(k, (size_t)P, sizeof(orc_keyed), orc_keyed_cmp);
+  for (int64_t j = 0; j < M; ++j) flags[k[j].p] = 1;
+  free(k);
+  return M;
+}
+
 double orc_lambda(int s, double clamp_start, double clamp_end, int clamp_steps) {
   int m = s < clamp_steps ? s : clamp_steps;
   return clamp_start + (clamp_end - clamp_start) * (double)m / (double)clamp_steps;
