@@ -72,6 +72,14 @@ typedef struct {
   float   z_min;                    /* 1e-6: depths and projected z at or below it are invalid             */
   int32_t device;                   /* CUDA device ordinal                                                  */
   void*   stream;                   /* cudaStream_t (NULL = legacy default stream)                          */
+  int32_t pair_budget;              /* M of the stochastic viewgraph sub-sampling: when
+                                       the pair list has more than M pairs, every iteration of epo_step evaluates
+                                       a fresh uniform random subset of M pairs.  0 (default) = off: all pairs
+                                       every step, as BASELINE.json's configs fix the list.  Paper default 1024. */
+  uint64_t subsample_seed;          /* seed of that draw: pair p (position in the list given to epo_set_pairs)
+                                       gets, at optimiser step s, the key = output number s * 2^32 + p + 1 of
+                                       SplitMix64(subsample_seed); the subset is the M pairs with the smallest
+                                       (key, p).  A pure function of (seed, s, p): reproducible, no host draw.  */
 } epo_config;
 
 /* Fill *cfg with the paper's hyper-parameters (n_views/width/height = 0, device 0, stream NULL). */
@@ -135,6 +143,10 @@ EPO_API epo_status epo_get_poses_f64(epo_ctx* ctx, double* poses);
 EPO_API epo_status epo_reset(epo_ctx* ctx, const float* poses);
 
 /* ---- introspection (used by the parity tests and the benchmark) ------------------------------- */
+/* The subset of the pair list that iteration `step` of epo_step evaluates (stochastic viewgraph sub-sampling,
+ * PAPER.md:465-474, 500; see epo_config.pair_budget): flags [P] in the caller's pair order, 1 = evaluated.  All 1
+ * when sub-sampling is off or the list is not longer than the budget.  Computed by the loop's own device kernel. */
+EPO_API epo_status epo_get_pair_subset(epo_ctx* ctx, int32_t step, uint8_t* flags /* [P] */);
 EPO_API epo_status epo_get_edge_counts(epo_ctx* ctx, int32_t* offsets /* [N+1] exclusive prefix sums */);
 EPO_API epo_status epo_get_edge_list(epo_ctx* ctx, int32_t view, uint16_t* uv /* [E][2] (u,v) */, float* z /* [E] */);
 EPO_API epo_status epo_get_dtf(epo_ctx* ctx, int32_t view, float* dtf /* [H][W]; fp16 fields are widened */);

@@ -23,7 +23,7 @@ _STATUS = {0: "EPO_OK", 1: "EPO_ERR_INVALID_ARG", 2: "EPO_ERR_BAD_STATE", 3: "EP
 # every symbol include/epo.h declares (tests check that the library exports exactly these)
 SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_set_views", "epo_set_pairs", "epo_loss_grad",
            "epo_step", "epo_get_poses", "epo_get_poses_f64", "epo_reset", "epo_get_edge_counts", "epo_get_edge_list",
-           "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_time_loss_grad_kernel",
+           "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel",
            "epo_last_error", "epo_version"]
 
 
@@ -34,7 +34,8 @@ class EpoConfig(C.Structure):
                 ("beta1", C.c_float), ("beta2", C.c_float), ("adam_eps", C.c_float), ("eps1", C.c_float),
                 ("eps2", C.c_float), ("w1", C.c_int32), ("w2", C.c_int32), ("smooth_window", C.c_int32),
                 ("early_stop", C.c_int32), ("dtf_format", C.c_int32), ("e_max", C.c_int32), ("z_min", C.c_float),
-                ("device", C.c_int32), ("stream", C.c_void_p)]
+                ("device", C.c_int32), ("stream", C.c_void_p), ("pair_budget", C.c_int32),
+                ("subsample_seed", C.c_uint64)]
 
 
 class EpoError(RuntimeError):
@@ -64,6 +65,7 @@ def load_library() -> C.CDLL:
     L.epo_get_dtf.argtypes = [vp, C.c_int32, f32p]
     L.epo_get_pair_order.argtypes = [vp, i32p, i32p]
     L.epo_get_trace.argtypes = [vp, C.c_int32, C.c_int32, f32p, f32p]
+    L.epo_get_pair_subset.argtypes = [vp, C.c_int32, vp]
     L.epo_get_work.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.epo_time_loss_grad_kernel.argtypes = [vp, C.c_float, C.c_int32, C.c_int32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.epo_last_error.argtypes = [vp]; L.epo_last_error.restype = C.c_char_p
@@ -213,6 +215,12 @@ class Epo:
         self._check(lib().epo_time_loss_grad_kernel(self._h, C.c_float(lam), reps, int(flush_l2), C.byref(a), C.byref(b)),
                     "epo_time_loss_grad_kernel")
         return float(a.value), float(b.value)
+
+    def get_pair_subset(self, step: int):
+        """Boolean mask (caller's pair order) of the pairs iteration `step` evaluates."""
+        flags = np.zeros(self.P, np.uint8)
+        self._check(lib().epo_get_pair_subset(self._h, int(step), _ptr(flags)), "epo_get_pair_subset")
+        return flags.astype(bool)
 
     def get_work(self):
         r = C.c_int64(); k = C.c_int64()

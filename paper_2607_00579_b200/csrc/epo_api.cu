@@ -66,7 +66,8 @@ void free_views(epo_ctx* c) {
 void free_pairs(epo_ctx* c) {
   cudaFree(c->d_pairs); cudaFree(c->d_perm); cudaFree(c->d_tgt_off); cudaFree(c->d_src_off); cudaFree(c->d_src_inc);
   cudaFree(c->d_work); cudaFree(c->d_work_off); cudaFree(c->d_part); cudaFree(c->d_pair_loss); cudaFree(c->d_pair_valid); cudaFree(c->d_out_f);
-  cudaFree(c->d_out_i);
+  cudaFree(c->d_out_i); cudaFree(c->d_sel_flag); cudaFree(c->d_sel_work); cudaFree(c->d_sel_info);
+  c->d_sel_flag = nullptr; c->d_sel_work = nullptr; c->d_sel_info = nullptr; c->subsample = false; c->sel_grid = 0;
   c->d_pairs = nullptr; c->d_perm = nullptr; c->d_tgt_off = nullptr; c->d_src_off = nullptr; c->d_src_inc = nullptr;
   c->d_work = nullptr; c->d_work_off = nullptr; c->d_part = nullptr; c->d_pair_loss = nullptr; c->d_pair_valid = nullptr; c->d_out_f = nullptr;
   c->d_out_i = nullptr;
@@ -118,6 +119,7 @@ epo_status epo_config_default(epo_config* cfg) {
   cfg->eps1 = 0.5f; cfg->eps2 = 0.1f; cfg->w1 = 25; cfg->w2 = 50;
   cfg->smooth_window = 1; cfg->early_stop = 1; cfg->dtf_format = 0; cfg->e_max = 0;
   cfg->z_min = 1e-6f; cfg->device = 0; cfg->stream = nullptr;
+  cfg->pair_budget = 0; cfg->subsample_seed = 0;
   return EPO_OK;
 }
 
@@ -128,7 +130,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
     return EPO_ERR_INVALID_ARG;
   if (!(cfg->huber_delta > 0.f) || cfg->clamp_steps < 1 || cfg->warmup_steps < 0 || cfg->max_steps <= cfg->warmup_steps ||
       cfg->w1 < 1 || cfg->w2 < 1 || (cfg->dtf_format != 0 && cfg->dtf_format != 1) || cfg->e_max < 0 ||
-      !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
+      cfg->pair_budget < 0 || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
     return EPO_ERR_INVALID_ARG;
   epo_ctx* c = new (std::nothrow) epo_ctx();
   if (!c) return EPO_ERR_OUT_OF_MEMORY;
@@ -286,6 +288,16 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
                                      : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
   cudaFree(d_user);
   double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
+  uint8_t* sflag = nullptr; int32_t* swork = nullptr; int32_t* sinfo = nullptr;
+  if (rc == EPO_OK) {
+    e = cudaMalloc(&sflag, (size_t)P);
+    if (e == cudaSuccess) e = cudaMalloc(&swork, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMalloc(&sinfo, 2 * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(sinfo, 0, 2 * sizeof(int32_t), st);
+    if (e != cudaSuccess)
+      rc = epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_set_pairs: %s",
+                    cudaGetErrorString(e));
+  }
   if (rc == EPO_OK) {
     // output staging: [loss | grad 6N | pair_loss P | loss trace | theta trace]
     size_t nf = 1 + (size_t)c->N * 6 + (size_t)P + (size_t)c->cfg.max_steps * 2;
@@ -302,12 +314,27 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
     cudaGetLastError();
     cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(toff); cudaFree(soff); cudaFree(sinc); cudaFree(woff);
     cudaFree(acc); cudaFree(pl); cudaFree(pv); cudaFree(of); cudaFree(oi);
+    cudaFree(sflag); cudaFree(swork); cudaFree(sinfo);
     return rc;
   }
   free_pairs(c);
   c->d_pairs = canon; c->d_perm = perm; c->d_tgt_off = toff; c->d_src_off = soff; c->d_src_inc = sinc; c->d_work = work;
   c->d_work_off = woff; c->n_work = n_work; c->P = P; c->d_part = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
   c->h_pairs.swap(hp); c->reproj_per_eval = reproj; c->lg_chunk = chunk;
+  c->d_sel_flag = sflag; c->d_sel_work = swork; c->d_sel_info = sinfo;
+  // stochastic pair sub-sampling: only when the list is longer than the budget (Alg. 3 l.3-6)
+  c->subsample = c->cfg.pair_budget > 0 && P > c->cfg.pair_budget;
+  {
+    int64_t max_items = 1;   // work items of the longest pair
+    for (int64_t k = 0; k < P; ++k) {
+      const int64_t n = c->h_edge_off[c->h_pairs[2 * k] + 1] - c->h_edge_off[c->h_pairs[2 * k]];
+      const int64_t it = (n + chunk - 1) / chunk;
+      if (it > max_items) max_items = it;
+    }
+    c->sel_grid = (int64_t)c->cfg.pair_budget * max_items;
+    if (c->sel_grid > n_work) c->sel_grid = n_work;
+    if (c->sel_grid < 1) c->sel_grid = 1;
+  }
   c->have_pairs = true; c->static_dirty = true;
   EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, (size_t)c->N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
   EPO_TRY(reset_optimiser(c));
@@ -320,8 +347,8 @@ epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss
   if (!loss || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_loss_grad: NULL loss or negative lambda");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
-  EPO_TRY(epo_launch_fused(c, lambda, false));
-  EPO_TRY(epo_launch_finish(c, false, false, false));
+  EPO_TRY(epo_launch_fused(c, lambda, false, false));
+  EPO_TRY(epo_launch_finish(c, false, false, false, false));
   bool sync = false;
   // loss: DevState.loss (double) -> float
   epo_launch_f64_to_f32(st, &c->d_state->loss, c->d_out_f, 1);
@@ -355,8 +382,9 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
   cudaStream_t st = c->stream;
   if (n_iters == 0) EPO_TRY(epo_launch_begin_step_call(c));
   for (int i = 0; i < n_iters; ++i) {
-    EPO_TRY(epo_launch_fused(c, -1.0f, true));
-    EPO_TRY(epo_launch_finish(c, true, true, i == 0));
+    if (c->subsample) EPO_TRY(epo_launch_select_pairs(c, -1, true, true));
+    EPO_TRY(epo_launch_fused(c, -1.0f, true, c->subsample));
+    EPO_TRY(epo_launch_finish(c, true, true, i == 0, c->subsample));
   }
   bool sync = false;
   if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));
@@ -509,6 +537,27 @@ epo_status epo_get_trace(epo_ctx* c, int32_t first, int32_t count, float* loss, 
     EPO_CUDA(c, copy_out(theta95, stage, (size_t)count * sizeof(float), st, &sync));
   }
   if (sync) EPO_CUDA(c, cudaStreamSynchronize(st));
+  return EPO_OK;
+}
+
+epo_status epo_get_pair_subset(epo_ctx* c, int32_t step, uint8_t* flags) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_pair_subset before epo_set_pairs");
+  if (!flags || step < 0) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_pair_subset: bad argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  std::vector<uint8_t> h((size_t)c->P, 1), out((size_t)c->P, 1);
+  if (c->subsample) {
+    // the kernel of the loop, at the given step, flags only; then canonical -> caller's order (marshalling)
+    EPO_TRY(epo_launch_select_pairs(c, step, false, false));
+    std::vector<int32_t> perm((size_t)c->P);
+    EPO_CUDA(c, cudaMemcpyAsync(h.data(), c->d_sel_flag, (size_t)c->P, cudaMemcpyDeviceToHost, st));
+    EPO_CUDA(c, cudaMemcpyAsync(perm.data(), c->d_perm, (size_t)c->P * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    EPO_CUDA(c, cudaStreamSynchronize(st));
+    for (int64_t q = 0; q < c->P; ++q) out[(size_t)perm[(size_t)q]] = h[(size_t)q];
+  }
+  EPO_CUDA(c, cudaMemcpyAsync(flags, out.data(), (size_t)c->P, cudaMemcpyDefault, st));
+  EPO_CUDA(c, cudaStreamSynchronize(st));
   return EPO_OK;
 }
 

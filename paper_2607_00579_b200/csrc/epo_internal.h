@@ -99,6 +99,12 @@ struct epo_ctx {
   int4* d_work;           // [n_work] {source, target, first point of the chunk (absolute), samples left}, target-major
   int32_t* d_work_off;    // [P+1] first work item of each canonical pair
   std::vector<int32_t> h_pairs;   // user order, for reprojection counting
+  // stochastic pair sub-sampling (cfg.pair_budget > 0 and P > budget): rebuilt by k_select_pairs every iteration
+  bool subsample;         // epo_step draws a subset each iteration
+  uint8_t* d_sel_flag;    // [P] canonical order: in this iteration's subset
+  int32_t* d_sel_work;    // [n_work] static work-item indices of the subset's pairs, in order
+  int32_t* d_sel_info;    // {work items, pairs} of the subset
+  int64_t sel_grid;       // upper bound on the subset's work items (the fused kernel's grid in that mode)
 
   // per-evaluation buffers
   double* d_part;         // [n_work][8] per-CTA partial sums {S, n, A[3], M[3]} (no atomics: reproducible)
@@ -172,11 +178,12 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
                            int32_t** out_src_inc, int4** out_work, int32_t** out_work_off, int64_t* out_n_work,
                            int chunk);
+epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override /* < 0: device step */, bool gated, bool build_work);
 // lossgrad.cu
-epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated);
+epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
-epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first);
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset);
 epo_status epo_launch_fill_schedule(epo_ctx* ctx);     // d_sched from the configuration (once, in epo_create)
 epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done (an epo_step call of zero iterations)
 void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n);

@@ -102,6 +102,144 @@ __global__ void k_fill_work(const int32_t* __restrict__ work_off, const int2* __
   for (int w = lo; w < hi; ++w) work[w] = make_int4(st.x, st.y, e0 + (w - lo) * chunk, n - (w - lo) * chunk);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Stochastic viewgraph sub-sampling (Alg. 3 l.3-6): every iteration evaluates a
+// fresh uniform random subset S of the pair list, |S| = M.  The draw is a pure function of (seed, step, pair):
+// pair p (position in the caller's list) gets key(step, p) = output number step * 2^32 + p + 1 of
+// SplitMix64(seed), and S = the M pairs with the smallest (key, p) (include/epo.h).  One CTA per iteration, no
+// host involvement: (1) radix refinement, 11 key bits per sweep, of the bin that holds the M-th smallest key until
+// it has at most kSelCap members (one sweep in practice: P / 2048 expected members), (2) the members are
+// collected in shared memory and the one of rank M is found by counting, (3) one more sweep in canonical
+// (target-major) order writes the membership flags and, by a block-wide scan, the iteration's work list: the
+// indices of the static work items of the selected pairs, in order.
+// ---------------------------------------------------------------------------------------------------------
+constexpr int kSelThreads = 1024, kSelBits = 11, kSelBins = 1 << kSelBits, kSelCap = 2048;
+
+__device__ __forceinline__ unsigned long long subset_key(unsigned long long seed, int step, int p) {
+  unsigned long long z = seed + 0x9E3779B97F4A7C15ull * (((unsigned long long)(unsigned)step << 32) + (unsigned long long)p + 1ull);
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// inclusive scan of an int2 over the CTA (kSelThreads threads); *total gets the CTA sum
+__device__ int2 block_scan2(int2 v, int2* warp_tot /* [32] shared */, int2* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int a = __shfl_up_sync(0xffffffffu, v.x, o), b = __shfl_up_sync(0xffffffffu, v.y, o);
+    if (lane >= o) { v.x += a; v.y += b; }
+  }
+  __syncthreads();                                  // warp_tot may still be read from the previous call
+  if (lane == 31) warp_tot[warp] = v;
+  __syncthreads();
+  if (warp == 0) {
+    int2 w = warp_tot[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int a = __shfl_up_sync(0xffffffffu, w.x, o), b = __shfl_up_sync(0xffffffffu, w.y, o);
+      if (lane >= o) { w.x += a; w.y += b; }
+    }
+    warp_tot[lane] = w;
+  }
+  __syncthreads();
+  if (warp > 0) { v.x += warp_tot[warp - 1].x; v.y += warp_tot[warp - 1].y; }
+  *total = warp_tot[31];
+  return v;
+}
+
+struct SelParams {
+  const int32_t* perm;       // canonical -> caller's pair index
+  const int32_t* work_off;   // [P+1] static work items of each canonical pair
+  const DevState* state;
+  uint8_t* flag;             // [P] canonical order: 1 = in this iteration's subset
+  int32_t* sel_work;         // [n_work] static work-item indices of the subset, in order
+  int32_t* info;             // {work items of the subset, pairs of the subset}
+  unsigned long long seed;
+  int P, M, step_override /* < 0: the device step counter */, gated;
+};
+
+__global__ void __launch_bounds__(kSelThreads) k_select_pairs(const SelParams p) {
+  __shared__ int hist[kSelBins];
+  __shared__ unsigned long long ckey[kSelCap];
+  __shared__ int cidx[kSelCap];
+  __shared__ int2 wtot[32];
+  __shared__ int s_bin, s_below, s_cnt, s_n;
+  __shared__ unsigned long long s_tkey;
+  __shared__ int s_tidx;
+  const int tid = threadIdx.x;
+  cudaTriggerProgrammaticLaunchCompletion();
+  cudaGridDependencySynchronize();
+  if (p.gated && p.state->stopped) return;
+  const int step = p.step_override >= 0 ? p.step_override : p.state->step;
+  // (1) the bin of the M-th smallest key: `prefix` = its leading `nbits` bits, k = rank wanted inside it (1-based)
+  unsigned long long prefix = 0;
+  int nbits = 0, k = p.M, members = p.P;
+  while (members > kSelCap && nbits < 64) {
+    const int db = 64 - nbits < kSelBits ? 64 - nbits : kSelBits;
+    for (int i = tid; i < kSelBins; i += kSelThreads) hist[i] = 0;
+    __syncthreads();
+    for (int q = tid; q < p.P; q += kSelThreads) {
+      const unsigned long long key = subset_key(p.seed, step, p.perm[q]);
+      if (nbits == 0 || (key >> (64 - nbits)) == prefix) atomicAdd(&hist[(int)((key >> (64 - nbits - db)) & ((1u << db) - 1))], 1);
+    }
+    __syncthreads();
+    // two bins per thread, exclusive scan, the bin where the running count crosses k
+    const int h0 = hist[2 * tid], h1 = hist[2 * tid + 1];
+    int2 tot;
+    const int2 inc = block_scan2(make_int2(h0 + h1, 0), wtot, &tot);
+    const int before = inc.x - h0 - h1;
+    if (before < k && k <= before + h0) { s_bin = 2 * tid; s_below = before; s_cnt = h0; }
+    else if (before + h0 < k && k <= before + h0 + h1) { s_bin = 2 * tid + 1; s_below = before + h0; s_cnt = h1; }
+    __syncthreads();
+    prefix = (prefix << db) | (unsigned long long)s_bin;
+    nbits += db; k -= s_below; members = s_cnt;
+    __syncthreads();
+  }
+  // (2) collect the members of that bin and find the one of rank k by (key, caller's index)
+  if (tid == 0) s_n = 0;
+  __syncthreads();
+  for (int q = tid; q < p.P; q += kSelThreads) {
+    const int u = p.perm[q];
+    const unsigned long long key = subset_key(p.seed, step, u);
+    if (nbits == 0 || (key >> (64 - nbits)) == prefix) {
+      const int pos = atomicAdd(&s_n, 1);
+      if (pos < kSelCap) { ckey[pos] = key; cidx[pos] = u; }
+    }
+  }
+  __syncthreads();
+  const int n = s_n < kSelCap ? s_n : kSelCap;   // s_n > kSelCap only if > 2048 pairs share one 64-bit key
+  for (int i = tid; i < n; i += kSelThreads) {
+    const unsigned long long ki = ckey[i]; const int ui = cidx[i];
+    int r = 0;
+    for (int j = 0; j < n; ++j) r += (ckey[j] < ki) || (ckey[j] == ki && cidx[j] < ui);
+    if (r == k - 1) { s_tkey = ki; s_tidx = ui; }
+  }
+  __syncthreads();
+  const unsigned long long tkey = s_tkey; const int tidx = s_tidx;
+  // (3) flags and the iteration's work list, canonical order
+  int2 carry = make_int2(0, 0);
+  for (int base = 0; base < p.P; base += kSelThreads) {
+    const int q = base + tid;
+    int f = 0, nw = 0, w0 = 0;
+    if (q < p.P) {
+      const int u = p.perm[q];
+      const unsigned long long key = subset_key(p.seed, step, u);
+      f = (key < tkey) || (key == tkey && u <= tidx);
+      p.flag[q] = (uint8_t)f;
+      if (f) { w0 = p.work_off[q]; nw = p.work_off[q + 1] - w0; }
+    }
+    int2 tot;
+    const int2 inc = block_scan2(make_int2(f, nw), wtot, &tot);
+    if (f && p.sel_work) {
+      const int off = carry.y + inc.y - nw;
+      for (int w = 0; w < nw; ++w) p.sel_work[off + w] = w0 + w;
+    }
+    carry.x += tot.x; carry.y += tot.y;
+  }
+  if (tid == 0) { p.info[0] = carry.y; p.info[1] = carry.x; }
+}
+
 }  // namespace
 
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2** out_pairs, int32_t** out_perm,
@@ -168,5 +306,20 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
 #undef PR_CUDA
   *out_pairs = canon; *out_perm = perm; *out_tgt_off = tgt_off; *out_src_off = src_off; *out_src_inc = src_inc;
   *out_work = work; *out_work_off = work_off; *out_n_work = n_work;
+  return EPO_OK;
+}
+
+epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override, bool gated, bool build_work) {
+  SelParams p;
+  p.perm = ctx->d_perm; p.work_off = ctx->d_work_off; p.state = ctx->d_state; p.flag = ctx->d_sel_flag;
+  p.sel_work = build_work ? ctx->d_sel_work : nullptr; p.info = ctx->d_sel_info; p.seed = ctx->cfg.subsample_seed;
+  p.P = (int)ctx->P; p.M = ctx->cfg.pair_budget; p.step_override = step_override; p.gated = gated ? 1 : 0;
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(1); lc.blockDim = dim3(kSelThreads); lc.dynamicSmemBytes = 0; lc.stream = ctx->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = (ctx->pdl && gated) ? 1 : 0;
+  EPO_CUDA(ctx, cudaLaunchKernelEx(&lc, k_select_pairs, p));
+  ctx->launches += 1;
   return EPO_OK;
 }

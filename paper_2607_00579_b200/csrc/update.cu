@@ -19,6 +19,7 @@ struct FinParams {
   const int2* pairs;
   const int32_t *tgt_off, *src_off, *src_inc, *work_off;
   const double* part;
+  const uint8_t* sel_flag;      // pair sub-sampling: membership of this iteration's subset (canonical order), else nullptr
   float* pair_loss;
   int32_t* pair_valid;
   double *grad, *loss_part;
@@ -136,12 +137,23 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   __shared__ int s_last;
   const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = p.N;
   constexpr int kWarps = kFinThreads / 32;
-  // The pair lists are static: read this camera's ranges and this warp's first pair before waiting for the
-  // fused kernel (programmatic dependent launch: this prologue overlaps the fused kernel's tail).
+  // The pair lists are static: read this camera's ranges, and for every lane one incident pair with its range of
+  // work items, before waiting for the fused kernel (programmatic dependent launch: this prologue overlaps the
+  // fused kernel's tail).  Incident pairs = first those with target c, then those with source c; warp w takes
+  // groups w, w + 8, ... of G consecutive ones (G <= 32 chosen so that all warps share a short list).
   const int t0 = p.tgt_off[c], nt = p.tgt_off[c + 1] - t0, s0 = p.src_off[c], n_inc = nt + p.src_off[c + 1] - s0;
-  auto pair_of = [&](int j) { return j < nt ? t0 + j : p.src_inc[s0 + j - nt]; };
-  int j = warp, q = 0, w0 = 0, w1 = 0;
-  if (j < n_inc) { q = pair_of(j); w0 = p.work_off[q]; w1 = p.work_off[q + 1]; }
+  int G = (n_inc + kWarps - 1) / kWarps;
+  G = G < 1 ? 1 : (G > 32 ? 32 : G);
+  auto fetch = [&](int j0, int* q, int* w0, int* w1) {
+    const int j = j0 + lane;
+    *q = -1; *w0 = 0; *w1 = 0;
+    if (lane < G && j < n_inc) {
+      *q = j < nt ? t0 + j : p.src_inc[s0 + j - nt];
+      *w0 = p.work_off[*q]; *w1 = p.work_off[*q + 1];
+    }
+  };
+  int j0 = warp * G, q, w0, w1;
+  fetch(j0, &q, &w0, &w1);
   cudaTriggerProgrammaticLaunchCompletion();       // the next fused kernel may start its own static prologue
   cudaGridDependencySynchronize();                 // partial sums, poses and the control block are final now
   if (p.gated && st->stopped) {
@@ -149,39 +161,46 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     return;
   }
   const double* Pc = p.poses + 12 * (size_t)c;
-  // ---- a-9: one warp per incident pair (first the pairs with target c, then those with source c); lane 0
-  // accumulates the loss sum, lanes 2..7 the six gradient coordinates
+  // ---- a-9: one warp per incident pair; lane 0 accumulates the loss sum, lanes 2..7 the six gradient
+  // coordinates.  With pair sub-sampling only the pairs of this iteration's subset count.
   double acc = 0.0;
-  while (j < n_inc) {
-    // per-pair sums: lane l adds value (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... (independent loads), then
-    // the four chunk classes are combined by two xor-shuffles: a fixed order
-    double v = 0.0;
-    for (int w = w0 + (lane >> 3); w < w1; w += 4) v += __ldcg(p.part + (size_t)w * kAccStride + (lane & 7));
-    const bool tgt = j < nt;
-    const int qc = q;
-    j += kWarps;
-    if (j < n_inc) { q = pair_of(j); w0 = p.work_off[q]; w1 = p.work_off[q + 1]; }   // next pair's range, in flight
-    v += __shfl_xor_sync(0xffffffffu, v, 8);
-    v += __shfl_xor_sync(0xffffffffu, v, 16);
-    const double n = __shfl_sync(0xffffffffu, v, 1);
-    if (tgt) {
-      const double S = __shfl_sync(0xffffffffu, v, 0);
-      const double L = n > 0.0 ? S / n : 0.0;
-      if (lane == 0) { p.pair_loss[qc] = (float)L; p.pair_valid[qc] = (int32_t)n; acc += L; }
-      else if (lane >= 2 && lane < 8 && n > 0.0) acc += v / n;
-    } else {
-      const double A0 = __shfl_sync(0xffffffffu, v, 2), A1 = __shfl_sync(0xffffffffu, v, 3), A2 = __shfl_sync(0xffffffffu, v, 4);
-      double m0 = __shfl_sync(0xffffffffu, v, 5), m1 = __shfl_sync(0xffffffffu, v, 6), m2 = __shfl_sync(0xffffffffu, v, 7);
-      if (lane >= 2 && lane < 8 && n > 0.0) {
-        const double* Pt = p.poses + 12 * (size_t)p.pairs[qc].y;
-        const int i = (lane - 2) % 3;
-        const double r0 = rel_pose_entry(Pc, Pt, i), r1 = rel_pose_entry(Pc, Pt, 4 + i), r2 = rel_pose_entry(Pc, Pt, 8 + i);
-        if (lane < 5) {
-          acc -= (r0 * A0 + r1 * A1 + r2 * A2) / n;                      // R^T A
-        } else {
-          const double t0 = rel_pose_entry(Pc, Pt, 3), t1 = rel_pose_entry(Pc, Pt, 7), t2 = rel_pose_entry(Pc, Pt, 11);
-          m0 -= t1 * A2 - t2 * A1; m1 -= t2 * A0 - t0 * A2; m2 -= t0 * A1 - t1 * A0;   // M' = M - t_ts x A
-          acc -= (r0 * m0 + r1 * m1 + r2 * m2) / n;                      // R^T M'
+  while (j0 < n_inc) {
+    unsigned todo = __ballot_sync(0xffffffffu, q >= 0 && (p.sel_flag == nullptr || p.sel_flag[q] != 0));
+    const int jc = j0, qm = q, w0m = w0, w1m = w1;
+    j0 += kWarps * G;
+    if (j0 < n_inc) fetch(j0, &q, &w0, &w1);       // the next group's ranges, in flight
+    while (todo) {
+      const int b = __ffs(todo) - 1;
+      todo &= todo - 1;
+      const int qc = __shfl_sync(0xffffffffu, qm, b);
+      const int wa = __shfl_sync(0xffffffffu, w0m, b), wb = __shfl_sync(0xffffffffu, w1m, b);
+      const bool tgt = jc + b < nt;
+      // per-pair sums: lane l adds value (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... (independent loads), then
+      // the four chunk classes are combined by two xor-shuffles: a fixed order
+      double v = 0.0;
+      for (int w = wa + (lane >> 3); w < wb; w += 4) v += __ldcg(p.part + (size_t)w * kAccStride + (lane & 7));
+      v += __shfl_xor_sync(0xffffffffu, v, 8);
+      v += __shfl_xor_sync(0xffffffffu, v, 16);
+      const double n = __shfl_sync(0xffffffffu, v, 1);
+      if (tgt) {
+        const double S = __shfl_sync(0xffffffffu, v, 0);
+        const double L = n > 0.0 ? S / n : 0.0;
+        if (lane == 0) { p.pair_loss[qc] = (float)L; p.pair_valid[qc] = (int32_t)n; acc += L; }
+        else if (lane >= 2 && lane < 8 && n > 0.0) acc += v / n;
+      } else {
+        const double A0 = __shfl_sync(0xffffffffu, v, 2), A1 = __shfl_sync(0xffffffffu, v, 3), A2 = __shfl_sync(0xffffffffu, v, 4);
+        double m0 = __shfl_sync(0xffffffffu, v, 5), m1 = __shfl_sync(0xffffffffu, v, 6), m2 = __shfl_sync(0xffffffffu, v, 7);
+        if (lane >= 2 && lane < 8 && n > 0.0) {
+          const double* Pt = p.poses + 12 * (size_t)p.pairs[qc].y;
+          const int i = (lane - 2) % 3;
+          const double r0 = rel_pose_entry(Pc, Pt, i), r1 = rel_pose_entry(Pc, Pt, 4 + i), r2 = rel_pose_entry(Pc, Pt, 8 + i);
+          if (lane < 5) {
+            acc -= (r0 * A0 + r1 * A1 + r2 * A2) / n;                      // R^T A
+          } else {
+            const double t0 = rel_pose_entry(Pc, Pt, 3), t1 = rel_pose_entry(Pc, Pt, 7), t2 = rel_pose_entry(Pc, Pt, 11);
+            m0 -= t1 * A2 - t2 * A1; m1 -= t2 * A0 - t0 * A2; m2 -= t0 * A1 - t1 * A0;   // M' = M - t_ts x A
+            acc -= (r0 * m0 + r1 * m1 + r2 * m2) / n;                      // R^T M'
+          }
         }
       }
     }
@@ -330,14 +349,16 @@ __global__ void k_f32_to_f64(const float* __restrict__ in, double* __restrict__ 
 
 }  // namespace
 
-epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first) {
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset) {
   FinParams p;
+  p.sel_flag = subset ? ctx->d_sel_flag : nullptr;
   p.pairs = ctx->d_pairs; p.tgt_off = ctx->d_tgt_off; p.src_off = ctx->d_src_off; p.src_inc = ctx->d_src_inc;
   p.work_off = ctx->d_work_off; p.part = ctx->d_part; p.pair_loss = ctx->d_pair_loss; p.pair_valid = ctx->d_pair_valid;
   p.grad = ctx->d_grad; p.loss_part = ctx->d_loss_part;
   p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.m = ctx->d_m; p.v = ctx->d_v;
   p.dR = ctx->d_dR; p.dt = ctx->d_dt; p.theta = ctx->d_theta; p.loss_trace = ctx->d_loss_trace;
-  p.state = ctx->d_state; p.N = ctx->N; p.P = ctx->P;
+  p.state = ctx->d_state; p.N = ctx->N;
+  p.P = subset ? (int64_t)ctx->cfg.pair_budget : ctx->P;     // the mean runs over the pairs that were evaluated
   p.sched = ctx->d_sched; p.beta1 = ctx->cfg.beta1; p.beta2 = ctx->cfg.beta2; p.adam_eps = ctx->cfg.adam_eps;
   p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.max_steps = ctx->cfg.max_steps;
   p.w1 = ctx->cfg.w1; p.w2 = ctx->cfg.w2; p.smooth = ctx->cfg.smooth_window; p.early_stop = ctx->cfg.early_stop;

@@ -114,3 +114,32 @@ def test_full_size_config5_early_stop_runs_to_its_own_stop():
     assert fired == done, (fired, done)
     assert e.step(10) == (0, 2)
     e.destroy()
+
+
+def test_full_size_config4_stochastic_pair_subsampling():
+    """Config 4's 39,800 pairs with the paper's budget M = 1024: the device draw equals the oracle's
+    bit for bit, and three iterations on the drawn subsets match the oracle in lock-step."""
+    M, seed = 1024, 2607
+    sc, e, prob = _full(4, early_stop=0, pair_budget=M, subsample_seed=seed)
+    Pn = len(sc.pairs)
+    for step in (0, 1, 500):
+        got = e.get_pair_subset(step)
+        assert got.sum() == M and np.array_equal(got, oracle.pair_subset(seed, step, Pn, M)), step
+    ocfg = oracle_config(coord_fp32=1, early_stop=0)
+    N = sc.n_views
+    m = np.zeros((N, 6)); v = np.zeros((N, 6))
+    P = e.get_poses_f64()
+    for k in range(3):
+        pairs_k = sc.pairs[oracle.pair_subset(seed, k, Pn, M)]
+        ref = oracle.loss_grad(prob, P, pairs_k, oracle.lam_schedule(k, ocfg), z_min=Z_MIN, coord_fp32=1)
+        inc = oracle.adam(ref["grad"].reshape(-1), m.reshape(-1), v.reshape(-1), k, oracle.lr_schedule(k, ocfg),
+                          ocfg.beta1, ocfg.beta2, ocfg.adam_eps).reshape(N, 6)
+        pred = np.stack([oracle.se3_compose(oracle.se3_exp(inc[c]), P[c]) for c in range(N)])
+        assert e.step(1)[0] == 1
+        new = e.get_poses_f64()
+        rot, tr = pose_errors(new, pred)
+        loss, _ = e.get_trace(k, 1)
+        assert rot <= 1e-3 and tr <= 1e-4, (k, rot, tr)
+        assert abs(float(loss[0]) - ref["loss"]) <= 1e-5 * abs(ref["loss"]), (k, float(loss[0]), ref["loss"])
+        P = new
+    e.destroy()

@@ -211,8 +211,11 @@ def _lockstep(sc, iters, cfg_kw, okw):
     assert np.array_equal(poses, sc.poses_init.astype(np.float64))
     worst = dict(rot=0.0, tr=0.0, theta=0.0, loss=0.0)
     thetas = []; phase = 0; stop_at = None
+    budget, seed = cfg_kw.get("pair_budget", 0), cfg_kw.get("subsample_seed", 0)
     for k in range(iters):
-        ref = oracle.loss_grad(prob, poses, sc.pairs, oracle.lam_schedule(k, ocfg), z_min=Z_MIN, coord_fp32=1)
+        # stochastic viewgraph sub-sampling: the oracle evaluates its own draw of step k
+        pairs_k = sc.pairs[oracle.pair_subset(seed, k, len(sc.pairs), budget)] if budget else sc.pairs
+        ref = oracle.loss_grad(prob, poses, pairs_k, oracle.lam_schedule(k, ocfg), z_min=Z_MIN, coord_fp32=1)
         inc = oracle.adam(ref["grad"].reshape(-1), m.reshape(-1), v.reshape(-1), k, oracle.lr_schedule(k, ocfg),
                           ocfg.beta1, ocfg.beta2, ocfg.adam_eps).reshape(N, 6)
         pred = np.stack([oracle.se3_compose(oracle.se3_exp(inc[c]), poses[c]) for c in range(N)])
@@ -322,6 +325,40 @@ def test_early_stop_parity():
     done2, _ = e.step(done)
     assert done2 == done
     e.destroy()
+
+
+# ------------------------------------------------------------------- stochastic pair sub-sampling
+@pytest.mark.parametrize("n_views,budget,seed", [(6, 7, 1), (12, 40, 2607), (50, 1024, 5)])
+def test_pair_subset_bit_exact(n_views, budget, seed):
+    """The subset drawn on the device at step s equals the oracle's (keys, full sort, first M), bit for bit:
+    30 pairs (below the radix threshold), 132 pairs, and 2450 pairs (radix refinement + candidate ranking)."""
+    sc = make_scene(config=4, n_views=n_views)
+    e = make_ctx(sc, pair_budget=budget, subsample_seed=seed)
+    P = len(sc.pairs)
+    for step in (0, 1, 2, 17, 1999):
+        got = e.get_pair_subset(step)
+        assert got.sum() == min(P, budget)
+        assert np.array_equal(got, oracle.pair_subset(seed, step, P, budget)), step
+    e.destroy()
+    off = make_ctx(sc)                                  # budget 0: every pair, every step
+    assert off.get_pair_subset(3).all()
+    off.destroy()
+
+
+def test_subsampled_iterations_match_the_oracle():
+    """epo_step with a pair budget: every iteration's loss, update and theta95 against the oracle evaluated on the
+    oracle's own draw of that step (mean over the M drawn pairs)."""
+    kw = dict(early_stop=0, pair_budget=9, subsample_seed=77)
+    worst, _, n = _lockstep(scene("room6"), 40, kw, dict(early_stop=0))
+    print(f"sub-sampled room6 (9 of 30 pairs per step): worst rot {worst['rot']:.2e} deg, trans {worst['tr']:.2e}, "
+          f"theta95 rel {worst['theta']:.2e}, loss rel {worst['loss']:.2e}")
+    assert n == 40
+    assert worst["rot"] <= 1e-3 and worst["tr"] <= 1e-4 and worst["theta"] <= 1e-3 and worst["loss"] <= 1e-5
+    # a budget at or above the list length changes nothing (Alg. 3 l.5)
+    a = make_ctx(scene("room6"), early_stop=0, pair_budget=30, subsample_seed=77); b = make_ctx(scene("room6"), early_stop=0)
+    a.step(10); b.step(10)
+    assert np.array_equal(a.get_poses_f64(), b.get_poses_f64())
+    a.destroy(); b.destroy()
 
 
 def test_step_in_pieces_equals_one_call():
