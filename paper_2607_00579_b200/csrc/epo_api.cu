@@ -66,8 +66,8 @@ void free_views(epo_ctx* c) {
 void free_pairs(epo_ctx* c) {
   cudaFree(c->d_pairs); cudaFree(c->d_perm); cudaFree(c->d_tgt_off); cudaFree(c->d_src_off); cudaFree(c->d_src_inc);
   cudaFree(c->d_work); cudaFree(c->d_work_off); cudaFree(c->d_part); cudaFree(c->d_pair_loss); cudaFree(c->d_pair_valid); cudaFree(c->d_out_f);
-  cudaFree(c->d_out_i); cudaFree(c->d_sel_flag); cudaFree(c->d_sel_work); cudaFree(c->d_sel_info);
-  c->d_sel_flag = nullptr; c->d_sel_work = nullptr; c->d_sel_info = nullptr; c->subsample = false; c->sel_grid = 0;
+  cudaFree(c->d_out_i); cudaFree(c->d_sel_flag); cudaFree(c->d_sel_work); cudaFree(c->d_sel_info); cudaFree(c->d_sel_scratch);
+  c->d_sel_scratch = nullptr; c->d_sel_flag = nullptr; c->d_sel_work = nullptr; c->d_sel_info = nullptr; c->subsample = false; c->sel_grid = 0;
   c->d_pairs = nullptr; c->d_perm = nullptr; c->d_tgt_off = nullptr; c->d_src_off = nullptr; c->d_src_inc = nullptr;
   c->d_work = nullptr; c->d_work_off = nullptr; c->d_part = nullptr; c->d_pair_loss = nullptr; c->d_pair_valid = nullptr; c->d_out_f = nullptr;
   c->d_out_i = nullptr;
@@ -288,7 +288,14 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
                                      : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
   cudaFree(d_user);
   double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
-  uint8_t* sflag = nullptr; int32_t* swork = nullptr; int32_t* sinfo = nullptr;
+  uint8_t* sflag = nullptr; int32_t* swork = nullptr; int32_t* sinfo = nullptr; int32_t* sscr = nullptr;
+  if (rc == EPO_OK && c->cfg.pair_budget > 0 && P > c->cfg.pair_budget && P > epo_select_max_pairs())
+    rc = epo_fail(c, EPO_ERR_UNSUPPORTED, "pair sub-sampling supports at most %lld pairs", (long long)epo_select_max_pairs());
+  if (rc == EPO_OK) {
+    e = cudaMalloc(&sscr, (size_t)kSelScrInts * sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(sscr, 0, (size_t)kSelScrInts * sizeof(int32_t), st);
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
+  }
   if (rc == EPO_OK) {
     e = cudaMalloc(&sflag, (size_t)P);
     if (e == cudaSuccess) e = cudaMalloc(&swork, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int32_t));
@@ -314,14 +321,14 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
     cudaGetLastError();
     cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(toff); cudaFree(soff); cudaFree(sinc); cudaFree(woff);
     cudaFree(acc); cudaFree(pl); cudaFree(pv); cudaFree(of); cudaFree(oi);
-    cudaFree(sflag); cudaFree(swork); cudaFree(sinfo);
+    cudaFree(sflag); cudaFree(swork); cudaFree(sinfo); cudaFree(sscr);
     return rc;
   }
   free_pairs(c);
   c->d_pairs = canon; c->d_perm = perm; c->d_tgt_off = toff; c->d_src_off = soff; c->d_src_inc = sinc; c->d_work = work;
   c->d_work_off = woff; c->n_work = n_work; c->P = P; c->d_part = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
   c->h_pairs.swap(hp); c->reproj_per_eval = reproj; c->lg_chunk = chunk;
-  c->d_sel_flag = sflag; c->d_sel_work = swork; c->d_sel_info = sinfo;
+  c->d_sel_flag = sflag; c->d_sel_work = swork; c->d_sel_info = sinfo; c->d_sel_scratch = sscr;
   // stochastic pair sub-sampling: only when the list is longer than the budget (Alg. 3 l.3-6)
   c->subsample = c->cfg.pair_budget > 0 && P > c->cfg.pair_budget;
   {

@@ -104,6 +104,7 @@ struct epo_ctx {
   uint8_t* d_sel_flag;    // [P] canonical order: in this iteration's subset
   int32_t* d_sel_work;    // [n_work] static work-item indices of the subset's pairs, in order
   int32_t* d_sel_info;    // {work items, pairs} of the subset
+  int32_t* d_sel_scratch; // kSelScrInts ints, zero between launches of k_select_pairs (layout below)
   int64_t sel_grid;       // upper bound on the subset's work items (the fused kernel's grid in that mode)
 
   // per-evaluation buffers
@@ -178,6 +179,13 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
                            int32_t** out_src_inc, int4** out_work, int32_t** out_work_off, int64_t* out_n_work,
                            int chunk);
+// scratch of k_select_pairs (ints): grid-barrier counter + exit ticket, candidate count, global histogram, per-CTA
+// totals, candidate keys (64-bit) and indices.  At most kSelMaxCtas CTAs of 4096 pairs (all resident: a spin barrier).
+constexpr int kSelMaxCtas = 128, kSelCandCap = 4096;
+constexpr int kSelScrBarrier = 0, kSelScrNCand = 2, kSelScrHist = 4, kSelScrTotals = kSelScrHist + 2048,
+              kSelScrCandKey = kSelScrTotals + 2 * kSelMaxCtas, kSelScrCandIdx = kSelScrCandKey + 2 * kSelCandCap,
+              kSelScrInts = kSelScrCandIdx + kSelCandCap;
+int64_t epo_select_max_pairs(void);
 epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override /* < 0: device step */, bool gated, bool build_work);
 // lossgrad.cu
 epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);

@@ -106,14 +106,21 @@ __global__ void k_fill_work(const int32_t* __restrict__ work_off, const int2* __
 // Stochastic viewgraph sub-sampling (Alg. 3 l.3-6): every iteration evaluates a
 // fresh uniform random subset S of the pair list, |S| = M.  The draw is a pure function of (seed, step, pair):
 // pair p (position in the caller's list) gets key(step, p) = output number step * 2^32 + p + 1 of
-// SplitMix64(seed), and S = the M pairs with the smallest (key, p) (include/epo.h).  One CTA per iteration, no
-// host involvement: (1) radix refinement, 11 key bits per sweep, of the bin that holds the M-th smallest key until
-// it has at most kSelCap members (one sweep in practice: P / 2048 expected members), (2) the members are
-// collected in shared memory and the one of rank M is found by counting, (3) one more sweep in canonical
-// (target-major) order writes the membership flags and, by a block-wide scan, the iteration's work list: the
-// indices of the static work items of the selected pairs, in order.
+// SplitMix64(seed), and S = the M pairs with the smallest (key, p) (include/epo.h).  One launch per iteration, no
+// host involvement.  CTA g owns the canonical pairs [g C, (g + 1) C), C = 4096; the CTAs are all resident (at most
+// kSelMaxCtas of them, one per SM) and meet at three grid barriers:
+//   A  histogram of the keys' leading 11 bits (shared, then global)                              -- barrier 1
+//   B  every CTA scans the 2048 bins for the one that holds the M-th smallest key and appends its own members of
+//      that bin (P / 2048 expected) to a global candidate list                                     -- barrier 2
+//   C  every CTA ranks the candidates by (key, p) and so knows the M-th smallest pair T
+//   D  flags of its own pairs ((key, p) <= T), block scan of (selected, their work items)         -- barrier 3
+//      then, with the totals of the CTAs before it, its part of the iteration's ordered work list.
+// The last CTA out re-zeroes the histogram and the counters for the next launch.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kSelThreads = 1024, kSelBits = 11, kSelBins = 1 << kSelBits, kSelCap = 2048;
+constexpr int kSelUnroll = 4;
+constexpr int kSelThreads = 1024, kSelBits = 11, kSelBins = 1 << kSelBits;
+constexpr int kSelChunk = kSelUnroll * kSelThreads;       // pairs per CTA
+constexpr int kSelStage = 1024;                           // candidates ranked from shared memory
 
 __device__ __forceinline__ unsigned long long subset_key(unsigned long long seed, int step, int p) {
   unsigned long long z = seed + 0x9E3779B97F4A7C15ull * (((unsigned long long)(unsigned)step << 32) + (unsigned long long)p + 1ull);
@@ -148,96 +155,143 @@ __device__ int2 block_scan2(int2 v, int2* warp_tot /* [32] shared */, int2* tota
   return v;
 }
 
+// all CTAs of the grid are resident (the launcher guarantees gridDim.x <= number of SMs): arrive, then spin
+__device__ __forceinline__ void grid_barrier(int* counter, int target) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    atomicAdd(counter, 1);
+    while (atomicAdd(counter, 0) < target) __nanosleep(64);
+    __threadfence();
+  }
+  __syncthreads();
+}
+
 struct SelParams {
-  const int32_t* perm;       // canonical -> caller's pair index
-  const int32_t* work_off;   // [P+1] static work items of each canonical pair
+  const int32_t* __restrict__ perm;       // canonical -> caller's pair index
+  const int32_t* __restrict__ work_off;   // [P+1] static work items of each canonical pair
   const DevState* state;
   uint8_t* flag;             // [P] canonical order: 1 = in this iteration's subset
-  int32_t* sel_work;         // [n_work] static work-item indices of the subset, in order
+  int32_t* sel_work;         // [n_work] static work-item indices of the subset, in order (nullptr: flags only)
   int32_t* info;             // {work items of the subset, pairs of the subset}
+  int32_t* scratch;          // EpoSelScratch, zero between launches
   unsigned long long seed;
   int P, M, step_override /* < 0: the device step counter */, gated;
 };
 
-__global__ void __launch_bounds__(kSelThreads) k_select_pairs(const SelParams p) {
+__global__ void __launch_bounds__(kSelThreads, 1) k_select_pairs(const SelParams p) {
   __shared__ int hist[kSelBins];
-  __shared__ unsigned long long ckey[kSelCap];
-  __shared__ int cidx[kSelCap];
+  __shared__ unsigned long long skey[kSelStage];
+  __shared__ int sidx[kSelStage];
   __shared__ int2 wtot[32];
-  __shared__ int s_bin, s_below, s_cnt, s_n;
+  __shared__ int s_bin, s_below;
   __shared__ unsigned long long s_tkey;
-  __shared__ int s_tidx;
-  const int tid = threadIdx.x;
+  __shared__ int s_tidx, s_last;
+  const int tid = threadIdx.x, G = (int)gridDim.x, g = (int)blockIdx.x;
+  int* bar = p.scratch + kSelScrBarrier;
+  int* ghist = p.scratch + kSelScrHist;
+  int* ncand = p.scratch + kSelScrNCand;
+  int2* tots = reinterpret_cast<int2*>(p.scratch + kSelScrTotals);
+  unsigned long long* ckey = reinterpret_cast<unsigned long long*>(p.scratch + kSelScrCandKey);
+  int* cidx = p.scratch + kSelScrCandIdx;
+  // this thread's pairs: static loads before the grid-dependency wait
+  int u[kSelUnroll], wo[kSelUnroll + 1];
+  const int q0 = g * kSelChunk + kSelUnroll * tid;
+#pragma unroll
+  for (int i = 0; i < kSelUnroll; ++i) {
+    u[i] = q0 + i < p.P ? __ldg(p.perm + q0 + i) : -1;
+    wo[i] = q0 + i <= p.P ? __ldg(p.work_off + q0 + i) : 0;
+  }
+  wo[kSelUnroll] = q0 + kSelUnroll <= p.P ? __ldg(p.work_off + q0 + kSelUnroll) : 0;
+  for (int i = tid; i < kSelBins; i += kSelThreads) hist[i] = 0;
   cudaTriggerProgrammaticLaunchCompletion();
   cudaGridDependencySynchronize();
   if (p.gated && p.state->stopped) return;
   const int step = p.step_override >= 0 ? p.step_override : p.state->step;
-  // (1) the bin of the M-th smallest key: `prefix` = its leading `nbits` bits, k = rank wanted inside it (1-based)
-  unsigned long long prefix = 0;
-  int nbits = 0, k = p.M, members = p.P;
-  while (members > kSelCap && nbits < 64) {
-    const int db = 64 - nbits < kSelBits ? 64 - nbits : kSelBits;
-    for (int i = tid; i < kSelBins; i += kSelThreads) hist[i] = 0;
-    __syncthreads();
-    for (int q = tid; q < p.P; q += kSelThreads) {
-      const unsigned long long key = subset_key(p.seed, step, p.perm[q]);
-      if (nbits == 0 || (key >> (64 - nbits)) == prefix) atomicAdd(&hist[(int)((key >> (64 - nbits - db)) & ((1u << db) - 1))], 1);
-    }
-    __syncthreads();
-    // two bins per thread, exclusive scan, the bin where the running count crosses k
-    const int h0 = hist[2 * tid], h1 = hist[2 * tid + 1];
+  unsigned long long key[kSelUnroll];
+#pragma unroll
+  for (int i = 0; i < kSelUnroll; ++i) key[i] = u[i] >= 0 ? subset_key(p.seed, step, u[i]) : ~0ull;
+  // ---- A: histogram of the leading bits
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < kSelUnroll; ++i)
+    if (u[i] >= 0) atomicAdd(&hist[(int)(key[i] >> (64 - kSelBits))], 1);
+  __syncthreads();
+  for (int i = tid; i < kSelBins; i += kSelThreads)
+    if (hist[i]) atomicAdd(&ghist[i], hist[i]);
+  grid_barrier(bar, G);
+  // ---- B: the bin of the M-th smallest key (two bins per thread), then this CTA's members of it
+  {
+    const int h0 = __ldcg(ghist + 2 * tid), h1 = __ldcg(ghist + 2 * tid + 1);
     int2 tot;
     const int2 inc = block_scan2(make_int2(h0 + h1, 0), wtot, &tot);
     const int before = inc.x - h0 - h1;
-    if (before < k && k <= before + h0) { s_bin = 2 * tid; s_below = before; s_cnt = h0; }
-    else if (before + h0 < k && k <= before + h0 + h1) { s_bin = 2 * tid + 1; s_below = before + h0; s_cnt = h1; }
-    __syncthreads();
-    prefix = (prefix << db) | (unsigned long long)s_bin;
-    nbits += db; k -= s_below; members = s_cnt;
+    if (before < p.M && p.M <= before + h0) { s_bin = 2 * tid; s_below = before; }
+    else if (before + h0 < p.M && p.M <= before + h0 + h1) { s_bin = 2 * tid + 1; s_below = before + h0; }
     __syncthreads();
   }
-  // (2) collect the members of that bin and find the one of rank k by (key, caller's index)
-  if (tid == 0) s_n = 0;
-  __syncthreads();
-  for (int q = tid; q < p.P; q += kSelThreads) {
-    const int u = p.perm[q];
-    const unsigned long long key = subset_key(p.seed, step, u);
-    if (nbits == 0 || (key >> (64 - nbits)) == prefix) {
-      const int pos = atomicAdd(&s_n, 1);
-      if (pos < kSelCap) { ckey[pos] = key; cidx[pos] = u; }
+  const int bin = s_bin, k = p.M - s_below;          // rank wanted inside the bin, 1-based
+#pragma unroll
+  for (int i = 0; i < kSelUnroll; ++i)
+    if (u[i] >= 0 && (int)(key[i] >> (64 - kSelBits)) == bin) {
+      const int pos = atomicAdd(ncand, 1);
+      if (pos < kSelCandCap) { ckey[pos] = key[i]; cidx[pos] = u[i]; }
     }
+  grid_barrier(bar, 2 * G);
+  // ---- C: the candidate of rank k by (key, caller's index)
+  {
+    int n = __ldcg(ncand);
+    n = n < kSelCandCap ? n : kSelCandCap;           // more only if P > 2048 * kSelCandCap / 4 (refused by the host)
+    const bool staged = n <= kSelStage;               // the usual case: rank from shared memory
+    if (staged) {
+      for (int i = tid; i < n; i += kSelThreads) { skey[i] = __ldcg(ckey + i); sidx[i] = __ldcg(cidx + i); }
+      __syncthreads();
+    }
+    for (int i = tid; i < n; i += kSelThreads) {
+      const unsigned long long ki = staged ? skey[i] : __ldcg(ckey + i); const int ui = staged ? sidx[i] : __ldcg(cidx + i);
+      int r = 0;
+      if (staged) for (int j = 0; j < n; ++j) r += (skey[j] < ki) || (skey[j] == ki && sidx[j] < ui);
+      else for (int j = 0; j < n; ++j) { const unsigned long long kj = __ldcg(ckey + j); r += (kj < ki) || (kj == ki && __ldcg(cidx + j) < ui); }
+      if (r == k - 1) { s_tkey = ki; s_tidx = ui; }
+    }
+    __syncthreads();
   }
-  __syncthreads();
-  const int n = s_n < kSelCap ? s_n : kSelCap;   // s_n > kSelCap only if > 2048 pairs share one 64-bit key
-  for (int i = tid; i < n; i += kSelThreads) {
-    const unsigned long long ki = ckey[i]; const int ui = cidx[i];
-    int r = 0;
-    for (int j = 0; j < n; ++j) r += (ckey[j] < ki) || (ckey[j] == ki && cidx[j] < ui);
-    if (r == k - 1) { s_tkey = ki; s_tidx = ui; }
-  }
-  __syncthreads();
   const unsigned long long tkey = s_tkey; const int tidx = s_tidx;
-  // (3) flags and the iteration's work list, canonical order
-  int2 carry = make_int2(0, 0);
-  for (int base = 0; base < p.P; base += kSelThreads) {
-    const int q = base + tid;
-    int f = 0, nw = 0, w0 = 0;
-    if (q < p.P) {
-      const int u = p.perm[q];
-      const unsigned long long key = subset_key(p.seed, step, u);
-      f = (key < tkey) || (key == tkey && u <= tidx);
-      p.flag[q] = (uint8_t)f;
-      if (f) { w0 = p.work_off[q]; nw = p.work_off[q + 1] - w0; }
+  // ---- D: flags, counts, ordered work list
+  int f[kSelUnroll], nw[kSelUnroll], fs = 0, ws = 0;
+#pragma unroll
+  for (int i = 0; i < kSelUnroll; ++i) {
+    f[i] = 0; nw[i] = 0;
+    if (u[i] >= 0) {
+      f[i] = (key[i] < tkey) || (key[i] == tkey && u[i] <= tidx);
+      p.flag[q0 + i] = (uint8_t)f[i];
+      if (f[i]) nw[i] = wo[i + 1] - wo[i];
     }
-    int2 tot;
-    const int2 inc = block_scan2(make_int2(f, nw), wtot, &tot);
-    if (f && p.sel_work) {
-      const int off = carry.y + inc.y - nw;
-      for (int w = 0; w < nw; ++w) p.sel_work[off + w] = w0 + w;
-    }
-    carry.x += tot.x; carry.y += tot.y;
+    fs += f[i]; ws += nw[i];
   }
-  if (tid == 0) { p.info[0] = carry.y; p.info[1] = carry.x; }
+  int2 tot;
+  const int2 inc = block_scan2(make_int2(fs, ws), wtot, &tot);
+  if (tid == 0) { tots[g] = tot; }
+  grid_barrier(bar, 3 * G);
+  int2 carry = make_int2(0, 0);
+  for (int j = 0; j < g; ++j) { const int2 t = __ldcg(tots + j); carry.x += t.x; carry.y += t.y; }
+  if (p.sel_work) {
+    int off = carry.y + inc.y - ws;
+#pragma unroll
+    for (int i = 0; i < kSelUnroll; ++i) {
+      for (int w = 0; w < nw[i]; ++w) p.sel_work[off + w] = wo[i] + w;
+      off += nw[i];
+    }
+  }
+  if (g == G - 1 && tid == 0) { p.info[0] = carry.y + tot.y; p.info[1] = carry.x + tot.x; }
+  // ---- the last CTA out cleans up for the next launch
+  __syncthreads();
+  if (tid == 0) s_last = atomicAdd(bar + 1, 1) == G - 1;
+  __syncthreads();
+  if (s_last) {
+    for (int i = tid; i < kSelBins; i += kSelThreads) ghist[i] = 0;
+    if (tid == 0) { *ncand = 0; bar[0] = 0; bar[1] = 0; }
+  }
 }
 
 }  // namespace
@@ -312,10 +366,12 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
 epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override, bool gated, bool build_work) {
   SelParams p;
   p.perm = ctx->d_perm; p.work_off = ctx->d_work_off; p.state = ctx->d_state; p.flag = ctx->d_sel_flag;
-  p.sel_work = build_work ? ctx->d_sel_work : nullptr; p.info = ctx->d_sel_info; p.seed = ctx->cfg.subsample_seed;
+  p.sel_work = build_work ? ctx->d_sel_work : nullptr; p.info = ctx->d_sel_info; p.scratch = ctx->d_sel_scratch;
+  p.seed = ctx->cfg.subsample_seed;
   p.P = (int)ctx->P; p.M = ctx->cfg.pair_budget; p.step_override = step_override; p.gated = gated ? 1 : 0;
   cudaLaunchConfig_t lc = {};
-  lc.gridDim = dim3(1); lc.blockDim = dim3(kSelThreads); lc.dynamicSmemBytes = 0; lc.stream = ctx->stream;
+  lc.gridDim = dim3((unsigned)((ctx->P + kSelChunk - 1) / kSelChunk));   // <= kSelMaxCtas, checked in epo_set_pairs
+  lc.blockDim = dim3(kSelThreads); lc.dynamicSmemBytes = 0; lc.stream = ctx->stream;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = (ctx->pdl && gated) ? 1 : 0;
@@ -323,3 +379,5 @@ epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override, bool gated, 
   ctx->launches += 1;
   return EPO_OK;
 }
+
+int64_t epo_select_max_pairs(void) { return (int64_t)kSelMaxCtas * kSelChunk; }
