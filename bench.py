@@ -41,6 +41,9 @@ def parse():
     ap.add_argument("--views", type=int, default=None, help="shrink the config (debugging only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--refine-iters", type=int, default=200)
+    ap.add_argument("--pair-budget", type=int, default=0,
+                    help="M of the stochastic viewgraph sub-sampling (PAPER.md:500); 0 = all pairs every step, the "
+                         "workload BASELINE.json's metric is quoted on")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--plumbing-test", action="store_true",
@@ -245,7 +248,7 @@ def main():
     sc = make_scene(args.config, n_views=args.views)
     stream = torch.cuda.current_stream()
     cfg = epo_config_default(n_views=sc.n_views, width=sc.W, height=sc.H, early_stop=0, device=local,
-                             stream=stream.cuda_stream)
+                             stream=stream.cuda_stream, pair_budget=args.pair_budget, subsample_seed=2607)
     e = Epo(cfg)
     # inputs resident in HBM before the timed region
     dK, dP, dD, dE = (torch.from_numpy(a).cuda() for a in (sc.K, sc.poses_init, sc.depth, sc.edges))
@@ -301,6 +304,18 @@ def main():
     refine_s = a.elapsed_time(b) / 1e3
     total_ms = max_over_ranks(total_ms, world, "cuda")
     value = whole_job_value(world, reproj, args.steps, total_ms)
+    sub = None; reproj_eff = reproj
+    if args.pair_budget > 0 and len(sc.pairs) > args.pair_budget:
+        # stochastic pair sub-sampling: a step evaluates M drawn pairs; count exactly what the timed steps evaluated
+        # (they were steps 0 .. K-1 after the reset) and quote the rate on that
+        n_src = np.diff(edge_off)[sc.pairs[:, 0]].astype(np.int64)
+        per_step = [int(n_src[e.get_pair_subset(k)].sum()) for k in range(args.steps)]
+        value = world * sum(per_step) / (total_ms / 1e3)
+        reproj_eff = int(round(sum(per_step) / len(per_step)))
+        sub = dict(pair_budget=args.pair_budget, pairs=len(sc.pairs), reprojections_per_timed_step=per_step[:4],
+                   full_list_equivalent=whole_job_value(world, reproj, args.steps, total_ms),
+                   note="value counts the reprojections of the drawn subsets only (warm_l2 and e2e use the mean of the "
+                        "timed steps' subsets); the roofline line is the kernel hook on the FULL pair list")
 
     # e2e through the C ABI with pinned HOST buffers (H2D + preprocessing + pairs + iterations + D2H)
     e2e = None
@@ -319,7 +334,7 @@ def main():
             e2.destroy()
         t_e2e = min(times[1:]) if len(times) > 1 else times[0]
         h2d = sum(int(x.numel() * x.element_size()) for x in (hK, hP, hD, hE, hpairs))
-        e2e = dict(value=world * reproj * args.refine_iters / t_e2e, unit=UNIT, h2d_bytes_per_step=h2d,
+        e2e = dict(value=world * reproj_eff * args.refine_iters / t_e2e, unit=UNIT, h2d_bytes_per_step=h2d,
                    d2h_bytes_per_step=int(hout.numel() * 4) + 8, seconds=t_e2e,
                    what=f"epo_create + epo_set_views(host) + epo_set_pairs(host) + epo_step({args.refine_iters}) + epo_get_poses(host)")
 
@@ -340,10 +355,12 @@ def main():
                       kernel="k_loss_grad<u8>", kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
                       algorithmic_bytes=alg_bytes, peak_source=peak_src,
                       note="algorithmic bytes = 8 B x attempted + 16 B x valid reprojections (DESIGN.md)"),
-        warm_l2=dict(ms_per_step=warm_ms, value=world * reproj / (warm_ms / 1e3)),
+        warm_l2=dict(ms_per_step=warm_ms, value=world * reproj_eff / (warm_ms / 1e3)),
         refinement=dict(iters=int(done), seconds=refine_s, views=sc.n_views),
         preprocessing=dict(set_views_s=t_views, set_pairs_s=t_pairs),
     )
+    if sub:
+        line["config"]["subsampling"] = sub
     if e2e:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

@@ -345,6 +345,29 @@ def test_pair_subset_bit_exact(n_views, budget, seed):
     off.destroy()
 
 
+def test_pair_subset_bit_exact_across_ctas():
+    """9000 pairs (the tiny scene's 12, repeated: duplicates are legal and weigh as often as they occur) span three
+    CTAs of the selection kernel with a ragged last one; a list beyond its capacity is refused, not mis-drawn."""
+    import paper_2607_00579_b200 as pkg
+    sc = scene("tiny")
+    from paper_2607_00579_b200 import Epo, epo_config_default
+    import torch
+    cfg = epo_config_default(n_views=sc.n_views, width=sc.W, height=sc.H, pair_budget=1024, subsample_seed=11,
+                             stream=torch.cuda.current_stream().cuda_stream)
+    e = Epo(cfg)
+    e.set_views(sc.K, sc.poses_init, sc.depth, sc.edges)
+    pairs = np.ascontiguousarray(np.tile(sc.pairs, (750, 1)))
+    e.set_pairs(pairs)
+    for step in (0, 3, 1234):
+        got = e.get_pair_subset(step)
+        assert got.sum() == 1024 and np.array_equal(got, oracle.pair_subset(11, step, len(pairs), 1024)), step
+    assert e.step(3) == (3, 0)                                    # the loop runs on the drawn subsets
+    big = np.ascontiguousarray(np.tile(sc.pairs, (43700, 1)))     # 524,400 pairs > 128 x 4096
+    assert pkg.lib().epo_set_pairs(e._h, big.ctypes.data, len(big)) == pkg.EPO_ERR_UNSUPPORTED
+    assert e.get_pair_subset(0).sum() == 1024                     # the context is unchanged
+    e.destroy()
+
+
 def test_subsampled_iterations_match_the_oracle():
     """epo_step with a pair budget: every iteration's loss, update and theta95 against the oracle evaluated on the
     oracle's own draw of that step (mean over the M drawn pairs)."""
