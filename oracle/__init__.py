@@ -109,6 +109,11 @@ def lib():
                               C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
                               C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                               C.POINTER(C.c_double)]
+        L.orc_viewgraph_counts.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
+                                           C.POINTER(C.c_float), C.c_int, C.c_double, C.c_double, C.c_int,
+                                           C.POINTER(C.c_int32)]
+        L.orc_viewgraph_pairs.restype = C.c_int64
+        L.orc_viewgraph_pairs.argtypes = [C.c_int, C.POINTER(C.c_int32), C.c_double, C.POINTER(C.c_int32)]
         L.orc_subset_key.restype = C.c_uint64
         L.orc_subset_key.argtypes = [C.c_uint64, C.c_int, C.c_int64]
         L.orc_pair_subset.restype = C.c_int64
@@ -271,6 +276,26 @@ def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair
 
 
 # ---------------------------------------------------------------------------------------------- O7
+def viewgraph_counts(K, poses, depth, stride=8, tau=3.0, z_min=1e-6, coord_fp32=0) -> np.ndarray:
+    """[N][N][2] = (consistent, usable) grid points of the cycle i -> j -> i."""
+    K = np.ascontiguousarray(K, np.float32); poses = np.ascontiguousarray(poses, np.float64).reshape(-1, 12)
+    depth = np.ascontiguousarray(depth, np.float32)
+    N, H, W = depth.shape
+    counts = np.zeros((N, N, 2), np.int32)
+    lib().orc_viewgraph_counts(N, W, H, _p(K, C.c_float), _p(poses, C.c_double), _p(depth, C.c_float), int(stride),
+                               C.c_double(tau), C.c_double(z_min), int(coord_fp32), _p(counts, C.c_int32))
+    return counts
+
+
+def viewgraph_pairs(counts: np.ndarray, min_frac=0.125) -> np.ndarray:
+    """Directed pair list [(i, j), (j, i) for valid i < j] from the cycle counts."""
+    counts = np.ascontiguousarray(counts, np.int32); N = counts.shape[0]
+    n = lib().orc_viewgraph_pairs(N, _p(counts, C.c_int32), C.c_double(min_frac), None)
+    pairs = np.zeros((max(n, 1), 2), np.int32)
+    lib().orc_viewgraph_pairs(N, _p(counts, C.c_int32), C.c_double(min_frac), _p(pairs, C.c_int32))
+    return pairs[:n]
+
+
 def subset_key(seed: int, step: int, p: int) -> int:
     """key(step, p) of the stochastic pair sub-sampling: a SplitMix64 output, see epo_oracle.c."""
     return int(lib().orc_subset_key(C.c_uint64(seed & 0xFFFFFFFFFFFFFFFF), int(step), C.c_int64(p)))

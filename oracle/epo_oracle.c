@@ -410,6 +410,127 @@ void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, con
  * O7  Schedules, Adam, SE(3) exponential  (readings S4, S10, S11)
  * ================================================================================================= */
 /* clamp lambda: clamp_start -> clamp_end linearly over the first clamp_steps steps */
+/* =================================================================================================
+ * Viewgraph estimation by exhaustive cycle-consistent reprojection (Eq. 2; 117; 380-384; 396).
+ * "we project each pixel p of image I_i onto I_j using pi (Eq. 2) ... The resulting p_{i->j} is then projected back
+ * onto I_i to obtain p_{i->j->i}.  An image pair is called valid if sufficiently many pixels satisfy a bidirectional
+ * reprojection error || p - p_{i->j->i} ||_2 < tau" -- "at least 12.5% of their reprojected 2D points ... below
+ * tau = 3.0 pixels"; "for every one of the C(N,2) candidate pairs a kernel projects a grid of source
+ * pixels into the target view and back".
+ *
+ * orc_viewgraph_counts: for every ORDERED pair (i, j), i != j, counts[(i N + j) 2 + {0,1}] = {consistent, usable}:
+ *   grid   p = (u, v), u = stride/2 + a stride < W, v = stride/2 + b stride < H               (reading V1)
+ *   usable Z_i(p) finite and > z_min                                                          (reading V2)
+ *   p_ij = pi(K_i, K_j, P_i, P_j, Z_i; p): x_j = T_j T_i^-1 K_i^-1 [u,v,1]^T Z_i, needs x_j.z > z_min and
+ *          0 <= x <= W-1, 0 <= y <= H-1                                                       (reading V3)
+ *   Z_j at the pixel nearest to p_ij, (floor(x + 1/2), floor(y + 1/2)); finite and > z_min    (reading V4)
+ *   p_iji = pi(K_j, K_i, P_j, P_i, that depth; p_ij) from the SUB-PIXEL position p_ij; needs z > z_min  (reading V5)
+ *   consistent iff (x' - u)^2 + (y' - v)^2 < tau^2                                            (Eq. text; reading V6)
+ * coord_fp32 = 1 evaluates the positions in IEEE binary32 with one stated operation order (the order of the loss
+ * path, reading P1, both ways) so that the integer decisions (bounds, nearest pixel, threshold) are the
+ * ones an FP32 implementation takes; coord_fp32 = 0 is everything in double.
+ * ================================================================================================= */
+static int orc_cycle_f64(int W, int H, const double Ki[4], const double Kj[4], const double Tji[12], const double Tij[12],
+                         const float* Zj_map, double u, double v, double Zi, double z_min, double tau) {
+  double xs[3], xt[3], px[2], back[3], xi[3], q[2];
+  orc_backproject_cam(Ki, u, v, Zi, xs);
+  for (int r = 0; r < 3; ++r) xt[r] = Tji[4 * r] * xs[0] + Tji[4 * r + 1] * xs[1] + Tji[4 * r + 2] * xs[2] + Tji[4 * r + 3];
+  if (!(xt[2] > z_min)) return 0;
+  orc_project_px(Kj, xt, px);
+  if (!(px[0] >= 0.0 && px[0] <= (double)(W - 1) && px[1] >= 0.0 && px[1] <= (double)(H - 1))) return 0;
+  const int xn = (int)floor(px[0] + 0.5), yn = (int)floor(px[1] + 0.5);
+  const double Zj = (double)Zj_map[(size_t)yn * W + xn];
+  if (!(isfinite(Zj) && Zj > z_min)) return 0;
+  orc_backproject_cam(Kj, px[0], px[1], Zj, back);
+  for (int r = 0; r < 3; ++r) xi[r] = Tij[4 * r] * back[0] + Tij[4 * r + 1] * back[1] + Tij[4 * r + 2] * back[2] + Tij[4 * r + 3];
+  if (!(xi[2] > z_min)) return 0;
+  orc_project_px(Ki, xi, q);
+  const double dx = q[0] - u, dy = q[1] - v;
+  return dx * dx + dy * dy < tau * tau;
+}
+
+/* binary32 positions, operation order:  ifx = 1/fx;  x_s = Z ((u - cx) ifx), y_s likewise, z_s = Z;
+ * X = fma(r00, x_s, fma(r01, y_s, fma(r02, z_s, t_x))) (Y, Z likewise);  iz = 1/Z;  x = fma(fx' X, iz, cx');
+ * nearest pixel floor(x + 0.5f);  error e2 = fma(dx, dx, dy dy) against tau*tau (one rounded product).          */
+static int orc_cycle_f32(int W, int H, const double Ki[4], const double Kj[4], const double Tji[12], const double Tij[12],
+                         const float* Zj_map, float u, float v, float Zi, double z_min, double tau) {
+  float A[12], B[12];
+  for (int k = 0; k < 12; ++k) { A[k] = (float)Tji[k]; B[k] = (float)Tij[k]; }
+  const float fxi = (float)Ki[0], fyi = (float)Ki[1], cxi = (float)Ki[2], cyi = (float)Ki[3];
+  const float fxj = (float)Kj[0], fyj = (float)Kj[1], cxj = (float)Kj[2], cyj = (float)Kj[3];
+  const float zmin = (float)z_min, tauf = (float)tau, tau2 = tauf * tauf;
+  const float ifxi = 1.0f / fxi, ifyi = 1.0f / fyi, ifxj = 1.0f / fxj, ifyj = 1.0f / fyj;
+  const float a_ = (u - cxi) * ifxi, b_ = (v - cyi) * ifyi;
+  const float xs = Zi * a_, ys = Zi * b_, zs = Zi;
+  const float X = fmaf(A[0], xs, fmaf(A[1], ys, fmaf(A[2], zs, A[3])));
+  const float Y = fmaf(A[4], xs, fmaf(A[5], ys, fmaf(A[6], zs, A[7])));
+  const float Z = fmaf(A[8], xs, fmaf(A[9], ys, fmaf(A[10], zs, A[11])));
+  if (!(Z > zmin)) return 0;
+  const float iz = 1.0f / Z;
+  const float fX = fxj * X, fY = fyj * Y;
+  const float x = fmaf(fX, iz, cxj), y = fmaf(fY, iz, cyj);
+  if (!(x >= 0.0f && x <= (float)(W - 1) && y >= 0.0f && y <= (float)(H - 1))) return 0;
+  const float xh = x + 0.5f, yh = y + 0.5f;
+  const int xn = (int)floorf(xh), yn = (int)floorf(yh);
+  const float Zj = Zj_map[(size_t)yn * W + xn];
+  if (!(isfinite(Zj) && Zj > zmin)) return 0;
+  const float c_ = (x - cxj) * ifxj, d_ = (y - cyj) * ifyj;
+  const float xb = Zj * c_, yb = Zj * d_, zb = Zj;
+  const float X2 = fmaf(B[0], xb, fmaf(B[1], yb, fmaf(B[2], zb, B[3])));
+  const float Y2 = fmaf(B[4], xb, fmaf(B[5], yb, fmaf(B[6], zb, B[7])));
+  const float Z2 = fmaf(B[8], xb, fmaf(B[9], yb, fmaf(B[10], zb, B[11])));
+  if (!(Z2 > zmin)) return 0;
+  const float iz2 = 1.0f / Z2;
+  const float gX = fxi * X2, gY = fyi * Y2;
+  const float x2 = fmaf(gX, iz2, cxi), y2 = fmaf(gY, iz2, cyi);
+  const float dx = x2 - u, dy = y2 - v;
+  const float dy2 = dy * dy;
+  const float e2 = fmaf(dx, dx, dy2);
+  return e2 < tau2;
+}
+
+void orc_viewgraph_counts(int N, int W, int H, const float* K, const double* poses, const float* depth, int stride,
+                          double tau, double z_min, int coord_fp32, int32_t* counts) {
+#pragma omp parallel for schedule(dynamic)
+  for (int ij = 0; ij < N * N; ++ij) {
+    const int i = ij / N, j = ij % N;
+    int32_t cons = 0, usable = 0;
+    if (i != j) {
+      double Ki[4], Kj[4], Tji[12], Tij[12];
+      for (int k = 0; k < 4; ++k) { Ki[k] = K[4 * i + k]; Kj[k] = K[4 * j + k]; }
+      orc_relative_pose(poses + 12 * i, poses + 12 * j, Tji);      /* source i -> target j */
+      orc_relative_pose(poses + 12 * j, poses + 12 * i, Tij);      /* and back */
+      const float* Zi_map = depth + (size_t)i * W * H;
+      const float* Zj_map = depth + (size_t)j * W * H;
+      for (int v = stride / 2; v < H; v += stride)
+        for (int u = stride / 2; u < W; u += stride) {
+          const float Zi = Zi_map[(size_t)v * W + u];
+          if (!(isfinite(Zi) && (double)Zi > z_min)) continue;
+          ++usable;
+          cons += coord_fp32 ? orc_cycle_f32(W, H, Ki, Kj, Tji, Tij, Zj_map, (float)u, (float)v, Zi, z_min, tau)
+                             : orc_cycle_f64(W, H, Ki, Kj, Tji, Tij, Zj_map, (double)u, (double)v, (double)Zi, z_min, tau);
+        }
+    }
+    counts[2 * ij] = cons; counts[2 * ij + 1] = usable;
+  }
+}
+
+/* The viewgraph: unordered pair {i, j} is valid iff BOTH directions keep at least min_frac of their usable grid points
+ * (reading V7: the loss uses both directions of a pair, Alg. 3 l.10); output = directed pairs (i, j), (j, i) for
+ * i < j ascending.  Returns the number of directed pairs; pairs may be NULL to count only.                         */
+int64_t orc_viewgraph_pairs(int N, const int32_t* counts, double min_frac, int32_t* pairs) {
+  int64_t n = 0;
+  for (int i = 0; i < N; ++i)
+    for (int j = i + 1; j < N; ++j) {
+      const int32_t *a = counts + 2 * ((size_t)i * N + j), *b = counts + 2 * ((size_t)j * N + i);
+      const int ok = a[1] > 0 && b[1] > 0 && (double)a[0] >= min_frac * (double)a[1] && (double)b[0] >= min_frac * (double)b[1];
+      if (!ok) continue;
+      if (pairs) { pairs[2 * n] = i; pairs[2 * n + 1] = j; pairs[2 * n + 2] = j; pairs[2 * n + 3] = i; }
+      n += 2;
+    }
+  return n;
+}
+
 /* ---------------------------------------------------------------------------------------------------------
  * Stochastic viewgraph sub-sampling (Alg. 3 l.3-6; PAPER.md:500 A1.3): "at each iteration we
  * evaluate the loss on a fresh uniform random subset S of E of size min(|E|, M)".
