@@ -106,6 +106,24 @@ EPO_API epo_status epo_set_views(epo_ctx* ctx, const float* K, const float* pose
                          const uint8_t* edges);
 
 /*
+ * Viewgraph estimation by exhaustive cycle-consistent reprojection (Eq. 2, 117, 380-384, 396) from the
+ * CURRENT poses, the intrinsics and the depth maps given to epo_set_views.  For every ordered pair (i, j) the grid of
+ * source pixels u = stride/2 + a stride, v = stride/2 + b stride with a usable depth (finite, > z_min) is projected
+ * into view j (must land in front of it and inside the image), lifted there with view j's depth at the nearest
+ * pixel, and projected back; a point is consistent if its round trip ends less than tau pixels from where it
+ * started.  The unordered pair {i, j} is valid if in BOTH directions at least min_frac of the usable points are
+ * consistent (paper: tau = 3.0, min_frac = 0.125; the grid stride is not stated, 8 is this library's default).
+ *   pairs     [capacity][2] out (nullable when capacity = 0): directed pairs (i, j), (j, i) for valid i < j, ascending;
+ *             ready for epo_set_pairs.  Host or device pointer.
+ *   n_pairs   out (host): number of directed pairs found; if it exceeds capacity the call fails with
+ *             EPO_ERR_INVALID_ARG after setting it, and writes no pairs.
+ *   counts    [N][N][2] out, nullable: (consistent, usable) of the cycle i -> j -> i (0, 0 on the diagonal).
+ * Synchronises the stream.  Does not change the context (call epo_set_pairs with the result).
+ */
+EPO_API epo_status epo_build_viewgraph(epo_ctx* ctx, int32_t grid_stride, float tau, float min_frac, int32_t* pairs,
+                                       int64_t capacity, int64_t* n_pairs, int32_t* counts);
+
+/*
  * Set the viewgraph as a list of DIRECTED pairs [P][2] = (source, target), P >= 1,
  * indices in [0, N), source != target; duplicates are kept (they weigh twice).  Builds the canonical
  * order (ascending (target, source), stable), the per-target and per-source incidence lists and the

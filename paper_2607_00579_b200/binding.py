@@ -21,7 +21,7 @@ _STATUS = {0: "EPO_OK", 1: "EPO_ERR_INVALID_ARG", 2: "EPO_ERR_BAD_STATE", 3: "EP
            4: "EPO_ERR_CUDA", 5: "EPO_ERR_UNSUPPORTED"}
 
 # every symbol include/epo.h declares (tests check that the library exports exactly these)
-SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_set_views", "epo_set_pairs", "epo_loss_grad",
+SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad",
            "epo_step", "epo_get_poses", "epo_get_poses_f64", "epo_reset", "epo_get_edge_counts", "epo_get_edge_list",
            "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel",
            "epo_last_error", "epo_version"]
@@ -55,6 +55,7 @@ def load_library() -> C.CDLL:
     L.epo_destroy.argtypes = [vp]; L.epo_destroy.restype = None
     L.epo_set_views.argtypes = [vp, f32p, f32p, f32p, vp]
     L.epo_set_pairs.argtypes = [vp, i32p, C.c_int64]
+    L.epo_build_viewgraph.argtypes = [vp, C.c_int32, C.c_float, C.c_float, i32p, C.c_int64, C.POINTER(C.c_int64), i32p]
     L.epo_loss_grad.argtypes = [vp, C.c_float, f32p, f32p, i32p, f32p]
     L.epo_step.argtypes = [vp, C.c_int32, i32p, i32p]
     L.epo_get_poses.argtypes = [vp, f32p]
@@ -140,6 +141,17 @@ class Epo:
         self._check(lib().epo_set_views(self._h, _ptr(K, np.float32), _ptr(poses, np.float32),
                                         _ptr(depth, np.float32), _ptr(edges, np.uint8)), "epo_set_views")
         self.P = 0
+
+    def build_viewgraph(self, stride: int = 8, tau: float = 3.0, min_frac: float = 0.125, want_counts: bool = False):
+        """Directed pair list [P][2] (int32) of the cycle-consistent viewgraph at the current poses (+ counts [N][N][2])."""
+        n = C.c_int64(0)
+        cap = self.N * (self.N - 1)
+        pairs = np.zeros((max(cap, 1), 2), np.int32)
+        counts = np.zeros((self.N, self.N, 2), np.int32) if want_counts else None
+        self._check(lib().epo_build_viewgraph(self._h, int(stride), C.c_float(tau), C.c_float(min_frac), _ptr(pairs), cap,
+                                              C.byref(n), _ptr(counts)), "epo_build_viewgraph")
+        pairs = np.ascontiguousarray(pairs[: n.value])
+        return (pairs, counts) if want_counts else pairs
 
     def set_pairs(self, pairs):
         n = int(pairs.shape[0])

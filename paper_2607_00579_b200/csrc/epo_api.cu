@@ -58,7 +58,8 @@ cudaError_t copy_out(void* dst, const void* src, size_t bytes, cudaStream_t st, 
 }
 
 void free_views(epo_ctx* c) {
-  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_pts);
+  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_pts); cudaFree(c->d_depth);
+  c->d_depth = nullptr;
   epo_free_atlas(&c->atlas);
   c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_pts = nullptr;
   c->have_views = false;
@@ -246,8 +247,9 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   if (rc == EPO_OK && e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
   tr.mark("points + drain");
   epo_free_dtf_scratch(&scratch);
-  cudaFree(d_depth); cudaFree(d_e); cudaFree(d_small);
+  cudaFree(d_e); cudaFree(d_small);
   if (rc != EPO_OK) {
+    cudaFree(d_depth);
     // d_K / d_poses may have been overwritten only if every build step succeeded and the final drain failed
     // (a sticky CUDA error: the context is unusable anyway)
     cudaGetLastError();
@@ -256,7 +258,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   }
   free_pairs(c); free_views(c);
   c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff;
-  c->d_pts = pts; c->atlas = atlas;
+  c->d_pts = pts; c->atlas = atlas; c->d_depth = d_depth;
   c->have_views = true; c->static_dirty = true;
   tr.mark("free temporaries");
   return EPO_OK;
@@ -545,6 +547,45 @@ epo_status epo_get_trace(epo_ctx* c, int32_t first, int32_t count, float* loss, 
   }
   if (sync) EPO_CUDA(c, cudaStreamSynchronize(st));
   return EPO_OK;
+}
+
+epo_status epo_build_viewgraph(epo_ctx* c, int32_t grid_stride, float tau, float min_frac, int32_t* pairs, int64_t capacity,
+                               int64_t* n_pairs, int32_t* counts) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_build_viewgraph before epo_set_views");
+  if (!n_pairs || grid_stride < 1 || !(tau > 0.f) || !(min_frac >= 0.f && min_frac <= 1.f) || capacity < 0 || (capacity > 0 && !pairs))
+    return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_build_viewgraph: bad argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t N = (size_t)c->N;
+  int2 *d_counts = nullptr, *d_pairs = nullptr; long long* d_n = nullptr;
+  cudaError_t e = cudaMalloc(&d_counts, N * N * sizeof(int2));
+  if (e == cudaSuccess) e = cudaMalloc(&d_pairs, (N * (N - 1) + 1) * sizeof(int2));
+  if (e == cudaSuccess) e = cudaMalloc(&d_n, sizeof(long long));
+  epo_status rc = e == cudaSuccess ? epo_launch_viewgraph(c, grid_stride, tau, min_frac, d_counts, d_pairs, d_n)
+                                   : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
+                                              "epo_build_viewgraph: %s", cudaGetErrorString(e));
+  long long n = 0;
+  if (rc == EPO_OK) {
+    e = cudaMemcpyAsync(&n, d_n, sizeof(long long), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_build_viewgraph: %s", cudaGetErrorString(e));
+  }
+  if (rc == EPO_OK) {
+    *n_pairs = n;
+    if (pairs && n > capacity) rc = epo_fail(c, EPO_ERR_INVALID_ARG, "epo_build_viewgraph: %lld pairs do not fit a capacity of %lld", n, (long long)capacity);
+  }
+  if (rc == EPO_OK && pairs && n > 0) {
+    e = cudaMemcpyAsync(pairs, d_pairs, (size_t)n * sizeof(int2), cudaMemcpyDefault, st);
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_build_viewgraph: %s", cudaGetErrorString(e));
+  }
+  if (rc == EPO_OK && counts) {
+    e = cudaMemcpyAsync(counts, d_counts, N * N * sizeof(int2), cudaMemcpyDefault, st);
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_build_viewgraph: %s", cudaGetErrorString(e));
+  }
+  cudaStreamSynchronize(st);
+  cudaFree(d_counts); cudaFree(d_pairs); cudaFree(d_n);
+  return rc;
 }
 
 epo_status epo_get_pair_subset(epo_ctx* c, int32_t step, uint8_t* flags) {

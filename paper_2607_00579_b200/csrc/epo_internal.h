@@ -86,6 +86,7 @@ struct epo_ctx {
   double* d_poses_init;   // [N][12] as given to epo_set_views / epo_reset
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
+  float* d_depth;         // [N][H][W] the depth maps as given (kept for epo_build_viewgraph)
   float4* d_pts;          // [E] camera-frame points (x_s, y_s, z_s, 0): K and Z are fixed, so row a-2 is hoisted
   EpoAtlas atlas;         // the distance fields as the fused kernel samples them (see EpoAtlas)
   std::vector<int32_t> h_edge_off;
@@ -187,6 +188,9 @@ constexpr int kSelScrBarrier = 0, kSelScrNCand = 2, kSelScrHist = 4, kSelScrTota
               kSelScrInts = kSelScrCandIdx + kSelCandCap;
 int64_t epo_select_max_pairs(void);
 epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override /* < 0: device step */, bool gated, bool build_work);
+// viewgraph.cu: cycle counts of all ordered pairs + ordered emission of the valid pairs
+epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_frac, int2* d_counts, int2* d_pairs,
+                                long long* d_n);
 // lossgrad.cu
 epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)

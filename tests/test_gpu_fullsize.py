@@ -143,3 +143,20 @@ def test_full_size_config4_stochastic_pair_subsampling():
         assert abs(float(loss[0]) - ref["loss"]) <= 1e-5 * abs(ref["loss"]), (k, float(loss[0]), ref["loss"])
         P = new
     e.destroy()
+
+
+def test_full_size_config3_viewgraph():
+    """Config 3's 100 views: all 9,900 ordered cycles (31.5 M grid points at stride 8) bit-exact against the oracle."""
+    import time
+    sc, e, prob = _full(3)
+    e.build_viewgraph()                                            # warm-up (allocations)
+    t0 = time.perf_counter(); pairs, counts = e.build_viewgraph(stride=8, tau=3.0, min_frac=0.125, want_counts=True)
+    t_gpu = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    ref = oracle.viewgraph_counts(sc.K, sc.poses_init.astype(np.float64), sc.depth, stride=8, tau=3.0, z_min=Z_MIN, coord_fp32=1)
+    t_cpu = time.perf_counter() - t0
+    assert np.array_equal(counts, ref)
+    assert np.array_equal(pairs, oracle.viewgraph_pairs(ref, 0.125))
+    print(f"config 3 viewgraph: {len(pairs)} directed pairs of 9900; library call {1e3 * t_gpu:.2f} ms (incl. D2H of pairs "
+          f"and counts), oracle {t_cpu:.2f} s on {oracle.num_threads()} threads")
+    e.destroy()

@@ -327,6 +327,43 @@ def test_early_stop_parity():
     e.destroy()
 
 
+# ------------------------------------------------------------------------------ viewgraph estimation
+@pytest.mark.parametrize("name,stride", [("tiny", 4), ("room6", 8), ("orbit8", 8), ("orbit10_dense", 5)])
+def test_viewgraph_counts_and_pairs_bit_exact(name, stride):
+    """epo_build_viewgraph at the initial poses: the (consistent, usable) counts of every
+    ordered pair and the resulting directed pair list equal the oracle's binary32-position variant exactly; against
+    the all-double oracle the counts differ by a handful of borderline grid points at most."""
+    sc = scene(name)
+    e = make_ctx(sc)
+    pairs, counts = e.build_viewgraph(stride=stride, tau=3.0, min_frac=0.125, want_counts=True)
+    poses = sc.poses_init.astype(np.float64)
+    ref32 = oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=3.0, z_min=Z_MIN, coord_fp32=1)
+    ref64 = oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=3.0, z_min=Z_MIN)
+    assert np.array_equal(counts, ref32)
+    assert np.array_equal(pairs, oracle.viewgraph_pairs(ref32, 0.125))
+    assert np.abs(counts - ref64).max() <= 4 and np.array_equal(counts[..., 1], ref64[..., 1])
+    print(f"{name}: {len(pairs)} directed pairs of {sc.n_views * (sc.n_views - 1)}; max count difference to the double oracle "
+          f"{np.abs(counts - ref64).max()}")
+    # other thresholds; a capacity that is too small is reported, not overrun
+    p2 = e.build_viewgraph(stride=stride, tau=1.0, min_frac=0.5)
+    assert np.array_equal(p2, oracle.viewgraph_pairs(
+        oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=1.0, z_min=Z_MIN, coord_fp32=1), 0.5))
+    if len(pairs) > 2:
+        import ctypes as C
+        import paper_2607_00579_b200 as pkg
+        n = C.c_int64(0); small = np.zeros((2, 2), np.int32)
+        st = pkg.lib().epo_build_viewgraph(e._h, stride, C.c_float(3.0), C.c_float(0.125), small.ctypes.data, 2, C.byref(n), None)
+        assert st == pkg.EPO_ERR_INVALID_ARG and n.value == len(pairs) and not small.any()
+    # the list goes straight into epo_set_pairs
+    if len(pairs):
+        e.set_pairs(pairs)
+        got = e.loss_grad(10.0)
+        prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
+        ref = oracle.loss_grad(prob, poses, pairs, 10.0, z_min=Z_MIN, coord_fp32=1)
+        assert abs(got["loss"] - ref["loss"]) <= 1e-5 * abs(ref["loss"])
+    e.destroy()
+
+
 # ------------------------------------------------------------------- stochastic pair sub-sampling
 @pytest.mark.parametrize("n_views,budget,seed", [(6, 7, 1), (12, 40, 2607), (50, 1024, 5)])
 def test_pair_subset_bit_exact(n_views, budget, seed):
