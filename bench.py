@@ -295,6 +295,7 @@ def main():
     e.reset(); torch.cuda.synchronize()
     k_ms_cold, k_min_cold = e.time_loss_grad_kernel(10.0, args.steps, True)
     k_ms_warm, k_min_warm = e.time_loss_grad_kernel(10.0, args.steps, False)
+    g_ms_cold, _ = e.time_gather_ceiling(10.0, args.steps, True)      # the kernel's memory side alone
     clocks = sampler.stop()
     got = e.loss_grad(10.0)
     n_valid = int(got["pair_valid"].sum())
@@ -354,7 +355,10 @@ def main():
         roofline=dict(bound="hbm", achieved=ach, peak=peak, unit="GB/s", frac=ach / peak, traffic=None,
                       kernel="k_loss_grad<u8>", kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
                       algorithmic_bytes=alg_bytes, peak_source=peak_src,
-                      note="algorithmic bytes = 8 B x attempted + 16 B x valid reprojections (DESIGN.md)"),
+                      note="algorithmic bytes = 8 B x attempted + 16 B x valid reprojections (DESIGN.md)",
+                      gather=dict(ms_cold_l2=g_ms_cold, frac=g_ms_cold / k_ms_cold,
+                                  note="duration of the kernel's memory side alone (points, positions, validity, the "
+                                       "2x2 gather of every valid sample; no loss, no Jacobian) / kernel duration")),
         warm_l2=dict(ms_per_step=warm_ms, value=world * reproj_eff / (warm_ms / 1e3)),
         refinement=dict(iters=int(done), seconds=refine_s, views=sc.n_views),
         preprocessing=dict(set_views_s=t_views, set_pairs_s=t_pairs),

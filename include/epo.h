@@ -182,6 +182,14 @@ EPO_API epo_status epo_get_work(epo_ctx* ctx, int64_t* reprojections_per_eval, i
 EPO_API epo_status epo_time_loss_grad_kernel(epo_ctx* ctx, float lambda, int32_t reps, int32_t flush_l2,
                                              float* ms_mean, float* ms_min);
 
+/* Measurement hook (bench.py "roofline.gather"): the same launches with the fused kernel's MEMORY SIDE only -- the
+ * point stream, the projected positions, validity and the 2x2 gather of every valid sample (the real tap index
+ * stream), the samples merely summed; no robust loss, no Jacobian.  Its duration is the kernel's gather roofline on
+ * this workload (north_star).  It overwrites the per-CTA partial sums; the next evaluation recomputes
+ * them. */
+EPO_API epo_status epo_time_gather_ceiling(epo_ctx* ctx, float lambda, int32_t reps, int32_t flush_l2,
+                                           float* ms_mean, float* ms_min);
+
 EPO_API const char* epo_last_error(const epo_ctx* ctx);
 EPO_API const char* epo_version(void);
 

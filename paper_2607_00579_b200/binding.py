@@ -23,7 +23,7 @@ _STATUS = {0: "EPO_OK", 1: "EPO_ERR_INVALID_ARG", 2: "EPO_ERR_BAD_STATE", 3: "EP
 # every symbol include/epo.h declares (tests check that the library exports exactly these)
 SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad",
            "epo_step", "epo_get_poses", "epo_get_poses_f64", "epo_reset", "epo_get_edge_counts", "epo_get_edge_list",
-           "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel",
+           "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel", "epo_time_gather_ceiling",
            "epo_last_error", "epo_version"]
 
 
@@ -69,6 +69,7 @@ def load_library() -> C.CDLL:
     L.epo_get_pair_subset.argtypes = [vp, C.c_int32, vp]
     L.epo_get_work.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.epo_time_loss_grad_kernel.argtypes = [vp, C.c_float, C.c_int32, C.c_int32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    L.epo_time_gather_ceiling.argtypes = L.epo_time_loss_grad_kernel.argtypes
     L.epo_last_error.argtypes = [vp]; L.epo_last_error.restype = C.c_char_p
     L.epo_version.argtypes = []; L.epo_version.restype = C.c_char_p
     return L
@@ -226,6 +227,13 @@ class Epo:
         a = C.c_float(); b = C.c_float()
         self._check(lib().epo_time_loss_grad_kernel(self._h, C.c_float(lam), reps, int(flush_l2), C.byref(a), C.byref(b)),
                     "epo_time_loss_grad_kernel")
+        return float(a.value), float(b.value)
+
+    def time_gather_ceiling(self, lam: float, reps: int, flush_l2: bool):
+        """(mean ms, min ms) of the fused kernel's memory side alone (its gather roofline on this workload)."""
+        a = C.c_float(); b = C.c_float()
+        self._check(lib().epo_time_gather_ceiling(self._h, C.c_float(lam), reps, int(flush_l2), C.byref(a), C.byref(b)),
+                    "epo_time_gather_ceiling")
         return float(a.value), float(b.value)
 
     def get_pair_subset(self, step: int):

@@ -609,8 +609,21 @@ epo_status epo_get_pair_subset(epo_ctx* c, int32_t step, uint8_t* flags) {
   return EPO_OK;
 }
 
+static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flush_l2, float* ms_mean, float* ms_min,
+                             bool gather_only);
+
 epo_status epo_time_loss_grad_kernel(epo_ctx* c, float lambda, int32_t reps, int32_t flush_l2, float* ms_mean,
                                      float* ms_min) {
+  return time_fused(c, lambda, reps, flush_l2, ms_mean, ms_min, false);
+}
+
+epo_status epo_time_gather_ceiling(epo_ctx* c, float lambda, int32_t reps, int32_t flush_l2, float* ms_mean,
+                                   float* ms_min) {
+  return time_fused(c, lambda, reps, flush_l2, ms_mean, ms_min, true);
+}
+
+static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flush_l2, float* ms_mean, float* ms_min,
+                             bool gather_only) {
   if (!c) return EPO_ERR_INVALID_ARG;
   if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_time_loss_grad_kernel before set_views/set_pairs");
   if (reps < 1 || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_time_loss_grad_kernel: bad argument");
@@ -627,7 +640,7 @@ epo_status epo_time_loss_grad_kernel(epo_ctx* c, float lambda, int32_t reps, int
   for (int r = 0; r < reps && e == cudaSuccess && rc == EPO_OK; ++r) {
     if (flush) e = cudaMemsetAsync(flush, r & 0xff, flush_bytes, st);
     if (e == cudaSuccess) e = cudaEventRecord(e0, st);
-    if (e == cudaSuccess) rc = epo_launch_fused_only(c, lambda);
+    if (e == cudaSuccess) rc = epo_launch_fused_only(c, lambda, gather_only);
     if (e == cudaSuccess) e = cudaEventRecord(e1, st);
     if (e == cudaSuccess) e = cudaEventSynchronize(e1);
     float ms = 0.f;

@@ -193,7 +193,7 @@ epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_f
                                 long long* d_n);
 // lossgrad.cu
 epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);
-epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)
+epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda, bool gather_only);   // the fused kernel alone (measurement hooks)
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
 epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset);
 epo_status epo_launch_fill_schedule(epo_ctx* ctx);     // d_sched from the configuration (once, in epo_create)

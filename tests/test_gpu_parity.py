@@ -421,6 +421,21 @@ def test_subsampled_iterations_match_the_oracle():
     a.destroy(); b.destroy()
 
 
+def test_measurement_hooks_leave_results_unchanged():
+    """epo_time_loss_grad_kernel / epo_time_gather_ceiling overwrite the per-CTA partial sums only: the next
+    evaluation and the loop are unaffected, and the memory side alone is not slower than the whole kernel."""
+    sc = scene("room6")
+    e = make_ctx(sc, early_stop=0)
+    before = e.loss_grad(10.0)
+    full = e.time_loss_grad_kernel(10.0, 5, False)
+    gat = e.time_gather_ceiling(10.0, 5, False)
+    assert 0.0 < gat[1] <= full[1] * 1.15
+    after = e.loss_grad(10.0)
+    assert after["loss"] == before["loss"] and np.array_equal(after["grad"], before["grad"])
+    assert e.step(3) == (3, 0)
+    e.destroy()
+
+
 def test_step_in_pieces_equals_one_call():
     sc = scene("tiny")
     a = make_ctx(sc, early_stop=0); b = make_ctx(sc, early_stop=0)
