@@ -58,16 +58,16 @@ cudaError_t copy_out(void* dst, const void* src, size_t bytes, cudaStream_t st, 
 }
 
 void free_views(epo_ctx* c) {
-  cudaFree(c->d_edge_off); cudaFree(c->d_edges); cudaFree(c->d_pts); cudaFree(c->d_depth);
+  epo_dfree(c, c->d_edge_off); epo_dfree(c, c->d_edges); epo_dfree(c, c->d_pts); epo_dfree(c, c->d_depth);
   c->d_depth = nullptr;
   epo_free_atlas(&c->atlas);
   c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_pts = nullptr;
   c->have_views = false;
 }
 void free_pairs(epo_ctx* c) {
-  cudaFree(c->d_pairs); cudaFree(c->d_perm); cudaFree(c->d_tgt_off); cudaFree(c->d_src_off); cudaFree(c->d_src_inc);
-  cudaFree(c->d_work); cudaFree(c->d_work_off); cudaFree(c->d_part); cudaFree(c->d_pair_loss); cudaFree(c->d_pair_valid); cudaFree(c->d_out_f);
-  cudaFree(c->d_out_i); cudaFree(c->d_sel_flag); cudaFree(c->d_sel_work); cudaFree(c->d_sel_info); cudaFree(c->d_sel_scratch);
+  epo_dfree(c, c->d_pairs); epo_dfree(c, c->d_perm); epo_dfree(c, c->d_tgt_off); epo_dfree(c, c->d_src_off); epo_dfree(c, c->d_src_inc);
+  epo_dfree(c, c->d_work); epo_dfree(c, c->d_work_off); epo_dfree(c, c->d_part); epo_dfree(c, c->d_pair_loss); epo_dfree(c, c->d_pair_valid); epo_dfree(c, c->d_out_f);
+  epo_dfree(c, c->d_out_i); epo_dfree(c, c->d_sel_flag); epo_dfree(c, c->d_sel_work); epo_dfree(c, c->d_sel_info); epo_dfree(c, c->d_sel_scratch);
   c->d_sel_scratch = nullptr; c->d_sel_flag = nullptr; c->d_sel_work = nullptr; c->d_sel_info = nullptr; c->subsample = false; c->sel_grid = 0;
   c->d_pairs = nullptr; c->d_perm = nullptr; c->d_tgt_off = nullptr; c->d_src_off = nullptr; c->d_src_inc = nullptr;
   c->d_work = nullptr; c->d_work_off = nullptr; c->d_part = nullptr; c->d_pair_loss = nullptr; c->d_pair_valid = nullptr; c->d_out_f = nullptr;
@@ -144,20 +144,30 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
   const size_t N = (size_t)c->N;
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_K, N * 4 * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_poses, N * 12 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_poses_next, N * 12 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_poses_init, N * 12 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_grad, N * 6 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_loss_part, N * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_m, N * 6 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_v, N * 6 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_dR, N * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_dt, N * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_state, sizeof(DevState));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_sched, (size_t)cfg->max_steps * 4 * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_theta, (size_t)cfg->max_steps * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc(&c->d_loss_trace, (size_t)cfg->max_steps * sizeof(double));
+  if (e == cudaSuccess) {
+    // keep freed blocks in the device's default pool instead of returning them to the driver at every sync
+    cudaMemPool_t pool = nullptr;
+    unsigned long long keep = ~0ull;
+    if (cudaDeviceGetDefaultMemPool(&pool, cfg->device) == cudaSuccess) cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    cudaGetLastError();
+    e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_alloc, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming);
+  }
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_K, N * 4 * sizeof(float));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_poses, N * 12 * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_poses_next, N * 12 * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_poses_init, N * 12 * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_grad, N * 6 * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_loss_part, N * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_m, N * 6 * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_v, N * 6 * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_dR, N * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_dt, N * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_state, sizeof(DevState));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_sched, (size_t)cfg->max_steps * 4 * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_theta, (size_t)cfg->max_steps * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_loss_trace, (size_t)cfg->max_steps * sizeof(double));
   if (e != cudaSuccess) {
     epo_status st = (e == cudaErrorMemoryAllocation) ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA;
     cudaGetLastError();
@@ -174,9 +184,13 @@ void epo_destroy(epo_ctx* c) {
   cudaSetDevice(c->cfg.device);
   cudaStreamSynchronize(c->stream);
   free_pairs(c); free_views(c);
-  cudaFree(c->d_K); cudaFree(c->d_poses); cudaFree(c->d_poses_next); cudaFree(c->d_poses_init); cudaFree(c->d_grad); cudaFree(c->d_loss_part);
-  cudaFree(c->d_m); cudaFree(c->d_v); cudaFree(c->d_dR); cudaFree(c->d_dt); cudaFree(c->d_state);
-  cudaFree(c->d_sched); cudaFree(c->d_theta); cudaFree(c->d_loss_trace);
+  epo_dfree(c, c->d_K); epo_dfree(c, c->d_poses); epo_dfree(c, c->d_poses_next); epo_dfree(c, c->d_poses_init); epo_dfree(c, c->d_grad); epo_dfree(c, c->d_loss_part);
+  epo_dfree(c, c->d_m); epo_dfree(c, c->d_v); epo_dfree(c, c->d_dR); epo_dfree(c, c->d_dt); epo_dfree(c, c->d_state);
+  epo_dfree(c, c->d_sched); epo_dfree(c, c->d_theta); epo_dfree(c, c->d_loss_trace);
+  cudaStreamSynchronize(c->stream);                 // the frees are stream-ordered: done before the context goes
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->ev_alloc) cudaEventDestroy(c->ev_alloc);
+  if (c->ev_copied) cudaEventDestroy(c->ev_copied);
   cudaGetLastError();
   delete c;
 }
@@ -209,12 +223,17 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   std::vector<int32_t> hoff;
   bool subsampled = false;
   epo_status rc = EPO_OK;
-  cudaError_t e = cudaMalloc(&d_depth, N * px * sizeof(float));
-  if (e == cudaSuccess) e = cudaMalloc(&d_e, N * px);
-  if (e == cudaSuccess) e = cudaMalloc(&d_small, N * 16 * sizeof(float));   // [K 4N | poses 12N] staging
+  cudaError_t e = epo_dmalloc(c, &d_depth, N * px * sizeof(float));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &d_e, N * px);
+  if (e == cudaSuccess) e = epo_dmalloc(c, &d_small, N * 16 * sizeof(float));   // [K 4N | poses 12N] staging
   tr.mark("alloc inputs");
-  // the edge maps first: the distance transform needs nothing else and runs while the depth maps arrive
-  if (e == cudaSuccess) e = copy_in(d_e, edges, N * px, st);
+  // the depth maps travel on the copy stream while the edge maps arrive and the distance transform runs here
+  bool depth_in_flight = false;
+  if (e == cudaSuccess) e = cudaEventRecord(c->ev_alloc, st);
+  if (e == cudaSuccess) e = copy_in(d_e, edges, N * px, st);      // issued first: the link serves it first
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(c->copy_stream, c->ev_alloc, 0);
+  if (e == cudaSuccess) { e = copy_in(d_depth, depth, N * px * sizeof(float), c->copy_stream); depth_in_flight = true; }
+  if (e == cudaSuccess) e = cudaEventRecord(c->ev_copied, c->copy_stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(d_small, hK.data(), N * 4 * sizeof(float), cudaMemcpyHostToDevice, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(d_small + N * 4, hP.data(), N * 12 * sizeof(float), cudaMemcpyHostToDevice, st);
   if (e != cudaSuccess)
@@ -223,9 +242,10 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   tr.mark("copy edges");
   if (rc == EPO_OK) rc = epo_build_dtf_atlas(c, d_e, &atlas, &scratch);
   tr.mark("distance fields");
-  if (rc == EPO_OK) {
-    e = copy_in(d_depth, depth, N * px * sizeof(float), st);
-    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
+  if (depth_in_flight) {
+    // whatever happened above, this stream goes on (or frees d_depth) only after the copy has landed
+    e = cudaStreamWaitEvent(st, c->ev_copied, 0);
+    if (e != cudaSuccess) { cudaStreamSynchronize(c->copy_stream); if (rc == EPO_OK) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e)); }
   }
   tr.mark("copy depth");
   if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff, &subsampled);
@@ -246,14 +266,14 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   e = cudaStreamSynchronize(st);
   if (rc == EPO_OK && e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
   tr.mark("points + drain");
-  epo_free_dtf_scratch(&scratch);
-  cudaFree(d_e); cudaFree(d_small);
+  epo_free_dtf_scratch(c, &scratch);
+  epo_dfree(c, d_e); epo_dfree(c, d_small);
   if (rc != EPO_OK) {
-    cudaFree(d_depth);
+    epo_dfree(c, d_depth);
     // d_K / d_poses may have been overwritten only if every build step succeeded and the final drain failed
     // (a sticky CUDA error: the context is unusable anyway)
     cudaGetLastError();
-    cudaFree(off); cudaFree(rec); cudaFree(pts); epo_free_atlas(&atlas);
+    epo_dfree(c, off); epo_dfree(c, rec); epo_dfree(c, pts); epo_free_atlas(&atlas);
     return rc;
   }
   free_pairs(c); free_views(c);
@@ -281,27 +301,27 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
     reproj += c->h_edge_off[s + 1] - c->h_edge_off[s];
   }
   int32_t* d_user = nullptr;
-  EPO_CUDA(c, cudaMalloc(&d_user, (size_t)P * 2 * sizeof(int32_t)));
+  EPO_CUDA(c, epo_dmalloc(c, &d_user, (size_t)P * 2 * sizeof(int32_t)));
   cudaError_t e = cudaMemcpyAsync(d_user, hp.data(), (size_t)P * 2 * sizeof(int32_t), cudaMemcpyHostToDevice, st);
   int2* canon = nullptr; int4* work = nullptr; int32_t *perm = nullptr, *toff = nullptr, *soff = nullptr, *sinc = nullptr, *woff = nullptr;
   int64_t n_work = 0;
   const int chunk = choose_chunk(c, hp, P);
   epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &woff, &n_work, chunk)
                                      : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
-  cudaFree(d_user);
+  epo_dfree(c, d_user);
   double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
   uint8_t* sflag = nullptr; int32_t* swork = nullptr; int32_t* sinfo = nullptr; int32_t* sscr = nullptr;
   if (rc == EPO_OK && c->cfg.pair_budget > 0 && P > c->cfg.pair_budget && P > epo_select_max_pairs())
     rc = epo_fail(c, EPO_ERR_UNSUPPORTED, "pair sub-sampling supports at most %lld pairs", (long long)epo_select_max_pairs());
   if (rc == EPO_OK) {
-    e = cudaMalloc(&sscr, (size_t)kSelScrInts * sizeof(int32_t));
+    e = epo_dmalloc(c, &sscr, (size_t)kSelScrInts * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemsetAsync(sscr, 0, (size_t)kSelScrInts * sizeof(int32_t), st);
     if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
   }
   if (rc == EPO_OK) {
-    e = cudaMalloc(&sflag, (size_t)P);
-    if (e == cudaSuccess) e = cudaMalloc(&swork, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int32_t));
-    if (e == cudaSuccess) e = cudaMalloc(&sinfo, 2 * sizeof(int32_t));
+    e = epo_dmalloc(c, &sflag, (size_t)P);
+    if (e == cudaSuccess) e = epo_dmalloc(c, &swork, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = epo_dmalloc(c, &sinfo, 2 * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemsetAsync(sinfo, 0, 2 * sizeof(int32_t), st);
     if (e != cudaSuccess)
       rc = epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_set_pairs: %s",
@@ -310,20 +330,20 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   if (rc == EPO_OK) {
     // output staging: [loss | grad 6N | pair_loss P | loss trace | theta trace]
     size_t nf = 1 + (size_t)c->N * 6 + (size_t)P + (size_t)c->cfg.max_steps * 2;
-    e = cudaMalloc(&acc, (size_t)(n_work > 0 ? n_work : 1) * kAccStride * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&pl, (size_t)P * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc(&pv, (size_t)P * sizeof(int32_t));
-    if (e == cudaSuccess) e = cudaMalloc(&of, nf * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc(&oi, (size_t)P * sizeof(int32_t));
+    e = epo_dmalloc(c, &acc, (size_t)(n_work > 0 ? n_work : 1) * kAccStride * sizeof(double));
+    if (e == cudaSuccess) e = epo_dmalloc(c, &pl, (size_t)P * sizeof(float));
+    if (e == cudaSuccess) e = epo_dmalloc(c, &pv, (size_t)P * sizeof(int32_t));
+    if (e == cudaSuccess) e = epo_dmalloc(c, &of, nf * sizeof(float));
+    if (e == cudaSuccess) e = epo_dmalloc(c, &oi, (size_t)P * sizeof(int32_t));
     if (e != cudaSuccess)
       rc = epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_set_pairs: %s",
                     cudaGetErrorString(e));
   }
   if (rc != EPO_OK) {
     cudaGetLastError();
-    cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(toff); cudaFree(soff); cudaFree(sinc); cudaFree(woff);
-    cudaFree(acc); cudaFree(pl); cudaFree(pv); cudaFree(of); cudaFree(oi);
-    cudaFree(sflag); cudaFree(swork); cudaFree(sinfo); cudaFree(sscr);
+    epo_dfree(c, canon); epo_dfree(c, work); epo_dfree(c, perm); epo_dfree(c, toff); epo_dfree(c, soff); epo_dfree(c, sinc); epo_dfree(c, woff);
+    epo_dfree(c, acc); epo_dfree(c, pl); epo_dfree(c, pv); epo_dfree(c, of); epo_dfree(c, oi);
+    epo_dfree(c, sflag); epo_dfree(c, swork); epo_dfree(c, sinfo); epo_dfree(c, sscr);
     return rc;
   }
   free_pairs(c);
@@ -427,12 +447,12 @@ epo_status epo_get_poses(epo_ctx* c, float* poses) {
     return EPO_OK;
   }
   float* tmp = nullptr;
-  EPO_CUDA(c, cudaMalloc(&tmp, (size_t)n * sizeof(float)));
+  EPO_CUDA(c, epo_dmalloc(c, &tmp, (size_t)n * sizeof(float)));
   epo_launch_f64_to_f32(st, c->d_poses, tmp, n);
   c->launches += 1;
   cudaError_t e = cudaMemcpyAsync(poses, tmp, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(tmp);
+  epo_dfree(c, tmp);
   if (e != cudaSuccess) return epo_fail(c, EPO_ERR_CUDA, "epo_get_poses: %s", cudaGetErrorString(e));
   return EPO_OK;
 }
@@ -450,10 +470,10 @@ epo_status epo_reset(epo_ctx* c, const float* poses) {
     for (size_t k = 0; k < n; ++k)
       if (!std::isfinite(hP[k])) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_reset: non-finite pose");
     float* tmp = nullptr;
-    EPO_CUDA(c, cudaMalloc(&tmp, n * sizeof(float)));
+    EPO_CUDA(c, epo_dmalloc(c, &tmp, n * sizeof(float)));
     cudaError_t e = cudaMemcpyAsync(tmp, hP.data(), n * sizeof(float), cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) { epo_launch_f32_to_f64(st, tmp, c->d_poses_init, (int64_t)n); c->launches += 1; e = cudaStreamSynchronize(st); }
-    cudaFree(tmp);
+    epo_dfree(c, tmp);
     if (e != cudaSuccess) return epo_fail(c, EPO_ERR_CUDA, "epo_reset: %s", cudaGetErrorString(e));
   }
   EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, n * sizeof(double), cudaMemcpyDeviceToDevice, st));
@@ -559,9 +579,9 @@ epo_status epo_build_viewgraph(epo_ctx* c, int32_t grid_stride, float tau, float
   cudaStream_t st = c->stream;
   const size_t N = (size_t)c->N;
   int2 *d_counts = nullptr, *d_pairs = nullptr; long long* d_n = nullptr;
-  cudaError_t e = cudaMalloc(&d_counts, N * N * sizeof(int2));
-  if (e == cudaSuccess) e = cudaMalloc(&d_pairs, (N * (N - 1) + 1) * sizeof(int2));
-  if (e == cudaSuccess) e = cudaMalloc(&d_n, sizeof(long long));
+  cudaError_t e = epo_dmalloc(c, &d_counts, N * N * sizeof(int2));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &d_pairs, (N * (N - 1) + 1) * sizeof(int2));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &d_n, sizeof(long long));
   epo_status rc = e == cudaSuccess ? epo_launch_viewgraph(c, grid_stride, tau, min_frac, d_counts, d_pairs, d_n)
                                    : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
                                               "epo_build_viewgraph: %s", cudaGetErrorString(e));
@@ -584,7 +604,7 @@ epo_status epo_build_viewgraph(epo_ctx* c, int32_t grid_stride, float tau, float
     if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_build_viewgraph: %s", cudaGetErrorString(e));
   }
   cudaStreamSynchronize(st);
-  cudaFree(d_counts); cudaFree(d_pairs); cudaFree(d_n);
+  epo_dfree(c, d_counts); epo_dfree(c, d_pairs); epo_dfree(c, d_n);
   return rc;
 }
 
@@ -632,7 +652,7 @@ static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flu
   const size_t flush_bytes = (size_t)256 << 20;   // > 126 MB L2
   void* flush = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
-  if (flush_l2) EPO_CUDA(c, cudaMalloc(&flush, flush_bytes));
+  if (flush_l2) EPO_CUDA(c, epo_dmalloc(c, &flush, flush_bytes));
   cudaError_t e = cudaEventCreate(&e0);
   if (e == cudaSuccess) e = cudaEventCreate(&e1);
   double sum = 0.0; float mn = 1e30f;
@@ -648,7 +668,7 @@ static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flu
     sum += ms; if (ms < mn) mn = ms;
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFree(flush);
+  epo_dfree(c, flush);
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
   if (rc != EPO_OK) return rc;

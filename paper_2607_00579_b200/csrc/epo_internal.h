@@ -72,6 +72,8 @@ constexpr float kU8LambdaMax = 14.5f;
 struct epo_ctx {
   epo_config cfg;
   cudaStream_t stream;
+  cudaStream_t copy_stream;   // epo_set_views: the depth maps arrive on it while the distance transform runs on `stream`
+  cudaEvent_t ev_alloc, ev_copied;
   int N, W, H;
   bool have_views, have_pairs;
   bool pdl;            // programmatic dependent launch between the kernels of the loop (EPO_NO_PDL=1 turns it off)
@@ -163,6 +165,17 @@ epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
     if (s_ != EPO_OK) return s_;   \
   } while (0)
 
+// ---- device memory: stream-ordered allocation from the device's default pool on the context's stream.  A free
+// costs no device synchronisation and a later allocation of the same size is served from the pool (epo_create sets
+// the pool's release threshold), which takes ~2.5 ms of cudaMalloc/cudaFree out of an epo_set_views call.
+template <class T>
+inline cudaError_t epo_dmalloc(epo_ctx* ctx, T** p, size_t bytes) {
+  return cudaMallocAsync(reinterpret_cast<void**>(p), bytes ? bytes : 1, ctx->stream);
+}
+inline void epo_dfree(epo_ctx* ctx, void* p) {
+  if (p) cudaFreeAsync(p, ctx->stream);
+}
+
 // ---- kernel launchers (each .cu file owns its kernels) ----------------------------------------
 // preprocess.cu
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
@@ -170,7 +183,7 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
                                 std::vector<int32_t>* h_off, bool* out_subsampled);
 struct EpoDtfScratch { int32_t* g; cudaSurfaceObject_t surf, surf8; };   // alive until the EDT kernels have run
 epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, EpoAtlas* atlas, EpoDtfScratch* scratch);
-void epo_free_dtf_scratch(EpoDtfScratch* s);
+void epo_free_dtf_scratch(epo_ctx* ctx, EpoDtfScratch* s);
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
                             const std::vector<int32_t>& h_off, const uint8_t* d_edges_u8, const float* d_depth,
                             bool subsampled, float4** out_pts);

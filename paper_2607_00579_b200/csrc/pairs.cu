@@ -306,9 +306,9 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
   int32_t *perm = nullptr, *tgt_off = nullptr, *src_off = nullptr, *src_inc = nullptr;
   int32_t *cnt = nullptr, *cursor = nullptr, *bucket = nullptr, *chunk_cnt = nullptr, *work_off = nullptr;
   auto free_all = [&]() {
-    cudaFree(canon); cudaFree(work); cudaFree(perm); cudaFree(tgt_off); cudaFree(src_off); cudaFree(src_inc); cudaFree(work_off);
+    epo_dfree(ctx, canon); epo_dfree(ctx, work); epo_dfree(ctx, perm); epo_dfree(ctx, tgt_off); epo_dfree(ctx, src_off); epo_dfree(ctx, src_inc); epo_dfree(ctx, work_off);
   };
-  auto free_tmp = [&]() { cudaFree(cnt); cudaFree(cursor); cudaFree(bucket); cudaFree(chunk_cnt); };
+  auto free_tmp = [&]() { epo_dfree(ctx, cnt); epo_dfree(ctx, cursor); epo_dfree(ctx, bucket); epo_dfree(ctx, chunk_cnt); };
 #define PR_CUDA(call)                                                                                \
   do {                                                                                               \
     cudaError_t e_ = (call);                                                                         \
@@ -319,16 +319,16 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
       return rc_;                                                                                    \
     }                                                                                                \
   } while (0)
-  PR_CUDA(cudaMalloc(&canon, P * sizeof(int2)));
-  PR_CUDA(cudaMalloc(&perm, P * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&tgt_off, (N + 1) * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&src_off, (N + 1) * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&src_inc, P * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&cnt, (N + 1) * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&cursor, (N + 1) * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&bucket, P * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&chunk_cnt, (P + 1) * sizeof(int32_t)));
-  PR_CUDA(cudaMalloc(&work_off, (P + 1) * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &canon, P * sizeof(int2)));
+  PR_CUDA(epo_dmalloc(ctx, &perm, P * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &tgt_off, (N + 1) * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &src_off, (N + 1) * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &src_inc, P * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &cnt, (N + 1) * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &cursor, (N + 1) * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &bucket, P * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &chunk_cnt, (P + 1) * sizeof(int32_t)));
+  PR_CUDA(epo_dmalloc(ctx, &work_off, (P + 1) * sizeof(int32_t)));
   const int gridP = (int)((P + 255) / 256);
   // by target
   PR_CUDA(cudaMemsetAsync(cnt, 0, (N + 1) * sizeof(int32_t), st));
@@ -351,11 +351,10 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
   int32_t n_work = 0;
   PR_CUDA(cudaMemcpyAsync(&n_work, work_off + P, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   PR_CUDA(cudaStreamSynchronize(st));
-  PR_CUDA(cudaMalloc(&work, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int4)));
+  PR_CUDA(epo_dmalloc(ctx, &work, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int4)));
   k_fill_work<<<gridP, 256, 0, st>>>(work_off, canon, ctx->d_edge_off, P, chunk, work);
   ctx->launches += 1;
   PR_CUDA(cudaGetLastError());
-  PR_CUDA(cudaStreamSynchronize(st));
   free_tmp();
 #undef PR_CUDA
   *out_pairs = canon; *out_perm = perm; *out_tgt_off = tgt_off; *out_src_off = src_off; *out_src_inc = src_inc;

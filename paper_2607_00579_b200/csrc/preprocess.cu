@@ -305,7 +305,7 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
   EdgeRec *full = nullptr, *fin = nullptr;
   epo_status rc = EPO_OK;
   auto cleanup = [&]() {
-    cudaFree(row_cnt); cudaFree(row_off); cudaFree(view_cnt);
+    epo_dfree(ctx, row_cnt); epo_dfree(ctx, row_off); epo_dfree(ctx, view_cnt);
   };
 #define PP_CUDA(call)                                                                                \
   do {                                                                                               \
@@ -313,14 +313,14 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
     if (e_ != cudaSuccess) {                                                                         \
       rc = epo_fail(ctx, e_ == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,     \
                     "%s failed: %s", #call, cudaGetErrorString(e_));                                 \
-      cleanup(); cudaFree(full_off); cudaFree(full); cudaFree(fin_off); cudaFree(fin);               \
+      cleanup(); epo_dfree(ctx, full_off); epo_dfree(ctx, full); epo_dfree(ctx, fin_off); epo_dfree(ctx, fin);               \
       return rc;                                                                                     \
     }                                                                                                \
   } while (0)
-  PP_CUDA(cudaMalloc(&row_cnt, (rows + 1) * sizeof(int32_t)));
-  PP_CUDA(cudaMalloc(&row_off, (rows + 1) * sizeof(int32_t)));
-  PP_CUDA(cudaMalloc(&view_cnt, (N + 1) * sizeof(int32_t)));
-  PP_CUDA(cudaMalloc(&full_off, (N + 1) * sizeof(int32_t)));
+  PP_CUDA(epo_dmalloc(ctx, &row_cnt, (rows + 1) * sizeof(int32_t)));
+  PP_CUDA(epo_dmalloc(ctx, &row_off, (rows + 1) * sizeof(int32_t)));
+  PP_CUDA(epo_dmalloc(ctx, &view_cnt, (N + 1) * sizeof(int32_t)));
+  PP_CUDA(epo_dmalloc(ctx, &full_off, (N + 1) * sizeof(int32_t)));
   const int grid_rows = (int)((rows + kWarpsPerBlock - 1) / kWarpsPerBlock);
   k_row_count<<<grid_rows, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, d_depth, rows, W, ctx->cfg.z_min, row_cnt);
   k_exclusive_scan<<<1, 1024, 0, st>>>(row_cnt, row_off, rows, 0);
@@ -330,7 +330,7 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
   PP_CUDA(cudaMemcpyAsync(hfull.data(), full_off, (N + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   PP_CUDA(cudaStreamSynchronize(st));
   const int64_t Efull = hfull[N];
-  PP_CUDA(cudaMalloc(&full, (size_t)(Efull > 0 ? Efull : 1) * sizeof(EdgeRec)));
+  PP_CUDA(epo_dmalloc(ctx, &full, (size_t)(Efull > 0 ? Efull : 1) * sizeof(EdgeRec)));
   k_row_scatter<<<grid_rows, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, d_depth, rows, W, H, ctx->cfg.z_min, row_off, full);
   ctx->launches += 1;
   const int e_max = ctx->cfg.e_max;
@@ -342,18 +342,17 @@ epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const f
     *out_off = full_off; *out_rec = full; *out_E = Efull; *h_off = hfull;
     full_off = nullptr; full = nullptr;
   } else {
-    PP_CUDA(cudaMalloc(&fin_off, (N + 1) * sizeof(int32_t)));
+    PP_CUDA(epo_dmalloc(ctx, &fin_off, (N + 1) * sizeof(int32_t)));
     k_view_counts<<<(N + 255) / 256, 256, 0, st>>>(row_off, N, H, view_cnt);
     k_exclusive_scan<<<1, 1024, 0, st>>>(view_cnt, fin_off, N, e_max);
     std::vector<int32_t> hfin(N + 1);
     PP_CUDA(cudaMemcpyAsync(hfin.data(), fin_off, (N + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     PP_CUDA(cudaStreamSynchronize(st));
-    PP_CUDA(cudaMalloc(&fin, (size_t)(hfin[N] > 0 ? hfin[N] : 1) * sizeof(EdgeRec)));
+    PP_CUDA(epo_dmalloc(ctx, &fin, (size_t)(hfin[N] > 0 ? hfin[N] : 1) * sizeof(EdgeRec)));
     dim3 grid((e_max + 255) / 256 > 64 ? 64 : (e_max + 255) / 256, N);
     k_subsample<<<grid, 256, 0, st>>>(full, full_off, fin_off, e_max, fin);
     ctx->launches += 3;
-    PP_CUDA(cudaStreamSynchronize(st));
-    cudaFree(full_off); cudaFree(full); full_off = nullptr; full = nullptr;
+    epo_dfree(ctx, full_off); epo_dfree(ctx, full); full_off = nullptr; full = nullptr;
     *out_off = fin_off; *out_rec = fin; *out_E = hfin[N]; *h_off = hfin;
   }
   PP_CUDA(cudaGetLastError());
@@ -377,10 +376,10 @@ void epo_free_atlas(EpoAtlas* a) {
 // Enqueues on the context's stream and does NOT synchronise; the caller releases *scratch_out (row-pass
 // buffer + the surface handle the column kernel writes through) with epo_free_dtf_scratch once the stream
 // has drained.
-void epo_free_dtf_scratch(EpoDtfScratch* s) {
+void epo_free_dtf_scratch(epo_ctx* ctx, EpoDtfScratch* s) {
   if (s->surf) cudaDestroySurfaceObject(s->surf);
   if (s->surf8) cudaDestroySurfaceObject(s->surf8);
-  cudaFree(s->g);
+  epo_dfree(ctx, s->g);
   s->surf = s->surf8 = 0; s->g = nullptr;
 }
 
@@ -405,7 +404,7 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, EpoAtlas
   cudaResourceDesc rd8 = rd; rd8.res.array.array = a.arr8;
   if (e == cudaSuccess) e = cudaCreateSurfaceObject(&surf, &rd);
   if (e == cudaSuccess && !half) e = cudaCreateSurfaceObject(&surf8, &rd8);
-  if (e == cudaSuccess) e = cudaMalloc(&g, (size_t)rows * W * sizeof(int32_t));
+  if (e == cudaSuccess) e = epo_dmalloc(ctx, &g, (size_t)rows * W * sizeof(int32_t));
   if (e == cudaSuccess) {
     const int grid_rows = (int)((rows + kWarpsPerBlock - 1) / kWarpsPerBlock);
     k_edt_rows<<<grid_rows, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, rows, W, W + H, g);
@@ -437,7 +436,7 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, EpoAtlas
     cudaStreamSynchronize(st);
     if (surf) cudaDestroySurfaceObject(surf);
     if (surf8) cudaDestroySurfaceObject(surf8);
-    cudaFree(g);
+    epo_dfree(ctx, g);
     epo_free_atlas(&a);
     return epo_fail(ctx, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "distance fields: %s",
                     cudaGetErrorString(e));
@@ -452,7 +451,7 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
   float4* pts = nullptr;
   cudaStream_t st = ctx->stream;
   // padded by one chunk of zeros: the fused kernel's tail lanes read past the end of a list and discard
-  EPO_CUDA(ctx, cudaMalloc(&pts, (size_t)(E + kLgPad) * sizeof(float4)));
+  EPO_CUDA(ctx, epo_dmalloc(ctx, &pts, (size_t)(E + kLgPad) * sizeof(float4)));
   EPO_CUDA(ctx, cudaMemsetAsync(pts + E, 0, (size_t)kLgPad * sizeof(float4), st));
   cudaError_t e = cudaSuccess;
   if (subsampled) {
@@ -470,8 +469,8 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
     const int tiles_x = (W + kTile - 1) / kTile, tiles_y = (H + kTile - 1) / kTile;
     const int64_t n_tiles = (int64_t)N * tiles_x * tiles_y;
     int32_t *tile_cnt = nullptr, *tile_off = nullptr;
-    e = cudaMalloc(&tile_cnt, (size_t)(n_tiles + 1) * sizeof(int32_t));
-    if (e == cudaSuccess) e = cudaMalloc(&tile_off, (size_t)(n_tiles + 1) * sizeof(int32_t));
+    e = epo_dmalloc(ctx, &tile_cnt, (size_t)(n_tiles + 1) * sizeof(int32_t));
+    if (e == cudaSuccess) e = epo_dmalloc(ctx, &tile_off, (size_t)(n_tiles + 1) * sizeof(int32_t));
     if (e == cudaSuccess) {
       const int grid = (int)((n_tiles + kWarpsPerBlock - 1) / kWarpsPerBlock);
       k_tile_count<<<grid, kWarpsPerBlock * 32, 0, st>>>(d_edges_u8, d_depth, N, W, H, tiles_x, tiles_y, ctx->cfg.z_min, tile_cnt);
@@ -480,11 +479,10 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
                                                           tile_off, d_K, pts);
       ctx->launches += 3;
       e = cudaGetLastError();
-      if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // the scratch below is freed on return
     }
-    cudaFree(tile_cnt); cudaFree(tile_off);
+    epo_dfree(ctx, tile_cnt); epo_dfree(ctx, tile_off);
   }
-  if (e != cudaSuccess) { cudaFree(pts); return epo_fail(ctx, EPO_ERR_CUDA, "point list: %s", cudaGetErrorString(e)); }
+  if (e != cudaSuccess) { epo_dfree(ctx, pts); return epo_fail(ctx, EPO_ERR_CUDA, "point list: %s", cudaGetErrorString(e)); }
   *out_pts = pts;
   return EPO_OK;
 }
