@@ -109,6 +109,12 @@ def lib():
                               C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
                               C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                               C.POINTER(C.c_double)]
+        L.orc_canny_blur.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_uint8), C.POINTER(C.c_uint8)]
+        L.orc_canny_sobel.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_uint8), C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+        L.orc_canny_suppress.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_int, C.c_int,
+                                         C.POINTER(C.c_uint8)]
+        L.orc_canny_hysteresis.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_uint8), C.POINTER(C.c_uint8)]
+        L.orc_canny.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint8), C.c_int, C.c_int, C.POINTER(C.c_uint8)]
         L.orc_viewgraph_counts.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
                                            C.POINTER(C.c_float), C.c_int, C.c_double, C.c_double, C.c_int,
                                            C.POINTER(C.c_int32)]
@@ -276,6 +282,42 @@ def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair
 
 
 # ---------------------------------------------------------------------------------------------- O7
+def _u8p(a):
+    return a.ctypes.data_as(C.POINTER(C.c_uint8))
+
+
+def canny_blur(img: np.ndarray) -> np.ndarray:
+    img = np.ascontiguousarray(img, np.uint8); H, W = img.shape
+    out = np.zeros_like(img); lib().orc_canny_blur(W, H, _u8p(img), _u8p(out)); return out
+
+
+def canny_sobel(b: np.ndarray):
+    b = np.ascontiguousarray(b, np.uint8); H, W = b.shape
+    gx = np.zeros((H, W), np.int32); gy = np.zeros((H, W), np.int32)
+    lib().orc_canny_sobel(W, H, _u8p(b), _p(gx, C.c_int32), _p(gy, C.c_int32)); return gx, gy
+
+
+def canny_suppress(gx, gy, low: int, high: int) -> np.ndarray:
+    gx = np.ascontiguousarray(gx, np.int32); gy = np.ascontiguousarray(gy, np.int32); H, W = gx.shape
+    c = np.zeros((H, W), np.uint8)
+    lib().orc_canny_suppress(W, H, _p(gx, C.c_int32), _p(gy, C.c_int32), int(low), int(high), _u8p(c)); return c
+
+
+def canny_hysteresis(cand: np.ndarray) -> np.ndarray:
+    cand = np.ascontiguousarray(cand, np.uint8); H, W = cand.shape
+    e = np.zeros((H, W), np.uint8); lib().orc_canny_hysteresis(W, H, _u8p(cand), _u8p(e)); return e
+
+
+def canny(images: np.ndarray, low: int, high: int) -> np.ndarray:
+    """Edge maps [N][H][W] (1 / 0) of 8-bit images: the Canny detector [4], readings C1-C6."""
+    images = np.ascontiguousarray(images, np.uint8)
+    if images.ndim == 2:
+        return canny(images[None], low, high)[0]
+    N, H, W = images.shape
+    e = np.zeros((N, H, W), np.uint8)
+    lib().orc_canny(N, W, H, _u8p(images), int(low), int(high), _u8p(e)); return e
+
+
 def viewgraph_counts(K, poses, depth, stride=8, tau=3.0, z_min=1e-6, coord_fp32=0) -> np.ndarray:
     """[N][N][2] = (consistent, usable) grid points of the cycle i -> j -> i."""
     K = np.ascontiguousarray(K, np.float32); poses = np.ascontiguousarray(poses, np.float64).reshape(-1, 12)

@@ -411,6 +411,104 @@ void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, con
  * ================================================================================================= */
 /* clamp lambda: clamp_start -> clamp_end linearly over the first clamp_steps steps */
 /* =================================================================================================
+ * Edge extraction: "the edge map E_i via the Canny edge detector [4]" (Alg. 1 l.6).
+ * The paper names the detector and nothing else; this is Canny's scheme [4] -- smooth, gradient, non-maximum
+ * suppression along the gradient, hysteresis thresholding -- in integer arithmetic on 8-bit images (readings C1-C6):
+ *   C1 smoothing   separable binomial [1 4 6 4 1]/16 (sigma ~ 1), replicate border, b = (sum w_y w_x p + 128) >> 8
+ *   C2 gradient    Sobel 3x3 on b, replicate border: gx = [-1 0 1; -2 0 2; -1 0 1], gy = its transpose
+ *   C3 magnitude   m2 = gx^2 + gy^2 (the squared L2 norm: thresholds are compared squared, no square root)
+ *   C4 direction   4 sectors by integer tests with tan(22.5 deg) ~ 13573 / 32768: |gy| 32768 < |gx| 13573 -> compare the
+ *                  left/right neighbours; |gy| 13573 > |gx| 32768 -> up/down; else the diagonal with the gradient's sign
+ *   C5 suppression a candidate has m2 > low^2, m2 > m2(first neighbour) and m2 >= m2(second neighbour) (first = left,
+ *                  up, or upper diagonal neighbour: of two equal neighbours the first one stays); border pixels are never candidates
+ *   C6 hysteresis  strong = candidate with m2 > high^2; the edge map = candidates 8-connected, through candidates,
+ *                  to a strong one.  Output 1 / 0.
+ * Stages are separate functions so that each can be checked on its own.
+ * ================================================================================================= */
+static inline int orc_clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
+
+void orc_canny_blur(int W, int H, const uint8_t* img, uint8_t* out) {
+  static const int w[5] = {1, 4, 6, 4, 1};
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      int acc = 0;
+      for (int dy = -2; dy <= 2; ++dy)
+        for (int dx = -2; dx <= 2; ++dx)
+          acc += w[dy + 2] * w[dx + 2] * (int)img[(size_t)orc_clampi(y + dy, 0, H - 1) * W + orc_clampi(x + dx, 0, W - 1)];
+      out[(size_t)y * W + x] = (uint8_t)((acc + 128) >> 8);
+    }
+}
+
+void orc_canny_sobel(int W, int H, const uint8_t* b, int32_t* gx, int32_t* gy) {
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      int p[3][3];
+      for (int dy = -1; dy <= 1; ++dy)
+        for (int dx = -1; dx <= 1; ++dx)
+          p[dy + 1][dx + 1] = (int)b[(size_t)orc_clampi(y + dy, 0, H - 1) * W + orc_clampi(x + dx, 0, W - 1)];
+      gx[(size_t)y * W + x] = (p[0][2] - p[0][0]) + 2 * (p[1][2] - p[1][0]) + (p[2][2] - p[2][0]);
+      gy[(size_t)y * W + x] = (p[2][0] - p[0][0]) + 2 * (p[2][1] - p[0][1]) + (p[2][2] - p[0][2]);
+    }
+}
+
+/* cand[y][x]: 0 = no, 1 = candidate (weak), 2 = strong */
+void orc_canny_suppress(int W, int H, const int32_t* gx, const int32_t* gy, int low, int high, uint8_t* cand) {
+  const int64_t lo2 = (int64_t)low * low, hi2 = (int64_t)high * high;
+  for (int y = 0; y < H; ++y)
+    for (int x = 0; x < W; ++x) {
+      uint8_t c = 0;
+      if (x > 0 && y > 0 && x < W - 1 && y < H - 1) {
+        const size_t i = (size_t)y * W + x;
+        const int64_t ax = llabs((long long)gx[i]), ay = llabs((long long)gy[i]);
+        const int64_t m2 = ax * ax + ay * ay;
+        if (m2 > lo2) {
+          int dx1, dy1;                       /* first neighbour; the second is its mirror image */
+          if (ay * 32768 < ax * 13573) { dx1 = -1; dy1 = 0; }
+          else if (ay * 13573 > ax * 32768) { dx1 = 0; dy1 = -1; }
+          else if ((gx[i] < 0) == (gy[i] < 0)) { dx1 = -1; dy1 = -1; }
+          else { dx1 = 1; dy1 = -1; }
+          const size_t a = (size_t)(y + dy1) * W + (x + dx1), b = (size_t)(y - dy1) * W + (x - dx1);
+          const int64_t ma = (int64_t)gx[a] * gx[a] + (int64_t)gy[a] * gy[a], mb = (int64_t)gx[b] * gx[b] + (int64_t)gy[b] * gy[b];
+          if (m2 > ma && m2 >= mb) c = m2 > hi2 ? 2 : 1;
+        }
+      }
+      cand[(size_t)y * W + x] = c;
+    }
+}
+
+void orc_canny_hysteresis(int W, int H, const uint8_t* cand, uint8_t* edges) {
+  int32_t* stack = (int32_t*)malloc((size_t)W * H * sizeof(int32_t));
+  int64_t top = 0;
+  for (int64_t i = 0; i < (int64_t)W * H; ++i) { edges[i] = 0; if (cand[i] == 2) { edges[i] = 1; stack[top++] = (int32_t)i; } }
+  while (top > 0) {
+    const int32_t i = stack[--top];
+    const int x = i % W, y = i / W;
+    for (int dy = -1; dy <= 1; ++dy)
+      for (int dx = -1; dx <= 1; ++dx) {
+        const int xx = x + dx, yy = y + dy;
+        if (xx < 0 || yy < 0 || xx >= W || yy >= H) continue;
+        const int32_t j = yy * W + xx;
+        if (cand[j] && !edges[j]) { edges[j] = 1; stack[top++] = j; }
+      }
+  }
+  free(stack);
+}
+
+void orc_canny(int N, int W, int H, const uint8_t* img, int low, int high, uint8_t* edges) {
+#pragma omp parallel for schedule(dynamic)
+  for (int n = 0; n < N; ++n) {
+    const size_t px = (size_t)W * H;
+    uint8_t* b = (uint8_t*)malloc(px); uint8_t* c = (uint8_t*)malloc(px);
+    int32_t* gx = (int32_t*)malloc(px * sizeof(int32_t)); int32_t* gy = (int32_t*)malloc(px * sizeof(int32_t));
+    orc_canny_blur(W, H, img + n * px, b);
+    orc_canny_sobel(W, H, b, gx, gy);
+    orc_canny_suppress(W, H, gx, gy, low, high, c);
+    orc_canny_hysteresis(W, H, c, edges + n * px);
+    free(b); free(c); free(gx); free(gy);
+  }
+}
+
+/* =================================================================================================
  * Viewgraph estimation by exhaustive cycle-consistent reprojection (Eq. 2; 117; 380-384; 396).
  * "we project each pixel p of image I_i onto I_j using pi (Eq. 2) ... The resulting p_{i->j} is then projected back
  * onto I_i to obtain p_{i->j->i}.  An image pair is called valid if sufficiently many pixels satisfy a bidirectional
