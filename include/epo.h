@@ -92,6 +92,17 @@ EPO_API epo_status epo_create(const epo_config* cfg, epo_ctx** out);
 EPO_API void epo_destroy(epo_ctx* ctx);
 
 /*
+ * Edge extraction ("the edge map E_i via the Canny edge detector [4]"; Alg. 1 l.6):
+ * images [N][H][W] 8-bit grey -> edges [N][H][W] u8 (1 = edge, 0), ready for epo_set_views.  Canny's scheme in integer
+ * arithmetic: binomial 5x5 smoothing (replicate border, rounded), Sobel 3x3, squared L2 magnitude, non-maximum
+ * suppression in four direction sectors, hysteresis with thresholds low <= high on the gradient magnitude (strict:
+ * a candidate has |g| > low, a strong one |g| > high; 0 <= low <= high <= 1442).  Border pixels are never edges.
+ * The paper states no parameters; the caller chooses the thresholds.  Host or device pointers; N, W, H are the
+ * context's.  Synchronises the stream (the hysteresis is iterated until nothing changes).
+ */
+EPO_API epo_status epo_extract_edges(epo_ctx* ctx, const uint8_t* images, int32_t low, int32_t high, uint8_t* edges);
+
+/*
  * Load the initial estimate G = {K_i, P_i, Z_i} (Eq. 1) and the edge maps E_i
  * (PAPER.md:62), and run the one-time preprocessing (Alg. 1 l.6-7):
  *   - edge-pixel compaction: per view, the list of (u, v, Z) with edges != 0 and finite Z > z_min, in

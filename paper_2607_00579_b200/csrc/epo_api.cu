@@ -569,6 +569,30 @@ epo_status epo_get_trace(epo_ctx* c, int32_t first, int32_t count, float* loss, 
   return EPO_OK;
 }
 
+epo_status epo_extract_edges(epo_ctx* c, const uint8_t* images, int32_t low, int32_t high, uint8_t* edges) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!images || !edges || low < 0 || high < low || high > 1442)    // |g| <= 1020 sqrt(2)
+    return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_extract_edges: bad argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t px = (size_t)c->N * c->W * c->H;
+  uint8_t *d_img = nullptr, *d_out = nullptr;
+  const bool in_dev = is_device_ptr(images), out_dev = is_device_ptr(edges);
+  cudaError_t e = cudaSuccess;
+  if (!in_dev) { e = epo_dmalloc(c, &d_img, px); if (e == cudaSuccess) e = cudaMemcpyAsync(d_img, images, px, cudaMemcpyHostToDevice, st); }
+  if (e == cudaSuccess && !out_dev) e = epo_dmalloc(c, &d_out, px);
+  epo_status rc = e == cudaSuccess ? epo_run_canny(c, in_dev ? images : d_img, low, high, out_dev ? edges : d_out)
+                                   : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
+                                              "epo_extract_edges: %s", cudaGetErrorString(e));
+  if (rc == EPO_OK && !out_dev) {
+    e = cudaMemcpyAsync(edges, d_out, px, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_extract_edges: %s", cudaGetErrorString(e));
+  }
+  epo_dfree(c, d_img); epo_dfree(c, d_out);
+  return rc;
+}
+
 epo_status epo_build_viewgraph(epo_ctx* c, int32_t grid_stride, float tau, float min_frac, int32_t* pairs, int64_t capacity,
                                int64_t* n_pairs, int32_t* counts) {
   if (!c) return EPO_ERR_INVALID_ARG;

@@ -201,6 +201,8 @@ constexpr int kSelScrBarrier = 0, kSelScrNCand = 2, kSelScrHist = 4, kSelScrTota
               kSelScrInts = kSelScrCandIdx + kSelCandCap;
 int64_t epo_select_max_pairs(void);
 epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override /* < 0: device step */, bool gated, bool build_work);
+// canny.cu: edge maps (1 / 0) of [N][H][W] 8-bit images, device pointers
+epo_status epo_run_canny(epo_ctx* ctx, const uint8_t* d_img, int low, int high, uint8_t* d_edges);
 // viewgraph.cu: cycle counts of all ordered pairs + ordered emission of the valid pairs
 epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_frac, int2* d_counts, int2* d_pairs,
                                 long long* d_n);

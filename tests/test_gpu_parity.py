@@ -327,6 +327,72 @@ def test_early_stop_parity():
     e.destroy()
 
 
+# ---------------------------------------------------------------------------------- edge extraction
+def _test_images(n, H, W, seed):
+    """Seeded 8-bit images with edges of every orientation and strength: rectangles and discs of random grey levels
+    on a smooth background, a long thin spiral (hysteresis chains that cross many tiles), and noise."""
+    rng = np.random.default_rng(seed)
+    yy, xx = np.mgrid[0:H, 0:W].astype(np.float64)
+    out = np.zeros((n, H, W), np.uint8)
+    for k in range(n):
+        img = 100 + 40 * np.sin(xx / (17 + 3 * k)) * np.cos(yy / 23.0)
+        for _ in range(12):
+            x0, y0 = rng.integers(0, W), rng.integers(0, H); w, h = rng.integers(4, W // 2), rng.integers(4, H // 2)
+            lvl = rng.integers(0, 256)
+            if rng.random() < 0.5:
+                img[y0:y0 + h, x0:x0 + w] = lvl
+            else:
+                img[(xx - x0) ** 2 + (yy - y0) ** 2 < (min(w, h) / 2) ** 2] = lvl
+        t = np.linspace(0, 14 * np.pi, 6000)
+        sx = (W / 2 + (2 + t * min(W, H) / 100) * np.cos(t)).astype(int); sy = (H / 2 + (2 + t * min(W, H) / 100) * np.sin(t)).astype(int)
+        ok = (sx >= 0) & (sx < W) & (sy >= 0) & (sy < H)
+        img[sy[ok], sx[ok]] += 14 + 10 * (np.arange(ok.sum()) % 97 == 0)      # faint line, strong only every 97th point
+        img = img + rng.normal(0, 1.5, (H, W))
+        out[k] = np.clip(np.rint(img), 0, 255).astype(np.uint8)
+    return out
+
+
+@pytest.mark.parametrize("shape,low,high", [((3, 96, 128), 20, 60), ((2, 101, 67), 8, 30), ((2, 33, 40), 0, 0), ((1, 392, 518), 12, 48)])
+def test_edge_extraction_bit_exact(shape, low, high):
+    """epo_extract_edges (Canny) against the oracle, byte for byte: sizes that are and are not
+    multiples of the 32-pixel tile, thresholds from 0 up, host and device pointers."""
+    import torch
+    from paper_2607_00579_b200 import Epo, epo_config_default
+    n, H, W = shape
+    imgs = _test_images(n, H, W, seed=n * 1000 + W)
+    e = Epo(epo_config_default(n_views=max(n, 2), width=W, height=H, stream=torch.cuda.current_stream().cuda_stream))
+    if n < 2:
+        imgs = np.concatenate([imgs, imgs[:, ::-1].copy()])
+    ref = oracle.canny(imgs, low, high)
+    got = e.extract_edges(imgs, low, high)
+    assert np.array_equal(got, ref), (np.argwhere(got != ref)[:5], int((got != ref).sum()))
+    d_out = torch.zeros(imgs.shape, dtype=torch.uint8, device="cuda")
+    e.extract_edges(torch.from_numpy(imgs).cuda(), low, high, out=d_out)
+    assert np.array_equal(d_out.cpu().numpy(), ref)
+    frac = ref.mean()
+    print(f"{shape} low={low} high={high}: {100 * frac:.1f} % edge pixels")
+    assert 0.005 < frac < 0.6
+    e.destroy()
+
+
+def test_edge_extraction_feeds_the_pipeline_and_rejects_bad_thresholds():
+    import paper_2607_00579_b200 as pkg
+    sc = scene("tiny")
+    e = make_ctx(sc)
+    grey = np.clip(40.0 * sc.depth, 0, 255).astype(np.uint8)          # depth shading: edges at depth discontinuities
+    edges = e.extract_edges(grey, 10, 30)
+    assert np.array_equal(edges, oracle.canny(grey, 10, 30))
+    e.set_views(sc.K, sc.poses_init, sc.depth, edges); e.set_pairs(sc.pairs)
+    prob = oracle.preprocess(sc.K, sc.depth, edges, z_min=Z_MIN)
+    got = e.loss_grad(10.0)
+    ref = oracle.loss_grad(prob, sc.poses_init.astype(np.float64), sc.pairs, 10.0, z_min=Z_MIN, coord_fp32=1)
+    assert abs(got["loss"] - ref["loss"]) <= 1e-5 * abs(ref["loss"])
+    L = pkg.lib()
+    for lo, hi in ((-1, 5), (10, 5), (0, 2000)):
+        assert L.epo_extract_edges(e._h, grey.ctypes.data, lo, hi, edges.ctypes.data) == pkg.EPO_ERR_INVALID_ARG
+    e.destroy()
+
+
 # ------------------------------------------------------------------------------ viewgraph estimation
 @pytest.mark.parametrize("name,stride", [("tiny", 4), ("room6", 8), ("orbit8", 8), ("orbit10_dense", 5)])
 def test_viewgraph_counts_and_pairs_bit_exact(name, stride):
