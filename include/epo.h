@@ -160,6 +160,9 @@ EPO_API epo_status epo_loss_grad(epo_ctx* ctx, float lambda, float* loss, float*
  * Iterations stop early when the step counter reaches max_steps or, if early_stop, when phase 2 is
  * reached.  iters_done / phase (0, 1, or 2 = second convergence reached) are nullable; host pointers
  * there make the call synchronise.
+ * With cfg.pair_budget = M > 0 and more than M pairs, iteration s evaluates the fresh uniform random subset of M
+ * pairs that epo_get_pair_subset(ctx, s, ...) reports, drawn by a device kernel inside the loop; loss
+ * and gradient are then means over those M pairs.  epo_loss_grad always evaluates the whole list.
  */
 EPO_API epo_status epo_step(epo_ctx* ctx, int32_t n_iters, int32_t* iters_done, int32_t* phase);
 
