@@ -37,7 +37,8 @@ class _Cfg(C.Structure):
                 ("max_steps", C.c_int32), ("beta1", C.c_double), ("beta2", C.c_double),
                 ("adam_eps", C.c_double), ("eps1", C.c_double), ("eps2", C.c_double), ("w1", C.c_int32),
                 ("w2", C.c_int32), ("smooth_window", C.c_int32), ("early_stop", C.c_int32),
-                ("z_min", C.c_double), ("coord_fp32", C.c_int32)]
+                ("z_min", C.c_double), ("coord_fp32", C.c_int32), ("stop_rule", C.c_int32), ("w_loss", C.c_int32),
+                ("eps_loss", C.c_double)]
 
 
 @dataclass
@@ -61,6 +62,9 @@ class Config:
     early_stop: int = 0
     z_min: float = 1e-6
     coord_fp32: int = 0      # 1: projected positions decided in fp32 (reading P1)
+    stop_rule: int = 0       # second-stage rule: 0 pose-based (the paper's), 1 loss-based
+    w_loss: int = 100
+    eps_loss: float = 5e-4
 
     def c(self) -> _Cfg:
         return _Cfg(**{f[0]: getattr(self, f[0]) for f in _Cfg._fields_})
@@ -86,6 +90,7 @@ def lib():
         L.orc_theta95.restype = C.c_double
         L.orc_round_to_half.restype = C.c_float
         L.orc_round_to_half.argtypes = [C.c_float]
+        L.orc_converged_loss.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_int, C.c_double]
         L.orc_converged.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_int, C.c_double, C.c_int]
         L.orc_adam.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
                                C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]
@@ -399,6 +404,12 @@ def theta95(cur, prev):
     cur = _d(cur); prev = _d(prev)
     lib().orc_theta95.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     return lib().orc_theta95(cur.size // 12, _p(cur, C.c_double), _p(prev, C.c_double))
+
+
+def converged_loss(loss, s, w, eps) -> bool:
+    """The loss-based stopping rule at step s: relative loss change below eps for w consecutive steps."""
+    loss = np.ascontiguousarray(loss, np.float64)
+    return bool(lib().orc_converged_loss(_p(loss, C.c_double), int(s), int(w), C.c_double(eps)))
 
 
 def converged(theta, s, w, eps, smooth=1) -> bool:

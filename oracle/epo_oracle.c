@@ -782,6 +782,8 @@ typedef struct {
   double beta1, beta2, adam_eps, eps1, eps2; int32_t w1, w2, smooth_window, early_stop;
   double z_min;
   int32_t coord_fp32;   /* 0: everything in double; 1: projected positions decided in fp32 (reading P1) */
+  int32_t stop_rule;    /* second-stage stopping rule: 0 pose-based (Eq. 9-10, the paper's), 1 loss-based */
+  int32_t w_loss; double eps_loss;   /* 100, 5e-4 */
 } orc_config;
 
 /* =================================================================================================
@@ -791,6 +793,21 @@ typedef struct {
  * poses [N][12] in/out; m, v [N][6] in/out; theta_hist [max_steps] in/out; *step, *phase in/out.
  * trace_loss[s] = loss at the poses BEFORE update s.  Returns the number of iterations executed.
  * ================================================================================================= */
+/* Loss-based stopping criterion (Tab. 7): "monitors relative changes in the loss, stopping when it remains
+ * below a threshold eps_2 = 5e-4 for w_2 = 100 consecutive steps".  Relative change of step k >= 1:
+ * r_k = |L_k - L_{k-1}| / |L_{k-1}| (infinite if L_{k-1} = 0 and L_k != 0, zero if both are 0); the rule holds at step s
+ * iff r_k < eps for the w steps k = s-w+1 .. s, which needs s >= w (reading L1).  It replaces only the SECOND-stage test:
+ * "All criteria share the same first stage".                                                                        */
+int orc_converged_loss(const double* loss, int s, int w, double eps) {
+  if (w < 1 || s < w) return 0;
+  for (int k = s - w + 1; k <= s; ++k) {
+    const double a = loss[k - 1], d = fabs(loss[k] - a);
+    const double r = a != 0.0 ? d / fabs(a) : (d == 0.0 ? 0.0 : INFINITY);
+    if (!(r < eps)) return 0;
+  }
+  return 1;
+}
+
 int orc_run(const orc_config* cfg, int n_iters, int N, int W, int H, const float* K, double* poses,
             const int32_t* edge_off, const uint16_t* uv, const float* z, const float* dtf, int64_t P,
             const int32_t* pairs, double* m, double* v, double* theta_hist, double* trace_loss,
@@ -818,7 +835,10 @@ int orc_run(const orc_config* cfg, int n_iters, int N, int W, int H, const float
     }
     theta_hist[s] = orc_theta95(N, poses, prev);
     if (*phase == 0) { if (orc_converged(theta_hist, s, cfg->w1, cfg->eps1, cfg->smooth_window)) *phase = 1; }
-    else if (*phase == 1) { if (orc_converged(theta_hist, s, cfg->w2, cfg->eps2, cfg->smooth_window)) *phase = 2; }
+    else if (*phase == 1) {
+      if (cfg->stop_rule == 1 ? orc_converged_loss(trace_loss, s, cfg->w_loss, cfg->eps_loss)
+                              : orc_converged(theta_hist, s, cfg->w2, cfg->eps2, cfg->smooth_window)) *phase = 2;
+    }
     if (poses_log) memcpy(poses_log + (size_t)done * N * 12, poses, (size_t)N * 12 * sizeof(double));
     *step = s + 1; ++done;
   }

@@ -192,3 +192,19 @@ def test_optimisation_descends_towards_ground_truth(tiny_scene, tiny_problem):
         return np.array(errs)
     e0 = rel_rot_err(s.poses_init.astype(np.float64)); e1 = rel_rot_err(opt.poses)
     assert e1.mean() < 0.25 * e0.mean()
+
+
+def test_Z11_loss_based_stopping_rule_on_hand_made_traces():
+    """relative loss change below eps for w consecutive steps (second stage only).  Hand-computed."""
+    geo = 2.0 * 0.999 ** np.arange(400)                       # relative change exactly ~1e-3 every step
+    assert not any(oracle.converged_loss(geo, s, 100, 5e-4) for s in range(400))
+    assert oracle.converged_loss(geo, 100, 100, 2e-3) and not oracle.converged_loss(geo, 99, 100, 2e-3)   # needs s >= w
+    flat = np.concatenate([np.linspace(3.0, 1.0, 50), np.full(200, 1.0)])
+    fired = [s for s in range(250) if oracle.converged_loss(flat, s, 100, 5e-4)]
+    assert fired[0] == 149          # changes k = 50 .. 149 are the first 100 zero changes (L_49 = L_50 = 1.0)
+    spike = flat.copy(); spike[120] = 1.01                    # two changes (120, 121) of 1 % restart the count
+    fired = [s for s in range(250) if oracle.converged_loss(spike, s, 100, 5e-4)]
+    assert fired[0] == 221
+    assert oracle.converged_loss(np.array([1.0, 1.0 + 4.9e-4]), 1, 1, 5e-4)
+    assert not oracle.converged_loss(np.array([1.0, 1.0 + 5.0e-4 + 1e-12]), 1, 1, 5e-4)       # strict
+    assert oracle.converged_loss(np.zeros(5), 4, 3, 1e-9) and not oracle.converged_loss(np.array([0.0, 1e-30]), 1, 1, 0.5)
