@@ -80,6 +80,12 @@ typedef struct {
                                        gets, at optimiser step s, the key = output number s * 2^32 + p + 1 of
                                        SplitMix64(subsample_seed); the subset is the M pairs with the smallest
                                        (key, p).  A pure function of (seed, s, p): reproducible, no host draw.  */
+  int32_t stop_rule;                /* second-stage stopping rule: 0 (default) pose-based, Eq. 9-10 with w2 / eps2;
+                                       1 loss-based (the variant of Tab. 7): the relative loss change
+                                       |L_s - L_{s-1}| / |L_{s-1}| stays below eps_loss for w_loss consecutive steps.
+                                       The first stage (phase 0 -> 1) is pose-based in both.                        */
+  int32_t w_loss;                   /* 100                                                           */
+  float   eps_loss;                 /* 5e-4                                                          */
 } epo_config;
 
 /* Fill *cfg with the paper's hyper-parameters (n_views/width/height = 0, device 0, stream NULL). */

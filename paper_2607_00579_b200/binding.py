@@ -35,7 +35,8 @@ class EpoConfig(C.Structure):
                 ("eps2", C.c_float), ("w1", C.c_int32), ("w2", C.c_int32), ("smooth_window", C.c_int32),
                 ("early_stop", C.c_int32), ("dtf_format", C.c_int32), ("e_max", C.c_int32), ("z_min", C.c_float),
                 ("device", C.c_int32), ("stream", C.c_void_p), ("pair_budget", C.c_int32),
-                ("subsample_seed", C.c_uint64)]
+                ("subsample_seed", C.c_uint64), ("stop_rule", C.c_int32), ("w_loss", C.c_int32),
+                ("eps_loss", C.c_float)]
 
 
 class EpoError(RuntimeError):

@@ -121,6 +121,7 @@ epo_status epo_config_default(epo_config* cfg) {
   cfg->smooth_window = 1; cfg->early_stop = 1; cfg->dtf_format = 0; cfg->e_max = 0;
   cfg->z_min = 1e-6f; cfg->device = 0; cfg->stream = nullptr;
   cfg->pair_budget = 0; cfg->subsample_seed = 0;
+  cfg->stop_rule = 0; cfg->w_loss = 100; cfg->eps_loss = 5e-4f;
   return EPO_OK;
 }
 
@@ -131,7 +132,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
     return EPO_ERR_INVALID_ARG;
   if (!(cfg->huber_delta > 0.f) || cfg->clamp_steps < 1 || cfg->warmup_steps < 0 || cfg->max_steps <= cfg->warmup_steps ||
       cfg->w1 < 1 || cfg->w2 < 1 || (cfg->dtf_format != 0 && cfg->dtf_format != 1) || cfg->e_max < 0 ||
-      cfg->pair_budget < 0 || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
+      cfg->pair_budget < 0 || (cfg->stop_rule != 0 && cfg->stop_rule != 1) || cfg->w_loss < 1 || !(cfg->eps_loss >= 0.f) || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
     return EPO_ERR_INVALID_ARG;
   epo_ctx* c = new (std::nothrow) epo_ctx();
   if (!c) return EPO_ERR_OUT_OF_MEMORY;

@@ -7,6 +7,8 @@
 // The pose parameterisation is a left se(3) increment per camera, T_c <- Exp(eps_c) T_c (north_star;
 // DESIGN.md reading S9).  The stop decision is written to the device control block so that the
 // following iterations' kernels exit immediately: epo_step never synchronises with the host.
+#include <math_constants.h>
+
 #include "epo_internal.h"
 
 namespace {
@@ -31,7 +33,8 @@ struct FinParams {
   int64_t P;
   double beta1, beta2, adam_eps, eps1, eps2;
   const double* sched;          // [max_steps][4] {lr_s, 1 - beta1^(s+1), 1 - beta2^(s+1), lambda_s}
-  int max_steps, w1, w2, smooth, early_stop;
+  int max_steps, w1, w2, smooth, early_stop, stop_rule, w_loss;
+  double eps_loss;
   int gated, step_mode, call_first;
 };
 
@@ -129,6 +132,20 @@ __device__ bool converged(const double* theta, double theta_s, int s, int w, dou
 //  a-11  per-camera pose change; then the LAST CTA to finish (atomic ticket) publishes the new poses, takes the
 //  a-12  two 95th percentiles, runs the windowed two-phase test and advances the device control block.
 // ---------------------------------------------------------------------------------------------------------
+// Loss-based rule: relative loss change |L_k - L_{k-1}| / |L_{k-1}| < eps for the w steps k = s-w+1 .. s
+// (s >= w); thread j tests step s - j, strided over the window.
+__device__ bool converged_loss(const double* trace, double loss_s, int s, int w, double eps) {
+  if (w < 1 || s < w) return false;                  // uniform
+  bool ok = true;
+  auto L = [&](int k) { return k == s ? loss_s : __ldcg(trace + k); };
+  for (int j = threadIdx.x; j < w; j += blockDim.x) {
+    const double a = L(s - j - 1), d = fabs(L(s - j) - a);
+    const double r = a != 0.0 ? d / fabs(a) : (d == 0.0 ? 0.0 : CUDART_INF);
+    ok = ok && (r < eps);
+  }
+  return __syncthreads_and(ok) != 0;
+}
+
 __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   DevState* st = p.state;
   extern __shared__ double sdyn[];                 // last CTA: dR[N], dt[N]
@@ -306,7 +323,10 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   const double th = r95 > t95 ? r95 : t95;
   int phase = st->phase;
   if (phase == 0) { if (converged(p.theta, th, s, p.w1, p.eps1, p.smooth)) phase = 1; }
-  else if (phase == 1) { if (converged(p.theta, th, s, p.w2, p.eps2, p.smooth)) phase = 2; }
+  else if (phase == 1) {
+    if (p.stop_rule == 1 ? converged_loss(p.loss_trace, loss, s, p.w_loss, p.eps_loss)
+                         : converged(p.theta, th, s, p.w2, p.eps2, p.smooth)) phase = 2;
+  }
   if (tid == 0) {
     p.theta[s] = th;
     p.loss_trace[s] = loss;
@@ -362,6 +382,7 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   p.sched = ctx->d_sched; p.beta1 = ctx->cfg.beta1; p.beta2 = ctx->cfg.beta2; p.adam_eps = ctx->cfg.adam_eps;
   p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.max_steps = ctx->cfg.max_steps;
   p.w1 = ctx->cfg.w1; p.w2 = ctx->cfg.w2; p.smooth = ctx->cfg.smooth_window; p.early_stop = ctx->cfg.early_stop;
+  p.stop_rule = ctx->cfg.stop_rule; p.w_loss = ctx->cfg.w_loss; p.eps_loss = ctx->cfg.eps_loss;
   p.gated = gated ? 1 : 0; p.step_mode = step_mode ? 1 : 0; p.call_first = call_first ? 1 : 0;
   const size_t smem = (size_t)2 * ctx->N * sizeof(double);   // the last CTA's copy of dR, dt
   if (smem > 200 * 1024) return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "more than %d views", 200 * 1024 / 16);

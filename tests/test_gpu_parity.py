@@ -210,7 +210,7 @@ def _lockstep(sc, iters, cfg_kw, okw):
     poses = e.get_poses_f64()
     assert np.array_equal(poses, sc.poses_init.astype(np.float64))
     worst = dict(rot=0.0, tr=0.0, theta=0.0, loss=0.0)
-    thetas = []; phase = 0; stop_at = None
+    thetas = []; losses = []; phase = 0; stop_at = None
     budget, seed = cfg_kw.get("pair_budget", 0), cfg_kw.get("subsample_seed", 0)
     for k in range(iters):
         # stochastic viewgraph sub-sampling: the oracle evaluates its own draw of step k
@@ -230,10 +230,11 @@ def _lockstep(sc, iters, cfg_kw, okw):
         worst["theta"] = max(worst["theta"], abs(float(theta[0]) - th_pred) / max(abs(th_pred), 1e-4 / 1e-3))
         worst["loss"] = max(worst["loss"], abs(float(loss[0]) - ref["loss"]) / abs(ref["loss"]))
         # the stopping rule, run by the oracle on the oracle's own theta values
-        thetas.append(th_pred)
+        thetas.append(th_pred); losses.append(ref["loss"])
         if phase == 0:
             if oracle.converged(np.array(thetas), k, ocfg.w1, ocfg.eps1, ocfg.smooth_window): phase = 1
-        elif phase == 1 and oracle.converged(np.array(thetas), k, ocfg.w2, ocfg.eps2, ocfg.smooth_window):
+        elif phase == 1 and (oracle.converged_loss(np.array(losses), k, ocfg.w_loss, ocfg.eps_loss) if ocfg.stop_rule == 1
+                             else oracle.converged(np.array(thetas), k, ocfg.w2, ocfg.eps2, ocfg.smooth_window)):
             phase = 2
         assert gphase == phase, (k, gphase, phase)
         if phase == 2 and stop_at is None:
@@ -499,6 +500,30 @@ def test_measurement_hooks_leave_results_unchanged():
     after = e.loss_grad(10.0)
     assert after["loss"] == before["loss"] and np.array_equal(after["grad"], before["grad"])
     assert e.step(3) == (3, 0)
+    e.destroy()
+
+
+def test_loss_based_stopping_rule():
+    """The loss-based second-stage criterion (Tab. 7; cfg.stop_rule = 1) with shortened windows: lock-step
+    phase parity with the oracle's rule at every iteration and the same stop step; the first stage stays pose-based."""
+    sc = scene("orbit10_dense")
+    kw = dict(w1=10, eps1=0.5, early_stop=1, stop_rule=1, w_loss=12, eps_loss=3e-3)
+    okw = {k: (float(np.float32(v)) if isinstance(v, float) else v) for k, v in kw.items()}
+    worst, stop_at, n = _lockstep(sc, 700, kw, okw)
+    print(f"loss-based stop: oracle rule fires after {stop_at} iterations, GPU ran {n}")
+    assert stop_at is not None and n == stop_at < 700
+    assert worst["rot"] <= 1e-3 and worst["tr"] <= 1e-4 and worst["loss"] <= 1e-5
+    e = make_ctx(sc, **kw)                                   # free-running, one call
+    done, phase = e.step(700)
+    assert phase == 2 and done < 700 and e.step(3) == (0, 2)
+    loss, theta = e.get_trace(0, done)
+    ph, fired = 0, None                                      # the rules re-run on the GPU's own traces
+    for s_ in range(done):
+        if ph == 0:
+            if oracle.converged(theta.astype(np.float64), s_, 10, okw["eps1"], 1): ph = 1
+        elif oracle.converged_loss(loss.astype(np.float64), s_, 12, okw["eps_loss"]):
+            fired = s_ + 1; break
+    assert fired == done, (fired, done)
     e.destroy()
 
 
