@@ -107,6 +107,10 @@ def lib():
                                     C.c_double, C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int32),
                                     C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_double),
                                     C.POINTER(C.c_double)]
+        L.orc_joint_grad.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
+                                     C.POINTER(C.c_int32), C.POINTER(C.c_uint16), C.POINTER(C.c_float),
+                                     C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_int32), C.c_double, C.c_double,
+                                     C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_run.restype = C.c_int
         L.orc_run.argtypes = [C.POINTER(_Cfg), C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float),
                               C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_uint16),
@@ -284,6 +288,19 @@ def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair
                         _p(pl, C.c_double), _p(pv, C.c_int32), _p(pG, C.c_double), _p(near, C.c_int32),
                         _p(grad, C.c_double), C.byref(L))
     return dict(loss=L.value, pair_loss=pl, pair_valid=pv, grad=grad, near=near, pair_G=pG)
+
+
+def joint_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, coord_fp32=0):
+    """Joint-phase gradients (Eq. 4-5): (d L / d ln f_c [N], d L / d Z_e [E] in edge-list order)."""
+    N = prob.n_views
+    poses = np.ascontiguousarray(np.asarray(poses, np.float64).reshape(N, 12))
+    pairs = np.ascontiguousarray(pairs, np.int32); P = pairs.shape[0]
+    g_f = np.zeros(N); g_z = np.zeros(int(prob.edge_off[-1]))
+    lib().orc_joint_grad(N, prob.W, prob.H, _p(prob.K, C.c_float), _p(poses, C.c_double), _p(prob.edge_off, C.c_int32),
+                         _p(prob.uv, C.c_uint16), _p(prob.z, C.c_float), _p(prob.dtf, C.c_float), P, _p(pairs, C.c_int32),
+                         C.c_double(lam), C.c_double(delta), C.c_double(z_min), int(coord_fp32), _p(g_f, C.c_double),
+                         _p(g_z, C.c_double))
+    return g_f, g_z
 
 
 # ---------------------------------------------------------------------------------------------- O7

@@ -242,7 +242,8 @@ void orc_relative_pose(const double Ts[12], const double Tt[12], double Tts[12])
 static void orc_pair_loss_grad_f32coords(int W, int H, int n_edges, const uint16_t* uv, const float* z,
                                          const double Ks[4], const double Kt[4], const double Tts[12],
                                          const float* dtf_t, double lambda, double delta, double z_min,
-                                         double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2]) {
+                                         double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2],
+                                         double* J /* nullable [2] */, double* dZ /* nullable [n_edges] */) {
   float T[12];
   for (int k = 0; k < 12; ++k) T[k] = (float)Tts[k];
   const float ifx = 1.0f / (float)Ks[0], ify = 1.0f / (float)Ks[1], cxs = (float)Ks[2], cys = (float)Ks[3];
@@ -251,6 +252,8 @@ static void orc_pair_loss_grad_f32coords(int W, int H, int n_edges, const uint16
   double S = 0.0; int32_t nv = 0;
   for (int k = 0; k < 12; ++k) G[k] = 0.0;
   near[0] = near[1] = 0;
+  if (J) J[0] = J[1] = 0.0;
+  if (dZ) for (int e = 0; e < n_edges; ++e) dZ[e] = 0.0;
   for (int e = 0; e < n_edges; ++e) {
     const float u = (float)uv[2 * e], v = (float)uv[2 * e + 1], Zs = z[e];
     const float a_ = (u - cxs) * ifx, b_ = (v - cys) * ify;
@@ -299,6 +302,13 @@ static void orc_pair_loss_grad_f32coords(int W, int H, int n_edges, const uint16
     G[4] += xt[2] * a[0] - xt[0] * a[2];
     G[5] += xt[0] * a[1] - xt[1] * a[0];
     for (int i = 0; i < 3; ++i) b[i] = Tts[i] * a[0] + Tts[4 + i] * a[1] + Tts[8 + i] * a[2];
+    /* joint phase (Eq. 4-5): d rho / d ln f_t, d rho / d ln f_s (both focal lengths of a camera scale
+     * together, f = f0 (1 + gamma)) and d rho / d Z_s of this edge pixel:
+     *   (x, y) - c_t = f_t (X, Y)/Z            ->  d rho / d ln f_t = rho' (dd/dx (x - cx_t) + dd/dy (y - cy_t))
+     *   x_s = Z ((u - cx)/fx, (v - cy)/fy, 1)  ->  d x_s / d ln f_s = (-x_s.x, -x_s.y, 0),  d x_s / d Z = x_s / Z
+     *   and d rho / d x_s = R_ts^T a = b                                                                           */
+    if (J) { J[0] += drho * (ddx * (x - Kt[2]) + ddy * (y - Kt[3])); J[1] -= b[0] * xs[0] + b[1] * xs[1]; }
+    if (dZ) dZ[e] = (b[0] * xs[0] + b[1] * xs[1] + b[2] * xs[2]) / (double)z[e];
     G[6] -= b[0]; G[7] -= b[1]; G[8] -= b[2];
     G[9]  -= xs[1] * b[2] - xs[2] * b[1];
     G[10] -= xs[2] * b[0] - xs[0] * b[2];
@@ -307,19 +317,23 @@ static void orc_pair_loss_grad_f32coords(int W, int H, int n_edges, const uint16
   *sum_rho = S; *n_valid = nv;
 }
 
-void orc_pair_loss_grad(int W, int H, int n_edges, const uint16_t* uv, const float* z,
-                        const double Ks[4], const double Kt[4], const double Ts[12], const double Tt[12],
-                        const float* dtf_t, double lambda, double delta, double z_min, int coord_fp32,
-                        double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2]) {
+void orc_pair_loss_grad_joint(int W, int H, int n_edges, const uint16_t* uv, const float* z,
+                              const double Ks[4], const double Kt[4], const double Ts[12], const double Tt[12],
+                              const float* dtf_t, double lambda, double delta, double z_min, int coord_fp32,
+                              double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2],
+                              double* J /* nullable [2]: sum d rho / d ln f_t, sum d rho / d ln f_s */,
+                              double* dZ /* nullable [n_edges]: d rho / d Z_s per edge pixel (0 if not valid) */) {
   double Tts[12];
   orc_relative_pose(Ts, Tt, Tts);
   if (coord_fp32) {
-    orc_pair_loss_grad_f32coords(W, H, n_edges, uv, z, Ks, Kt, Tts, dtf_t, lambda, delta, z_min, sum_rho, n_valid, G, near);
+    orc_pair_loss_grad_f32coords(W, H, n_edges, uv, z, Ks, Kt, Tts, dtf_t, lambda, delta, z_min, sum_rho, n_valid, G, near, J, dZ);
     return;
   }
   double S = 0.0; int32_t nv = 0;
   for (int k = 0; k < 12; ++k) G[k] = 0.0;
   near[0] = near[1] = 0;
+  if (J) J[0] = J[1] = 0.0;
+  if (dZ) for (int e = 0; e < n_edges; ++e) dZ[e] = 0.0;
   for (int e = 0; e < n_edges; ++e) {
     double xs[3], xt[3], px[2];
     orc_backproject_cam(Ks, (double)uv[2 * e], (double)uv[2 * e + 1], (double)z[e], xs);
@@ -356,6 +370,13 @@ void orc_pair_loss_grad(int W, int H, int n_edges, const uint16_t* uv, const flo
     G[4] += xt[2] * a[0] - xt[0] * a[2];
     G[5] += xt[0] * a[1] - xt[1] * a[0];
     for (int i = 0; i < 3; ++i) b[i] = Tts[i] * a[0] + Tts[4 + i] * a[1] + Tts[8 + i] * a[2];
+    /* joint phase (Eq. 4-5): d rho / d ln f_t, d rho / d ln f_s (both focal lengths of a camera scale
+     * together, f = f0 (1 + gamma)) and d rho / d Z_s of this edge pixel:
+     *   (x, y) - c_t = f_t (X, Y)/Z            ->  d rho / d ln f_t = rho' (dd/dx (x - cx_t) + dd/dy (y - cy_t))
+     *   x_s = Z ((u - cx)/fx, (v - cy)/fy, 1)  ->  d x_s / d ln f_s = (-x_s.x, -x_s.y, 0),  d x_s / d Z = x_s / Z
+     *   and d rho / d x_s = R_ts^T a = b                                                                           */
+    if (J) { J[0] += drho * (ddx * (x - Kt[2]) + ddy * (y - Kt[3])); J[1] -= b[0] * xs[0] + b[1] * xs[1]; }
+    if (dZ) dZ[e] = (b[0] * xs[0] + b[1] * xs[1] + b[2] * xs[2]) / (double)z[e];
     G[6] -= b[0]; G[7] -= b[1]; G[8] -= b[2];
     G[9]  -= xs[1] * b[2] - xs[2] * b[1];
     G[10] -= xs[2] * b[0] - xs[0] * b[2];
@@ -372,6 +393,44 @@ void orc_pair_loss_grad(int W, int H, int n_edges, const uint16_t* uv, const flo
  * edge_off [N+1], uv [E][2], z [E] hold all views' lists; dtf [N][H][W]; K float [N][4]; poses double [N][12].
  * Nullable outputs: pair_G [P][12] (un-normalised sums), near [P][2].
  * ================================================================================================= */
+void orc_pair_loss_grad(int W, int H, int n_edges, const uint16_t* uv, const float* z,
+                        const double Ks[4], const double Kt[4], const double Ts[12], const double Tt[12],
+                        const float* dtf_t, double lambda, double delta, double z_min, int coord_fp32,
+                        double* sum_rho, int32_t* n_valid, double G[12], int32_t near[2]) {
+  orc_pair_loss_grad_joint(W, H, n_edges, uv, z, Ks, Kt, Ts, Tt, dtf_t, lambda, delta, z_min, coord_fp32, sum_rho, n_valid,
+                           G, near, NULL, NULL);
+}
+
+/* Joint-phase gradients of the loss (Eq. 4-5; 64: "in the subsequent joint phase, optimization is extended
+ * to include the depth maps"): with L = (1/P) sum_pairs (1/n_p) sum rho and n_p held fixed as for the poses,
+ *   g_logf[c]  = d L / d ln f_c   (as target and as source; d L / d gamma_c = g_logf[c] / (1 + gamma_c))
+ *   g_depth[e] = d L / d Z of edge-list entry e (all pairs whose source owns e); with Z = Z0 alpha + beta (Eq. 5):
+ *                d L / d alpha = Z0 g_depth, d L / d beta = g_depth.
+ * Serial over pairs in list order (a fixed accumulation order).                                                     */
+void orc_joint_grad(int N, int W, int H, const float* K, const double* poses, const int32_t* edge_off,
+                    const uint16_t* uv, const float* z, const float* dtf, int64_t P, const int32_t* pairs,
+                    double lambda, double delta, double z_min, int coord_fp32, double* g_logf, double* g_depth) {
+  int max_n = 1;
+  for (int i = 0; i < N; ++i) if (edge_off[i + 1] - edge_off[i] > max_n) max_n = edge_off[i + 1] - edge_off[i];
+  double* dZ = (double*)malloc((size_t)max_n * sizeof(double));
+  for (int i = 0; i < N; ++i) g_logf[i] = 0.0;
+  for (int64_t e = 0; e < edge_off[N]; ++e) g_depth[e] = 0.0;
+  for (int64_t p = 0; p < P; ++p) {
+    const int s = pairs[2 * p], t = pairs[2 * p + 1], n = edge_off[s + 1] - edge_off[s];
+    double Ks[4], Kt[4], S, G[12], J[2]; int32_t nv, nr[2];
+    for (int i = 0; i < 4; ++i) { Ks[i] = K[4 * s + i]; Kt[i] = K[4 * t + i]; }
+    orc_pair_loss_grad_joint(W, H, n, uv + 2 * (size_t)edge_off[s], z + edge_off[s], Ks, Kt, poses + 12 * (size_t)s,
+                             poses + 12 * (size_t)t, dtf + (size_t)t * W * H, lambda, delta, z_min, coord_fp32, &S, &nv, G, nr,
+                             J, dZ);
+    if (nv == 0) continue;
+    g_logf[t] += J[0] / nv; g_logf[s] += J[1] / nv;
+    for (int e = 0; e < n; ++e) g_depth[edge_off[s] + e] += dZ[e] / nv;
+  }
+  for (int i = 0; i < N; ++i) g_logf[i] /= (double)P;
+  for (int64_t e = 0; e < edge_off[N]; ++e) g_depth[e] /= (double)P;
+  free(dZ);
+}
+
 void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, const int32_t* edge_off,
                    const uint16_t* uv, const float* z, const float* dtf, int64_t P, const int32_t* pairs,
                    double lambda, double delta, double z_min, int coord_fp32, double* pair_loss,
