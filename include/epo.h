@@ -160,6 +160,19 @@ EPO_API epo_status epo_loss_grad(epo_ctx* ctx, float lambda, float* loss, float*
                          float* grad);
 
 /*
+ * Joint-phase gradients at the CURRENT poses (Eq. 4-5; "in the subsequent joint phase,
+ * optimization is extended to include the depth maps"), same loss, same clamp, n_valid held fixed:
+ *   g_logf [N]         d loss / d ln f_c, both focal lengths of camera c scaled together (Eq. 4: f = f0 (1 + gamma), so
+ *                      d loss / d gamma_c = g_logf[c] / (1 + gamma_c)), as target and as source of its pairs
+ *   g_depth [N][H][W]  d loss / d Z_c(u, v) at the edge pixels of the lists (0 elsewhere); with Eq. 5, Z = Z0 alpha + beta:
+ *                      d loss / d alpha = Z0 g_depth, d loss / d beta = g_depth
+ *   loss [1]           nullable: the loss of this evaluation
+ * Evaluates all pairs (no sub-sampling).  Sums are accumulated with atomics (run-to-run differences at rounding
+ * level).  Does not change poses or optimiser state: this library does not optimise f or Z.
+ */
+EPO_API epo_status epo_loss_grad_joint(epo_ctx* ctx, float lambda, float* loss, float* g_logf, float* g_depth);
+
+/*
  * Run up to n_iters iterations of Alg. 2 on the device without host synchronisation between them:
  *   lambda_s -> loss + gradient -> Adam (lr_s: PAPER.md:121) -> T_c <- Exp(eps_c) T_c
  *   -> theta95^s (Eq. 9-10, 95th percentiles) -> Converged tests (phase 0 -> 1 -> 2).

@@ -128,7 +128,7 @@ epo_status epo_config_default(epo_config* cfg) {
 epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   if (!cfg || !out) return EPO_ERR_INVALID_ARG;
   *out = nullptr;
-  if (cfg->n_views < 2 || cfg->width < 2 || cfg->height < 2 || cfg->width > 65535 || cfg->height > 65535)
+  if (cfg->n_views < 2 || cfg->n_views > 65535 || cfg->width < 2 || cfg->height < 2 || cfg->width > 65535 || cfg->height > 65535)
     return EPO_ERR_INVALID_ARG;
   if (!(cfg->huber_delta > 0.f) || cfg->clamp_steps < 1 || cfg->warmup_steps < 0 || cfg->max_steps <= cfg->warmup_steps ||
       cfg->w1 < 1 || cfg->w2 < 1 || (cfg->dtf_format != 0 && cfg->dtf_format != 1) || cfg->e_max < 0 ||
@@ -402,6 +402,45 @@ epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss
   if (sync) EPO_CUDA(c, cudaStreamSynchronize(st));
   EPO_CUDA(c, cudaGetLastError());
   return EPO_OK;
+}
+
+epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_logf, float* g_depth) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_loss_grad_joint before epo_set_views/epo_set_pairs");
+  if (!g_logf || !g_depth || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_loss_grad_joint: NULL output or negative lambda");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t N = (size_t)c->N, px = N * c->W * c->H;
+  // the evaluation first: per-pair valid counts (and the loss), then the joint pass over the same samples
+  EPO_TRY(epo_launch_fused(c, lambda, false, false));
+  EPO_TRY(epo_launch_finish(c, false, false, false, false));
+  double* d_gf = nullptr; float* d_gf32 = nullptr; float* d_gz = nullptr;
+  const bool gz_dev = is_device_ptr(g_depth);
+  cudaError_t e = epo_dmalloc(c, &d_gf, N * sizeof(double));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &d_gf32, N * sizeof(float));
+  if (e == cudaSuccess && !gz_dev) e = epo_dmalloc(c, &d_gz, px * sizeof(float));
+  float* gz = gz_dev ? g_depth : d_gz;
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_gf, 0, N * sizeof(double), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(gz, 0, px * sizeof(float), st);
+  epo_status rc = e == cudaSuccess ? epo_launch_fused_joint(c, lambda, d_gf, gz)
+                                   : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
+                                              "epo_loss_grad_joint: %s", cudaGetErrorString(e));
+  bool sync = false;
+  if (rc == EPO_OK) {
+    epo_launch_f64_to_f32(st, d_gf, d_gf32, (int64_t)N);
+    c->launches += 1;
+    e = copy_out(g_logf, d_gf32, N * sizeof(float), st, &sync);
+    if (e == cudaSuccess && !gz_dev) e = copy_out(g_depth, d_gz, px * sizeof(float), st, &sync);
+    if (e == cudaSuccess && loss) {
+      epo_launch_f64_to_f32(st, &c->d_state->loss, c->d_out_f, 1);
+      c->launches += 1;
+      e = copy_out(loss, c->d_out_f, sizeof(float), st, &sync);
+    }
+    if (e == cudaSuccess && sync) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_loss_grad_joint: %s", cudaGetErrorString(e));
+  }
+  epo_dfree(c, d_gf); epo_dfree(c, d_gf32); epo_dfree(c, d_gz);
+  return rc;
 }
 
 epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* phase) {

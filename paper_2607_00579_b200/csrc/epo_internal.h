@@ -99,7 +99,7 @@ struct epo_ctx {
   int32_t* d_tgt_off;     // [N+1] CSR by target over canonical ids
   int32_t* d_src_off;     // [N+1]
   int32_t* d_src_inc;     // [P] canonical ids grouped by source, ascending
-  int4* d_work;           // [n_work] {source, target, first point of the chunk (absolute), samples left}, target-major
+  int4* d_work;           // [n_work] {source | target << 16, canonical pair, first point of the chunk (absolute), samples left}, target-major
   int32_t* d_work_off;    // [P+1] first work item of each canonical pair
   std::vector<int32_t> h_pairs;   // user order, for reprojection counting
   // stochastic pair sub-sampling (cfg.pair_budget > 0 and P > budget): rebuilt by k_select_pairs every iteration
@@ -208,6 +208,7 @@ epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_f
                                 long long* d_n);
 // lossgrad.cu
 epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);
+epo_status epo_launch_fused_joint(epo_ctx* ctx, float lambda, double* d_g_logf, float* d_g_depth);   // joint-phase pass
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda, bool gather_only);   // the fused kernel alone (measurement hooks)
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
 epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset);

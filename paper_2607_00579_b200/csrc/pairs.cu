@@ -90,8 +90,9 @@ __global__ void k_chunk_counts(const int2* __restrict__ canon, const int32_t* __
   cnt[p] = (n + chunk - 1) / chunk;
 }
 
-// work item = {source, target, first point of the chunk (absolute index into the point list), samples of the
-// source's list from there on}: the fused kernel needs no other table before it can start loading points
+// work item = {source | target << 16, canonical pair index, first point of the chunk (absolute index into the point
+// list), samples of the source's list from there on}: the fused kernel needs no other table before it can start
+// loading points (N <= 65535 is checked in epo_create)
 __global__ void k_fill_work(const int32_t* __restrict__ work_off, const int2* __restrict__ canon,
                             const int32_t* __restrict__ edge_off, int64_t P, int chunk, int4* __restrict__ work) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -99,7 +100,7 @@ __global__ void k_fill_work(const int32_t* __restrict__ work_off, const int2* __
   const int2 st = canon[p];
   const int e0 = edge_off[st.x], n = edge_off[st.x + 1] - e0;
   int lo = work_off[p], hi = work_off[p + 1];
-  for (int w = lo; w < hi; ++w) work[w] = make_int4(st.x, st.y, e0 + (w - lo) * chunk, n - (w - lo) * chunk);
+  for (int w = lo; w < hi; ++w) work[w] = make_int4(st.x | (st.y << 16), (int)p, e0 + (w - lo) * chunk, n - (w - lo) * chunk);
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -222,14 +222,15 @@ k_edt_cols(const int32_t* __restrict__ g, int W, int H, cudaSurfaceObject_t atla
 // The operation order is the one the fp32-position reading (P1) states.
 // ---------------------------------------------------------------------------------------------
 __global__ void k_make_points(const EdgeRec* __restrict__ rec, const int32_t* __restrict__ off,
-                              const float* __restrict__ K, float4* __restrict__ pts) {
+                              const float* __restrict__ K, int W, float4* __restrict__ pts) {
   const int view = blockIdx.y;
   const int lo = off[view], n = off[view + 1] - lo;
   const float ifx = 1.0f / K[4 * view], ify = 1.0f / K[4 * view + 1], cx = K[4 * view + 2], cy = K[4 * view + 3];
   for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
     const EdgeRec r = rec[lo + e];
     const float u = (float)(r.uv & 0xffffu), v = (float)(r.uv >> 16);
-    pts[lo + e] = make_float4(r.z * ((u - cx) * ifx), r.z * ((v - cy) * ify), r.z, 0.f);
+    pts[lo + e] = make_float4(r.z * ((u - cx) * ifx), r.z * ((v - cy) * ify), r.z,
+                              __int_as_float((int)(r.uv >> 16) * W + (int)(r.uv & 0xffffu)));   // .w: pixel index (joint phase)
   }
 }
 
@@ -286,7 +287,7 @@ __global__ void k_tile_points(const uint8_t* __restrict__ edges, const float* __
     if (f) {
       const float z = depth[idx];
       pts[pos + __popc(m & ((1u << lane) - 1u))] =
-          make_float4(z * (((float)u - cx) * ifx), z * (((float)v - cy) * ify), z, 0.f);
+          make_float4(z * (((float)u - cx) * ifx), z * (((float)v - cy) * ify), z, __int_as_float(v * W + u));   // .w: pixel index
     }
     pos += __popc(m);
   }
@@ -459,7 +460,7 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
     int max_n = 1;
     for (int i = 0; i < ctx->N; ++i) max_n = h_off[i + 1] - h_off[i] > max_n ? h_off[i + 1] - h_off[i] : max_n;
     dim3 grid((max_n + 255) / 256, ctx->N);
-    k_make_points<<<grid, 256, 0, st>>>(d_rec, d_off, d_K, pts);
+    k_make_points<<<grid, 256, 0, st>>>(d_rec, d_off, d_K, ctx->W, pts);
     ctx->launches += 1;
     e = cudaGetLastError();
   } else {

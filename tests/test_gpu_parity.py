@@ -328,6 +328,39 @@ def test_early_stop_parity():
     e.destroy()
 
 
+# ------------------------------------------------------------------------------ joint-phase gradients
+@pytest.mark.parametrize("name", ["tiny", "room6", "orbit8"])
+@pytest.mark.parametrize("lam", [10.0, 20.0])
+def test_joint_phase_gradients_parity(name, lam):
+    """epo_loss_grad_joint (Eq. 4-5): d L / d ln f per camera and d L / d Z per edge pixel against the
+    oracle's fp32-position variant at 1e-4 relative (per camera; per view in the 2-norm and per entry with a floor),
+    exact zeros off the edge lists, and no side effect on the ordinary evaluation."""
+    sc = scene(name)
+    e = make_ctx(sc)
+    prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
+    poses = sc.poses_init.astype(np.float64)
+    before = e.loss_grad(lam)
+    got = e.loss_grad_joint(lam)
+    gf, gz = oracle.joint_grad(prob, poses, sc.pairs, lam, z_min=Z_MIN, coord_fp32=1)
+    assert abs(got["loss"] - before["loss"]) <= 1e-6 * abs(before["loss"])
+    assert np.all(np.abs(got["g_logf"] - gf) <= 1e-4 * np.abs(gf) + 1e-9), (got["g_logf"], gf)
+    mask = np.zeros(sc.depth.shape, bool)
+    worst = 0.0
+    for i in range(sc.n_views):
+        lo, hi = prob.edge_off[i], prob.edge_off[i + 1]
+        u, v = prob.uv[lo:hi, 0].astype(int), prob.uv[lo:hi, 1].astype(int)
+        mask[i, v, u] = True
+        mine, ref = got["g_depth"][i, v, u].astype(np.float64), gz[lo:hi]
+        assert np.linalg.norm(mine - ref) <= 1e-4 * np.linalg.norm(ref) + 1e-12
+        assert np.all(np.abs(mine - ref) <= 1e-4 * np.abs(ref) + 1e-5 * np.abs(ref).max())
+        worst = max(worst, np.linalg.norm(mine - ref) / max(np.linalg.norm(ref), 1e-30))
+    assert not got["g_depth"][~mask].any()
+    print(f"{name} lam={lam}: d/dlnf rel err {np.max(np.abs(got['g_logf'] - gf) / np.abs(gf)):.2e}, d/dZ per-view rel err {worst:.2e}")
+    after = e.loss_grad(lam)
+    assert after["loss"] == before["loss"] and np.array_equal(after["grad"], before["grad"])
+    e.destroy()
+
+
 # ---------------------------------------------------------------------------------- edge extraction
 def _test_images(n, H, W, seed):
     """Seeded 8-bit images with edges of every orientation and strength: rectangles and discs of random grey levels
