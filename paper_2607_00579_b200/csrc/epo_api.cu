@@ -1,5 +1,6 @@
 // Host side of the C ABI declared in include/epo.h: argument validation, host/device pointer
 // marshalling, device-memory ownership and launch sequencing.  No arithmetic of the method lives here.
+#include <algorithm>
 #include <chrono>
 #include <cmath>
 #include <cstdlib>
@@ -312,8 +313,13 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   epo_dfree(c, d_user);
   double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
   uint8_t* sflag = nullptr; int32_t* swork = nullptr; int32_t* sinfo = nullptr; int32_t* sscr = nullptr;
-  if (rc == EPO_OK && c->cfg.pair_budget > 0 && P > c->cfg.pair_budget && P > epo_select_max_pairs())
-    rc = epo_fail(c, EPO_ERR_UNSUPPORTED, "pair sub-sampling supports at most %lld pairs", (long long)epo_select_max_pairs());
+  if (rc == EPO_OK && c->cfg.pair_budget > 0 && P > c->cfg.pair_budget) {
+    // k_select_pairs meets at grid barriers: all its CTAs (4096 pairs each) must be resident at once, one per SM
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->cfg.device);
+    const int64_t max_pairs = std::min<int64_t>(epo_select_max_pairs(), (int64_t)sms * 4096);
+    if (P > max_pairs) rc = epo_fail(c, EPO_ERR_UNSUPPORTED, "pair sub-sampling supports at most %lld pairs", (long long)max_pairs);
+  }
   if (rc == EPO_OK) {
     e = epo_dmalloc(c, &sscr, (size_t)kSelScrInts * sizeof(int32_t));
     if (e == cudaSuccess) e = cudaMemsetAsync(sscr, 0, (size_t)kSelScrInts * sizeof(int32_t), st);

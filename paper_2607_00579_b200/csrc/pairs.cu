@@ -374,7 +374,9 @@ epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override, bool gated, 
   lc.blockDim = dim3(kSelThreads); lc.dynamicSmemBytes = 0; lc.stream = ctx->stream;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
-  lc.attrs = at; lc.numAttrs = (ctx->pdl && gated) ? 1 : 0;
+  // programmatic dependent launch only inside the loop and only when the static lists are not the work of the
+  // kernels just before this one (the same rule as for the fused kernel)
+  lc.attrs = at; lc.numAttrs = (ctx->pdl && gated && !ctx->static_dirty) ? 1 : 0;
   EPO_CUDA(ctx, cudaLaunchKernelEx(&lc, k_select_pairs, p));
   ctx->launches += 1;
   return EPO_OK;
