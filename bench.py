@@ -155,7 +155,7 @@ def cpu_baseline(sc, seconds_target=12.0):
     while True:
         opt.run(1); iters += 1
         dt = time.time() - t0
-        if dt >= seconds_target or iters >= 50:
+        if dt >= seconds_target or iters >= 400:
             break
     return dict(value=reproj * iters / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
                 sample=f"{iters} whole iterations (all {len(sc.pairs)} pairs, {reproj} reprojections each) in {dt:.1f} s; "

@@ -17,9 +17,10 @@
  *   - pixel (u,v) is the sample position; DTF[v][u] is the field value AT (u,v)        (reading S2)
  *   - pose perturbation: T <- Exp(eps) T, eps = (v, w), translation part first          (reading S9)
  *
- * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): Z0..Z10 of SURVEY.md §8(c).  Numerical VALUES of
- * the loss/gradient on realistic scenes are "parity unpinned" beyond those checks (nothing in the
- * paper prints one).
+ * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): Z0..Z11 of SURVEY.md §8(c) for the loop; S0..S3 (pair
+ * sub-sampling), V1..V5 (viewgraph estimation), K1..K5 (Canny), J1..J3 (joint-phase gradients): DESIGN.md §5.
+ * Numerical VALUES of the loss/gradient on realistic scenes are "parity unpinned" beyond those checks (nothing in
+ * the paper prints one).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC -o liboracle.so epo_oracle.c -lm
  */
