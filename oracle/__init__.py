@@ -90,6 +90,9 @@ def lib():
         L.orc_theta95.restype = C.c_double
         L.orc_round_to_half.restype = C.c_float
         L.orc_round_to_half.argtypes = [C.c_float]
+        L.orc_adamw.argtypes = [C.c_int64, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                C.POINTER(C.c_double), C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double,
+                                C.c_double]
         L.orc_converged_loss.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_int, C.c_double]
         L.orc_converged.argtypes = [C.POINTER(C.c_double), C.c_int, C.c_int, C.c_double, C.c_int]
         L.orc_adam.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
@@ -400,6 +403,15 @@ def adam(g, m, v, s, lr, beta1=0.9, beta2=0.999, adam_eps=1e-8):
     lib().orc_adam(g.size, _p(g, C.c_double), _p(m, C.c_double), _p(v, C.c_double), s, lr, beta1, beta2,
                    adam_eps, _p(out, C.c_double))
     return out
+
+
+def adamw(p, g, m, v, t, lr, beta1=0.9, beta2=0.999, adam_eps=1e-8, wd=0.01, p_id=0.0):
+    """In-place AdamW step number t (1-based) of one variable group, decay towards p_id (reading J6)."""
+    g = _d(g)
+    for a in (p, m, v):
+        assert a.dtype == np.float64 and a.flags.c_contiguous and a.size == g.size
+    lib().orc_adamw(C.c_int64(g.size), _p(p, C.c_double), _p(g, C.c_double), _p(m, C.c_double), _p(v, C.c_double), int(t),
+                    C.c_double(lr), C.c_double(beta1), C.c_double(beta2), C.c_double(adam_eps), C.c_double(wd), C.c_double(p_id))
 
 
 # ---------------------------------------------------------------------------------------------- O8

@@ -779,6 +779,23 @@ void orc_adam(int n, const double* g, double* m, double* v, int s, double lr, do
   }
 }
 
+/* AdamW [28] on the joint phase's variables ("All parameters are optimized with the AdamW optimizer with
+ * beta1 = 0.9, beta2 = 0.999, and weight decay 0.01"), in place: decoupled decay first, then the Adam step,
+ *   p <- p - lr wd (p - p_id) ;  m, v as in Adam ;  p <- p - lr (m / c1) / (sqrt(v / c2) + eps),  c_k = 1 - beta_k^t
+ * with t the 1-based count of steps THIS variable group has taken.  p_id is the variable's identity value (gamma: 0,
+ * alpha: 1, beta: 0; "initialized to their identity values"): the decay pulls towards it (reading J6;
+ * for p_id = 0 this is torch.optim.AdamW exactly).                                                                  */
+void orc_adamw(int64_t n, double* p, const double* g, double* m, double* v, int t, double lr, double beta1, double beta2,
+               double adam_eps, double wd, double p_id) {
+  const double c1 = 1.0 - pow(beta1, (double)t), c2 = 1.0 - pow(beta2, (double)t);
+  for (int64_t i = 0; i < n; ++i) {
+    p[i] -= lr * wd * (p[i] - p_id);
+    m[i] = beta1 * m[i] + (1.0 - beta1) * g[i];
+    v[i] = beta2 * v[i] + (1.0 - beta2) * g[i] * g[i];
+    p[i] -= lr * (m[i] / c1) / (sqrt(v[i] / c2) + adam_eps);
+  }
+}
+
 /* =================================================================================================
  * O8  Pose change and the windowed two-phase stopping rule
  * ================================================================================================= */

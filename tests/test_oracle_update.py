@@ -208,3 +208,24 @@ def test_Z11_loss_based_stopping_rule_on_hand_made_traces():
     assert oracle.converged_loss(np.array([1.0, 1.0 + 4.9e-4]), 1, 1, 5e-4)
     assert not oracle.converged_loss(np.array([1.0, 1.0 + 5.0e-4 + 1e-12]), 1, 1, 5e-4)       # strict
     assert oracle.converged_loss(np.zeros(5), 4, 3, 1e-9) and not oracle.converged_loss(np.array([0.0, 1e-30]), 1, 1, 0.5)
+
+
+def test_Z12_adamw_matches_torch_optim_adamw_and_decays_towards_the_identity():
+    rng = SplitMix64(12)
+    n, steps = 25, 30
+    p = rng.normal(n); m = np.zeros(n); v = np.zeros(n)
+    tp = torch.tensor(p.copy(), dtype=torch.float64, requires_grad=True)
+    opt = torch.optim.AdamW([tp], lr=1.0, betas=(0.9, 0.999), eps=1e-8, weight_decay=0.01)
+    q = p + 1.0; mq = np.zeros(n); vq = np.zeros(n)               # the same run shifted by the identity value 1
+    for t in range(1, steps + 1):
+        g = rng.normal(n) * (10.0 ** float(rng.uniform(1, -3, 2)[0]))
+        lr = oracle.lr_schedule(t + 30, oracle.Config())
+        oracle.adamw(p, g, m, v, t, lr)
+        oracle.adamw(q, g, mq, vq, t, lr, p_id=1.0)
+        for grp in opt.param_groups:
+            grp["lr"] = lr
+        tp.grad = torch.from_numpy(g.copy()); opt.step()
+        assert np.max(np.abs(tp.detach().numpy() - p)) < 1e-12
+        assert np.max(np.abs((q - 1.0) - p)) < 1e-12
+    z = np.full(3, 5.0); oracle.adamw(z, np.zeros(3), np.zeros(3), np.zeros(3), 1, 0.1, wd=0.5, p_id=1.0)
+    assert np.allclose(z, 5.0 - 0.1 * 0.5 * 4.0)                  # zero gradient: only the decay towards 1 acts
