@@ -86,6 +86,13 @@ typedef struct {
                                        The first stage (phase 0 -> 1) is pose-based in both.                        */
   int32_t w_loss;                   /* 100                                                           */
   float   eps_loss;                 /* 5e-4                                                          */
+  int32_t joint_phase;              /* 0 (default): epo_step optimises the poses only.  1: also the joint phase's variables
+                                       (PAPER.md:64, 78-87): a focal scale per camera, f = f0 (1 + gamma) (Eq. 4), from the
+                                       first iteration, and the affine depth Z = Z0 alpha + beta (Eq. 5) of every listed
+                                       edge pixel in iterations that start in phase >= 1; AdamW with the loop's learning
+                                       rate and weight_decay towards the identity.  An iteration then runs the fused
+                                       kernel twice (loss + pose gradient, then the joint gradients).                  */
+  float   weight_decay;             /* 0.01                                                          */
 } epo_config;
 
 /* Fill *cfg with the paper's hyper-parameters (n_views/width/height = 0, device 0, stream NULL). */
@@ -192,6 +199,11 @@ EPO_API epo_status epo_get_poses_f64(epo_ctx* ctx, double* poses);
 /* Replace the current poses ([N][12] fp32; NULL = the poses given to epo_set_views) and reset Adam
  * moments, step counter, phase and traces.  Preprocessing and pair lists are kept. */
 EPO_API epo_status epo_reset(epo_ctx* ctx, const float* poses);
+
+/* Joint-phase variables (cfg.joint_phase = 1), all nullable, host or device pointers, fp64: gamma [N]; alpha and beta
+ * as [N][H][W] maps (1 and 0 off the edge lists).  The current intrinsics are K0 (1 + gamma), the current depth of a
+ * listed edge pixel is Z0 alpha + beta. */
+EPO_API epo_status epo_get_joint_variables(epo_ctx* ctx, double* gamma, double* alpha, double* beta);
 
 /* ---- introspection (used by the parity tests and the benchmark) ------------------------------- */
 /* The subset of the pair list that iteration `step` of epo_step evaluates (stochastic viewgraph sub-sampling,

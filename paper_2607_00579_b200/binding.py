@@ -21,7 +21,7 @@ _STATUS = {0: "EPO_OK", 1: "EPO_ERR_INVALID_ARG", 2: "EPO_ERR_BAD_STATE", 3: "EP
            4: "EPO_ERR_CUDA", 5: "EPO_ERR_UNSUPPORTED"}
 
 # every symbol include/epo.h declares (tests check that the library exports exactly these)
-SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_extract_edges", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad", "epo_loss_grad_joint",
+SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_extract_edges", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad", "epo_loss_grad_joint", "epo_get_joint_variables",
            "epo_step", "epo_get_poses", "epo_get_poses_f64", "epo_reset", "epo_get_edge_counts", "epo_get_edge_list",
            "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel", "epo_time_gather_ceiling",
            "epo_last_error", "epo_version"]
@@ -36,7 +36,7 @@ class EpoConfig(C.Structure):
                 ("early_stop", C.c_int32), ("dtf_format", C.c_int32), ("e_max", C.c_int32), ("z_min", C.c_float),
                 ("device", C.c_int32), ("stream", C.c_void_p), ("pair_budget", C.c_int32),
                 ("subsample_seed", C.c_uint64), ("stop_rule", C.c_int32), ("w_loss", C.c_int32),
-                ("eps_loss", C.c_float)]
+                ("eps_loss", C.c_float), ("joint_phase", C.c_int32), ("weight_decay", C.c_float)]
 
 
 class EpoError(RuntimeError):
@@ -60,6 +60,7 @@ def load_library() -> C.CDLL:
     L.epo_build_viewgraph.argtypes = [vp, C.c_int32, C.c_float, C.c_float, i32p, C.c_int64, C.POINTER(C.c_int64), i32p]
     L.epo_loss_grad.argtypes = [vp, C.c_float, f32p, f32p, i32p, f32p]
     L.epo_loss_grad_joint.argtypes = [vp, C.c_float, f32p, f32p, f32p]
+    L.epo_get_joint_variables.argtypes = [vp, vp, vp, vp]
     L.epo_step.argtypes = [vp, C.c_int32, i32p, i32p]
     L.epo_get_poses.argtypes = [vp, f32p]
     L.epo_get_poses_f64.argtypes = [vp, vp]
@@ -189,6 +190,12 @@ class Epo:
         gz = np.zeros((self.N, self.H, self.W), np.float32)
         self._check(lib().epo_loss_grad_joint(self._h, C.c_float(lam), _ptr(loss), _ptr(gf), _ptr(gz)), "epo_loss_grad_joint")
         return dict(loss=float(loss[0]), g_logf=gf, g_depth=gz)
+
+    def get_joint_variables(self):
+        """(gamma [N], alpha [N][H][W], beta [N][H][W]) as float64 numpy arrays (cfg.joint_phase = 1)."""
+        g = np.zeros(self.N); a = np.zeros((self.N, self.H, self.W)); b = np.zeros((self.N, self.H, self.W))
+        self._check(lib().epo_get_joint_variables(self._h, _ptr(g), _ptr(a), _ptr(b)), "epo_get_joint_variables")
+        return g, a, b
 
     def step(self, n_iters: int, sync: bool = True):
         """Runs up to n_iters iterations; returns (iters_done, phase) if sync else None."""

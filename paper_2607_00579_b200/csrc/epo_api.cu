@@ -62,6 +62,7 @@ void free_views(epo_ctx* c) {
   epo_dfree(c, c->d_edge_off); epo_dfree(c, c->d_edges); epo_dfree(c, c->d_pts); epo_dfree(c, c->d_depth);
   c->d_depth = nullptr;
   epo_free_atlas(&c->atlas);
+  epo_joint_free(c);
   c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_pts = nullptr;
   c->have_views = false;
 }
@@ -93,8 +94,9 @@ int choose_chunk(const epo_ctx* c, const std::vector<int32_t>& pairs, int64_t P)
   return (int)passes * kLgPass;
 }
 
-epo_status reset_optimiser(epo_ctx* c) {
+epo_status reset_optimiser(epo_ctx* c, bool joint = true) {
   cudaStream_t st = c->stream;
+  if (joint) EPO_TRY(epo_joint_reset(c));
   EPO_CUDA(c, cudaMemsetAsync(c->d_m, 0, (size_t)c->N * 6 * sizeof(double), st));
   EPO_CUDA(c, cudaMemsetAsync(c->d_v, 0, (size_t)c->N * 6 * sizeof(double), st));
   EPO_CUDA(c, cudaMemsetAsync(c->d_state, 0, sizeof(DevState), st));
@@ -123,6 +125,7 @@ epo_status epo_config_default(epo_config* cfg) {
   cfg->z_min = 1e-6f; cfg->device = 0; cfg->stream = nullptr;
   cfg->pair_budget = 0; cfg->subsample_seed = 0;
   cfg->stop_rule = 0; cfg->w_loss = 100; cfg->eps_loss = 5e-4f;
+  cfg->joint_phase = 0; cfg->weight_decay = 0.01f;
   return EPO_OK;
 }
 
@@ -133,7 +136,8 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
     return EPO_ERR_INVALID_ARG;
   if (!(cfg->huber_delta > 0.f) || cfg->clamp_steps < 1 || cfg->warmup_steps < 0 || cfg->max_steps <= cfg->warmup_steps ||
       cfg->w1 < 1 || cfg->w2 < 1 || (cfg->dtf_format != 0 && cfg->dtf_format != 1) || cfg->e_max < 0 ||
-      cfg->pair_budget < 0 || (cfg->stop_rule != 0 && cfg->stop_rule != 1) || cfg->w_loss < 1 || !(cfg->eps_loss >= 0.f) || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
+      cfg->pair_budget < 0 || (cfg->joint_phase != 0 && cfg->joint_phase != 1) || !(cfg->weight_decay >= 0.f) ||
+      (cfg->joint_phase && cfg->pair_budget > 0) || (cfg->stop_rule != 0 && cfg->stop_rule != 1) || cfg->w_loss < 1 || !(cfg->eps_loss >= 0.f) || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
     return EPO_ERR_INVALID_ARG;
   epo_ctx* c = new (std::nothrow) epo_ctx();
   if (!c) return EPO_ERR_OUT_OF_MEMORY;
@@ -264,7 +268,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
   }
-  if (rc == EPO_OK) rc = reset_optimiser(c);
+  if (rc == EPO_OK) rc = reset_optimiser(c, false);
   e = cudaStreamSynchronize(st);
   if (rc == EPO_OK && e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_set_views: %s", cudaGetErrorString(e));
   tr.mark("points + drain");
@@ -282,6 +286,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff;
   c->d_pts = pts; c->atlas = atlas; c->d_depth = d_depth;
   c->have_views = true; c->static_dirty = true;
+  EPO_TRY(epo_joint_alloc(c));                      // joint loop: variables at the identity, Z0 and K0 kept
   tr.mark("free temporaries");
   return EPO_OK;
 }
@@ -428,7 +433,7 @@ epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_l
   float* gz = gz_dev ? g_depth : d_gz;
   if (e == cudaSuccess) e = cudaMemsetAsync(d_gf, 0, N * sizeof(double), st);
   if (e == cudaSuccess) e = cudaMemsetAsync(gz, 0, px * sizeof(float), st);
-  epo_status rc = e == cudaSuccess ? epo_launch_fused_joint(c, lambda, d_gf, gz)
+  epo_status rc = e == cudaSuccess ? epo_launch_fused_joint(c, lambda, d_gf, gz, false)
                                    : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
                                               "epo_loss_grad_joint: %s", cudaGetErrorString(e));
   bool sync = false;
@@ -449,6 +454,31 @@ epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_l
   return rc;
 }
 
+epo_status epo_get_joint_variables(epo_ctx* c, double* gamma, double* alpha, double* beta) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views || !c->cfg.joint_phase) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_joint_variables needs cfg.joint_phase and epo_set_views");
+  if ((alpha == nullptr) != (beta == nullptr)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_joint_variables: alpha and beta come together");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t N = (size_t)c->N, px = N * c->W * c->H;
+  double *d_a = nullptr, *d_b = nullptr;
+  const bool maps = alpha != nullptr, dev = maps && is_device_ptr(alpha) && is_device_ptr(beta);
+  cudaError_t e = cudaSuccess;
+  if (maps && !dev) { e = epo_dmalloc(c, &d_a, px * sizeof(double)); if (e == cudaSuccess) e = epo_dmalloc(c, &d_b, px * sizeof(double)); }
+  epo_status rc = e == cudaSuccess ? epo_joint_export(c, nullptr, maps ? (dev ? alpha : d_a) : nullptr, maps ? (dev ? beta : d_b) : nullptr)
+                                   : epo_fail(c, EPO_ERR_OUT_OF_MEMORY, "epo_get_joint_variables: %s", cudaGetErrorString(e));
+  bool sync = false;
+  if (rc == EPO_OK && gamma) e = copy_out(gamma, c->d_gamma, N * sizeof(double), st, &sync);
+  if (rc == EPO_OK && e == cudaSuccess && maps && !dev) {
+    e = copy_out(alpha, d_a, px * sizeof(double), st, &sync);
+    if (e == cudaSuccess) e = copy_out(beta, d_b, px * sizeof(double), st, &sync);
+  }
+  if (e == cudaSuccess && sync) e = cudaStreamSynchronize(st);
+  if (rc == EPO_OK && e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_get_joint_variables: %s", cudaGetErrorString(e));
+  epo_dfree(c, d_a); epo_dfree(c, d_b);
+  return rc;
+}
+
 epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* phase) {
   if (!c) return EPO_ERR_INVALID_ARG;
   if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_step before epo_set_views/epo_set_pairs");
@@ -460,6 +490,15 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
     if (c->subsample) EPO_TRY(epo_launch_select_pairs(c, -1, true, true));
     EPO_TRY(epo_launch_fused(c, -1.0f, true, c->subsample));
     EPO_TRY(epo_launch_finish(c, true, true, i == 0, c->subsample));
+    if (c->cfg.joint_phase) {
+      // the joint gradients at the state this iteration's loss was evaluated at, then AdamW on gamma / alpha / beta
+      // and the new intrinsics and points (all three self-gated by DevState.joint_pending)
+      EPO_CUDA(c, cudaMemsetAsync(c->d_glogf, 0, (size_t)c->N * sizeof(double), st));
+      EPO_CUDA(c, cudaMemsetAsync(c->d_gz, 0, (size_t)c->N * c->W * c->H * sizeof(float), st));
+      EPO_TRY(epo_launch_fused_joint(c, -1.0f, c->d_glogf, c->d_gz, true));
+      EPO_TRY(epo_launch_joint_update(c));
+      c->static_dirty = true;                       // the points were rewritten: the next fused launch is serialised
+    }
   }
   bool sync = false;
   if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));

@@ -48,6 +48,9 @@ struct DevState {
   int32_t phase;       // 0, 1, 2 (Alg. 2 l.13-17)
   int32_t stopped;     // step >= max_steps, or early_stop && phase == 2
   int32_t iters_done;  // iterations executed since the last epo_step began
+  int32_t phase_prev;  // joint loop: phase at the START of the iteration k_finish has just completed
+  int32_t joint_pending;   // joint loop: an iteration has completed and its joint pass / variable update are due
+  int32_t phase1_step; // joint loop: iteration index at which phase 0 -> 1 happened (depth steps from the next one)
   int32_t ticket;      // CTAs of k_finish that have finished (the last one runs the serial tail and re-zeroes it)
   int32_t pad_;
   double loss;         // loss of the last evaluation
@@ -86,6 +89,14 @@ struct epo_ctx {
   double* d_poses;        // [N][12] current (fp64: T_ts is formed without fp32 cancellation)
   double* d_poses_next;   // [N][12] poses after the update in flight (published by the last CTA of k_finish)
   double* d_poses_init;   // [N][12] as given to epo_set_views / epo_reset
+  // joint loop (cfg.joint_phase): focal scale gamma per camera, depth affine (alpha, beta) per point
+  double* d_poses_prev;   // [N][12] poses at the start of the iteration just completed (the joint pass evaluates there)
+  float* d_K0;            // [N][4] intrinsics as given
+  double* d_gamma;        // [3][N] gamma, Adam m, v
+  double* d_ab;           // [3][E][2] (alpha, beta), Adam m, v, point order
+  float* d_z0;            // [E] depth as given, point order
+  float* d_gz;            // [N][H][W] d L / d Z map of the joint pass
+  double* d_glogf;        // [N] d L / d ln f
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
   float* d_depth;         // [N][H][W] the depth maps as given (kept for epo_build_viewgraph)
@@ -203,12 +214,18 @@ int64_t epo_select_max_pairs(void);
 epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override /* < 0: device step */, bool gated, bool build_work);
 // canny.cu: edge maps (1 / 0) of [N][H][W] 8-bit images, device pointers
 epo_status epo_run_canny(epo_ctx* ctx, const uint8_t* d_img, int low, int high, uint8_t* d_edges);
+// joint.cu: the joint loop's variable update (AdamW on gamma, alpha, beta; new K and points) and its state
+epo_status epo_joint_alloc(epo_ctx* ctx);              // after the points exist (epo_set_views)
+void epo_joint_free(epo_ctx* ctx);
+epo_status epo_joint_reset(epo_ctx* ctx);              // identity variables, zero moments, K and points as given
+epo_status epo_launch_joint_update(epo_ctx* ctx);      // gated by DevState.joint_pending
+epo_status epo_joint_export(epo_ctx* ctx, double* d_gamma_out, double* d_alpha_map, double* d_beta_map);
 // viewgraph.cu: cycle counts of all ordered pairs + ordered emission of the valid pairs
 epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_frac, int2* d_counts, int2* d_pairs,
                                 long long* d_n);
 // lossgrad.cu
 epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);
-epo_status epo_launch_fused_joint(epo_ctx* ctx, float lambda, double* d_g_logf, float* d_g_depth);   // joint-phase pass
+epo_status epo_launch_fused_joint(epo_ctx* ctx, float lambda, double* d_g_logf, float* d_g_depth, bool in_loop);   // joint-phase pass
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda, bool gather_only);   // the fused kernel alone (measurement hooks)
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
 epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset);

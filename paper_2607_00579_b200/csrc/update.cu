@@ -26,7 +26,7 @@ struct FinParams {
   int32_t* pair_valid;
   double *grad, *loss_part;
   // optimiser state
-  double *poses, *poses_next;
+  double *poses, *poses_next, *poses_prev /* nullable */;
   double *m, *v, *dR, *dt, *theta, *loss_trace;
   DevState* state;
   int N;
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   cudaTriggerProgrammaticLaunchCompletion();       // the next fused kernel may start its own static prologue
   cudaGridDependencySynchronize();                 // partial sums, poses and the control block are final now
   if (p.gated && st->stopped) {
-    if (p.call_first && blockIdx.x == 0 && threadIdx.x == 0) st->iters_done = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { if (p.call_first) st->iters_done = 0; st->joint_pending = 0; }
     return;
   }
   const double* Pc = p.poses + 12 * (size_t)c;
@@ -309,7 +309,10 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     sdR[i] = __ldcg(p.dR + i); sdt[i] = __ldcg(p.dt + i);
     lv += __ldcg(p.loss_part + i);
   }
-  for (int i = tid; i < 12 * N; i += kFinThreads) p.poses[i] = __ldcg(p.poses_next + i);
+  for (int i = tid; i < 12 * N; i += kFinThreads) {
+    if (p.poses_prev) p.poses_prev[i] = p.poses[i];
+    p.poses[i] = __ldcg(p.poses_next + i);
+  }
   const double loss = block_sum(lv, &sg[0][0]) / (double)p.P;     // (contains the barrier that publishes sdR / sdt)
   // 95th percentiles, linear interpolation at rank 0.95 (N-1) (reading S12)
   const double rank = 95.0 / 100.0 * (double)(N - 1);
@@ -322,6 +325,7 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   const double t95 = (k0 + 1 < N) ? sel[2] + fr * (sel[3] - sel[2]) : sel[2];
   const double th = r95 > t95 ? r95 : t95;
   int phase = st->phase;
+  const int phase0 = phase;
   if (phase == 0) { if (converged(p.theta, th, s, p.w1, p.eps1, p.smooth)) phase = 1; }
   else if (phase == 1) {
     if (p.stop_rule == 1 ? converged_loss(p.loss_trace, loss, s, p.w_loss, p.eps_loss)
@@ -332,6 +336,8 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     p.loss_trace[s] = loss;
     st->loss = loss;
     st->phase = phase;
+    st->phase_prev = phase0; st->joint_pending = 1;
+    if (phase0 == 0 && phase == 1) st->phase1_step = s;
     st->step = s + 1;
     st->iters_done = p.call_first ? 1 : st->iters_done + 1;
     st->stopped = (s + 1 >= p.max_steps) || (p.early_stop && phase == 2);
@@ -375,7 +381,7 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   p.pairs = ctx->d_pairs; p.tgt_off = ctx->d_tgt_off; p.src_off = ctx->d_src_off; p.src_inc = ctx->d_src_inc;
   p.work_off = ctx->d_work_off; p.part = ctx->d_part; p.pair_loss = ctx->d_pair_loss; p.pair_valid = ctx->d_pair_valid;
   p.grad = ctx->d_grad; p.loss_part = ctx->d_loss_part;
-  p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.m = ctx->d_m; p.v = ctx->d_v;
+  p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.poses_prev = ctx->cfg.joint_phase ? ctx->d_poses_prev : nullptr; p.m = ctx->d_m; p.v = ctx->d_v;
   p.dR = ctx->d_dR; p.dt = ctx->d_dt; p.theta = ctx->d_theta; p.loss_trace = ctx->d_loss_trace;
   p.state = ctx->d_state; p.N = ctx->N;
   p.P = subset ? (int64_t)ctx->cfg.pair_budget : ctx->P;     // the mean runs over the pairs that were evaluated

@@ -361,6 +361,74 @@ def test_joint_phase_gradients_parity(name, lam):
     e.destroy()
 
 
+def test_joint_loop_every_iteration_matches_the_oracle():
+    """cfg.joint_phase = 1: focal scale from the first iteration, affine depth of the listed
+    edge pixels from the first iteration that starts in phase 1, AdamW towards the identity.  Lock-step: at every
+    iteration the oracle restarts from the GPU's own state (poses, gamma, alpha, beta), evaluates loss, pose gradient
+    and joint gradients with its own routines, steps with its own Adam / AdamW moments, and every variable is compared."""
+    import copy
+    sc = scene("room6")
+    kw = dict(early_stop=0, joint_phase=1, w1=6, eps1=5.0)            # phase 1 after a handful of iterations
+    e = make_ctx(sc, **kw)
+    ocfg = oracle_config(coord_fp32=1, early_stop=0, w1=6, eps1=float(np.float32(5.0)))
+    prob0 = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
+    N, E = sc.n_views, int(prob0.edge_off[-1])
+    view = np.repeat(np.arange(N), np.diff(prob0.edge_off)); uu = prob0.uv[:, 0].astype(int); vv = prob0.uv[:, 1].astype(int)
+    m = np.zeros((N, 6)); v = np.zeros((N, 6))
+    mg = np.zeros(N); vg = np.zeros(N); ma = np.zeros(E); va = np.zeros(E); mb = np.zeros(E); vb = np.zeros(E)
+    poses = e.get_poses_f64(); gamma, amap, bmap = e.get_joint_variables()
+    assert not gamma.any() and np.all(amap == 1.0) and not bmap.any()
+    thetas = []; phase = 0; t_depth = 0; worst = dict(rot=0.0, tr=0.0, loss=0.0, gamma=0.0, alpha=0.0, beta=0.0)
+    wd = float(np.float32(0.01))
+    for k in range(24):
+        alpha, beta = amap[view, vv, uu].copy(), bmap[view, vv, uu].copy()
+        prob = copy.copy(prob0)
+        prob.K = prob0.K.copy()
+        prob.K[:, 0] = (prob0.K[:, 0].astype(np.float64) * (1.0 + gamma)).astype(np.float32)
+        prob.K[:, 1] = (prob0.K[:, 1].astype(np.float64) * (1.0 + gamma)).astype(np.float32)
+        prob.z = (prob0.z.astype(np.float64) * alpha + beta).astype(np.float32)
+        lam, lr = oracle.lam_schedule(k, ocfg), oracle.lr_schedule(k, ocfg)
+        ref = oracle.loss_grad(prob, poses, sc.pairs, lam, z_min=Z_MIN, coord_fp32=1)
+        gf, gz = oracle.joint_grad(prob, poses, sc.pairs, lam, z_min=Z_MIN, coord_fp32=1)
+        inc = oracle.adam(ref["grad"].reshape(-1), m.reshape(-1), v.reshape(-1), k, lr, ocfg.beta1, ocfg.beta2, ocfg.adam_eps).reshape(N, 6)
+        pred = np.stack([oracle.se3_compose(oracle.se3_exp(inc[c]), poses[c]) for c in range(N)])
+        g_pred = gamma.copy()
+        oracle.adamw(g_pred, gf / (1.0 + gamma), mg, vg, k + 1, lr, ocfg.beta1, ocfg.beta2, ocfg.adam_eps, wd, 0.0)
+        a_pred, b_pred = alpha.copy(), beta.copy()
+        if phase >= 1:                                                # the iteration starts in phase 1: depth steps
+            t_depth += 1
+            oracle.adamw(a_pred, prob0.z.astype(np.float64) * gz, ma, va, t_depth, lr, ocfg.beta1, ocfg.beta2, ocfg.adam_eps, wd, 1.0)
+            oracle.adamw(b_pred, gz, mb, vb, t_depth, lr, ocfg.beta1, ocfg.beta2, ocfg.adam_eps, wd, 0.0)
+        done, gphase = e.step(1)
+        assert done == 1
+        new = e.get_poses_f64(); gamma, amap, bmap = e.get_joint_variables()
+        loss, _ = e.get_trace(k, 1)
+        rot, tr = pose_errors(new, pred)
+        worst["rot"] = max(worst["rot"], rot); worst["tr"] = max(worst["tr"], tr)
+        worst["loss"] = max(worst["loss"], abs(float(loss[0]) - ref["loss"]) / abs(ref["loss"]))
+        worst["gamma"] = max(worst["gamma"], float(np.max(np.abs(gamma - g_pred))))
+        worst["alpha"] = max(worst["alpha"], float(np.max(np.abs(amap[view, vv, uu] - a_pred))))
+        worst["beta"] = max(worst["beta"], float(np.max(np.abs(bmap[view, vv, uu] - b_pred))))
+        thetas.append(oracle.theta95(pred, poses))
+        if phase == 0 and oracle.converged(np.array(thetas), k, ocfg.w1, ocfg.eps1, ocfg.smooth_window): phase = 1
+        assert gphase == phase or gphase == 2, (k, gphase, phase)
+        poses = new
+    print(f"joint loop: phase {phase} after 24 iterations, {t_depth} depth steps; worst one-step differences: rot {worst['rot']:.2e} deg, "
+          f"trans {worst['tr']:.2e}, loss rel {worst['loss']:.2e}, gamma {worst['gamma']:.2e}, alpha {worst['alpha']:.2e}, beta {worst['beta']:.2e}")
+    assert phase >= 1 and t_depth >= 5
+    assert worst["rot"] <= 1e-3 and worst["tr"] <= 1e-4 and worst["loss"] <= 1e-5
+    # a step is ~lr = 1e-4 .. 3e-3 per variable; the depth gradients are summed with float atomics (order varies)
+    assert worst["gamma"] <= 3e-7 and worst["alpha"] <= 1e-5 and worst["beta"] <= 1e-5
+    # the variables really moved, and reset puts everything back
+    assert np.abs(gamma).max() > 1e-4 and np.abs(amap[view, vv, uu] - 1.0).max() > 1e-4
+    e.reset()
+    g0, a0, b0 = e.get_joint_variables()
+    assert not g0.any() and np.all(a0 == 1.0) and not b0.any()
+    fresh = make_ctx(sc, **kw)
+    assert e.loss_grad(10.0)["loss"] == fresh.loss_grad(10.0)["loss"]
+    e.destroy(); fresh.destroy()
+
+
 # ---------------------------------------------------------------------------------- edge extraction
 def _test_images(n, H, W, seed):
     """Seeded 8-bit images with edges of every orientation and strength: rectangles and discs of random grey levels
