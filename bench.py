@@ -44,6 +44,9 @@ def parse():
     ap.add_argument("--pair-budget", type=int, default=0,
                     help="M of the stochastic viewgraph sub-sampling (PAPER.md:500); 0 = all pairs every step, the "
                          "workload BASELINE.json's metric is quoted on")
+    ap.add_argument("--joint-phase", type=int, default=0,
+                    help="1: epo_step also optimises focal scale and edge-pixel depth (DESIGN.md 6.7); a step then runs "
+                         "the fused kernel twice, value still counts the loss's reprojections once")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--plumbing-test", action="store_true",
@@ -248,7 +251,8 @@ def main():
     sc = make_scene(args.config, n_views=args.views)
     stream = torch.cuda.current_stream()
     cfg = epo_config_default(n_views=sc.n_views, width=sc.W, height=sc.H, early_stop=0, device=local,
-                             stream=stream.cuda_stream, pair_budget=args.pair_budget, subsample_seed=2607)
+                             stream=stream.cuda_stream, pair_budget=args.pair_budget, subsample_seed=2607,
+                             joint_phase=args.joint_phase)
     e = Epo(cfg)
     # inputs resident in HBM before the timed region
     dK, dP, dD, dE = (torch.from_numpy(a).cuda() for a in (sc.K, sc.poses_init, sc.depth, sc.edges))
@@ -355,7 +359,8 @@ def main():
         data="synthetic",
         config=dict(workload=workload_name(sc), l2="flushed between timed steps (256 MiB write)",
                     reprojections_per_step=reproj, valid_per_step=n_valid, valid_fraction=n_valid / max(reproj, 1),
-                    edge_pixels=int(edge_off[-1]), parallelism="replicas only" if world > 1 else "1 GPU"),
+                    edge_pixels=int(edge_off[-1]), parallelism="replicas only" if world > 1 else "1 GPU",
+                    joint_phase=args.joint_phase),
         clocks=clocks, gpu_launches=int(k1 - k0),
         roofline=dict(bound="hbm", achieved=ach, peak=peak, unit="GB/s", frac=ach / peak, traffic=None,
                       kernel="k_loss_grad<u8>", kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
