@@ -425,17 +425,21 @@ epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_l
   // the evaluation first: per-pair valid counts (and the loss), then the joint pass over the same samples
   EPO_TRY(epo_launch_fused(c, lambda, false, false));
   EPO_TRY(epo_launch_finish(c, false, false, false, false));
-  double* d_gf = nullptr; float* d_gf32 = nullptr; float* d_gz = nullptr;
+  double* d_gf = nullptr; float* d_gf32 = nullptr; float* d_gz = nullptr; float* d_gpt = nullptr;
   const bool gz_dev = is_device_ptr(g_depth);
+  const size_t E = (size_t)(c->E > 0 ? c->E : 1);
   cudaError_t e = epo_dmalloc(c, &d_gf, N * sizeof(double));
   if (e == cudaSuccess) e = epo_dmalloc(c, &d_gf32, N * sizeof(float));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &d_gpt, E * sizeof(float));
   if (e == cudaSuccess && !gz_dev) e = epo_dmalloc(c, &d_gz, px * sizeof(float));
   float* gz = gz_dev ? g_depth : d_gz;
   if (e == cudaSuccess) e = cudaMemsetAsync(d_gf, 0, N * sizeof(double), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(d_gpt, 0, E * sizeof(float), st);
   if (e == cudaSuccess) e = cudaMemsetAsync(gz, 0, px * sizeof(float), st);
-  epo_status rc = e == cudaSuccess ? epo_launch_fused_joint(c, lambda, d_gf, gz, false)
+  epo_status rc = e == cudaSuccess ? epo_launch_fused_joint(c, lambda, d_gf, d_gpt, false)
                                    : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
                                               "epo_loss_grad_joint: %s", cudaGetErrorString(e));
+  if (rc == EPO_OK) rc = epo_joint_scatter_gz(c, d_gpt, gz);     // point order -> the dense map
   bool sync = false;
   if (rc == EPO_OK) {
     epo_launch_f64_to_f32(st, d_gf, d_gf32, (int64_t)N);
@@ -450,7 +454,7 @@ epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_l
     if (e == cudaSuccess && sync) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_loss_grad_joint: %s", cudaGetErrorString(e));
   }
-  epo_dfree(c, d_gf); epo_dfree(c, d_gf32); epo_dfree(c, d_gz);
+  epo_dfree(c, d_gf); epo_dfree(c, d_gf32); epo_dfree(c, d_gz); epo_dfree(c, d_gpt);
   return rc;
 }
 
@@ -494,7 +498,7 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
       // the joint gradients at the state this iteration's loss was evaluated at, then AdamW on gamma / alpha / beta
       // and the new intrinsics and points (all three self-gated by DevState.joint_pending)
       EPO_CUDA(c, cudaMemsetAsync(c->d_glogf, 0, (size_t)c->N * sizeof(double), st));
-      EPO_CUDA(c, cudaMemsetAsync(c->d_gz, 0, (size_t)c->N * c->W * c->H * sizeof(float), st));
+      EPO_CUDA(c, cudaMemsetAsync(c->d_gz, 0, (size_t)(c->E > 0 ? c->E : 1) * sizeof(float), st));
       EPO_TRY(epo_launch_fused_joint(c, -1.0f, c->d_glogf, c->d_gz, true));
       EPO_TRY(epo_launch_joint_update(c));
       c->static_dirty = true;                       // the points were rewritten: the next fused launch is serialised

@@ -95,7 +95,7 @@ struct epo_ctx {
   double* d_gamma;        // [3][N] gamma, Adam m, v
   double* d_ab;           // [3][E][2] (alpha, beta), Adam m, v, point order
   float* d_z0;            // [E] depth as given, point order
-  float* d_gz;            // [N][H][W] d L / d Z map of the joint pass
+  float* d_gz;            // [E] d L / d Z of the joint pass, point order
   double* d_glogf;        // [N] d L / d ln f
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
@@ -219,6 +219,7 @@ epo_status epo_joint_alloc(epo_ctx* ctx);              // after the points exist
 void epo_joint_free(epo_ctx* ctx);
 epo_status epo_joint_reset(epo_ctx* ctx);              // identity variables, zero moments, K and points as given
 epo_status epo_launch_joint_update(epo_ctx* ctx);      // gated by DevState.joint_pending
+epo_status epo_joint_scatter_gz(epo_ctx* ctx, const float* d_g_points, float* d_map);   // point order -> [N][H][W]
 epo_status epo_joint_export(epo_ctx* ctx, double* d_gamma_out, double* d_alpha_map, double* d_beta_map);
 // viewgraph.cu: cycle counts of all ordered pairs + ordered emission of the valid pairs
 epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_frac, int2* d_counts, int2* d_pairs,

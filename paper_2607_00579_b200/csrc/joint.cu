@@ -14,7 +14,7 @@ struct JointParams {
   const DevState* state;
   const double* sched;
   const double* glogf;       // [N]
-  const float* gz;           // [N][H][W]
+  const float* gz;           // [E] point order
   const float* K0;           // [N][4]
   float* K;                  // [N][4] current
   double* gamma;             // [3][N]
@@ -68,7 +68,7 @@ __global__ void k_joint_points(const JointParams q) {
     double a = q.ab[2 * i], b = q.ab[2 * i + 1];
     const double Z0 = (double)q.z0[i];
     if (depth_on) {
-      const double g = (double)q.gz[((size_t)view * q.H) * q.W + pix];
+      const double g = (double)q.gz[i];
       const size_t E2 = 2 * (size_t)q.E;
       a = adamw_step(a, Z0 * g, q.ab + E2 + 2 * i, q.ab + 2 * E2 + 2 * i, t, lr, q, 1.0);
       b = adamw_step(b, g, q.ab + E2 + 2 * i + 1, q.ab + 2 * E2 + 2 * i + 1, t, lr, q, 0.0);
@@ -88,6 +88,15 @@ __global__ void k_joint_init(float4* __restrict__ pts, float* __restrict__ z0, d
   ab[2 * i] = 1.0; ab[2 * i + 1] = 0.0;
   ab[2 * E + 2 * i] = ab[2 * E + 2 * i + 1] = 0.0;
   ab[4 * E + 2 * i] = ab[4 * E + 2 * i + 1] = 0.0;
+}
+
+// d L / d Z in point order -> the dense [N][H][W] map of the API (zeroed by the caller)
+__global__ void k_joint_scatter_gz(const float4* __restrict__ pts, const float* __restrict__ g, const int32_t* __restrict__ off,
+                                   int W, int H, float* __restrict__ map) {
+  const int view = blockIdx.y;
+  const int lo = off[view], n = off[view + 1] - lo;
+  for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
+    map[(size_t)view * W * H + __float_as_int(pts[(size_t)lo + e].w)] = g[(size_t)lo + e];
 }
 
 // dense maps of alpha (1 off the lists) and beta (0 off the lists)
@@ -139,7 +148,7 @@ epo_status epo_joint_alloc(epo_ctx* c) {
   if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_gamma, 3 * N * sizeof(double));
   if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_ab, 6 * E * sizeof(double));
   if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_z0, E * sizeof(float));
-  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_gz, N * c->W * c->H * sizeof(float));
+  if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_gz, E * sizeof(float));
   if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_glogf, N * sizeof(double));
   if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_K0, c->d_K, N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(c->d_gamma, 0, 3 * N * sizeof(double), c->stream);
@@ -180,6 +189,15 @@ epo_status epo_launch_joint_update(epo_ctx* c) {
   dim3 grid((unsigned)std::min((m + 255) / 256, 64), (unsigned)c->N);
   k_joint_points<<<grid, 256, 0, c->stream>>>(q);
   c->launches += 2;
+  EPO_CUDA(c, cudaGetLastError());
+  return EPO_OK;
+}
+
+epo_status epo_joint_scatter_gz(epo_ctx* c, const float* d_g_points, float* d_map) {
+  const int m = max_list(c);
+  dim3 grid((unsigned)std::min((m + 255) / 256, 64), (unsigned)c->N);
+  k_joint_scatter_gz<<<grid, 256, 0, c->stream>>>(c->d_pts, d_g_points, c->d_edge_off, c->W, c->H, d_map);
+  c->launches += 1;
   EPO_CUDA(c, cudaGetLastError());
   return EPO_OK;
 }
