@@ -334,7 +334,7 @@ def main():
         hpairs = torch.from_numpy(sc.pairs).pin_memory()
         hout = torch.empty((sc.n_views, 12), dtype=torch.float32).pin_memory()
         times = []
-        for rep in range(3):
+        for rep in range(5):
             torch.cuda.synchronize(); t0 = time.perf_counter()
             e2 = Epo(cfg)
             e2.set_views(hK, hP, hD, hE); e2.set_pairs(hpairs)
