@@ -28,12 +28,12 @@ struct JointParams {
   int force;                 // rebuild the points from the current variables without stepping (epo_joint_reset)
 };
 
-__device__ __forceinline__ double adamw_step(double p, double g, double* m, double* v, int t, double lr, const JointParams& q,
-                                             double p_id) {
+// c1 = 1 - beta1^t, c2 = 1 - beta2^t of the group's step count t (the same for every variable of a launch)
+__device__ __forceinline__ double adamw_step(double p, double g, double* m, double* v, double c1, double c2, double lr,
+                                             const JointParams& q, double p_id) {
   p -= lr * q.wd * (p - p_id);
   const double mm = q.beta1 * *m + (1.0 - q.beta1) * g, vv = q.beta2 * *v + (1.0 - q.beta2) * g * g;
   *m = mm; *v = vv;
-  const double c1 = 1.0 - pow(q.beta1, (double)t), c2 = 1.0 - pow(q.beta2, (double)t);
   return p - lr * (mm / c1) / (sqrt(vv / c2) + q.adam_eps);
 }
 
@@ -45,7 +45,8 @@ __global__ void k_joint_cams(const JointParams q) {
   const int s = q.state->step - 1;
   const double lr = q.sched[4 * (size_t)s];
   double g = q.gamma[c];
-  g = adamw_step(g, q.glogf[c] / (1.0 + g), q.gamma + q.N + c, q.gamma + 2 * q.N + c, s + 1, lr, q, 0.0);
+  const double c1 = 1.0 - pow(q.beta1, (double)(s + 1)), c2 = 1.0 - pow(q.beta2, (double)(s + 1));
+  g = adamw_step(g, q.glogf[c] / (1.0 + g), q.gamma + q.N + c, q.gamma + 2 * q.N + c, c1, c2, lr, q, 0.0);
   q.gamma[c] = g;
   q.K[4 * c] = (float)((double)q.K0[4 * c] * (1.0 + g));
   q.K[4 * c + 1] = (float)((double)q.K0[4 * c + 1] * (1.0 + g));
@@ -60,6 +61,7 @@ __global__ void k_joint_points(const JointParams q) {
   const bool depth_on = !q.force && q.state->phase_prev >= 1;
   const int t = s - q.state->phase1_step;            // 1 for the first iteration that starts in phase 1
   const double lr = depth_on ? q.sched[4 * (size_t)s] : 0.0;
+  const double c1 = depth_on ? 1.0 - pow(q.beta1, (double)t) : 1.0, c2 = depth_on ? 1.0 - pow(q.beta2, (double)t) : 1.0;
   const float ifx = 1.0f / q.K[4 * view], ify = 1.0f / q.K[4 * view + 1], cx = q.K[4 * view + 2], cy = q.K[4 * view + 3];
   for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
     const size_t i = (size_t)lo + e;
@@ -70,8 +72,8 @@ __global__ void k_joint_points(const JointParams q) {
     if (depth_on) {
       const double g = (double)q.gz[i];
       const size_t E2 = 2 * (size_t)q.E;
-      a = adamw_step(a, Z0 * g, q.ab + E2 + 2 * i, q.ab + 2 * E2 + 2 * i, t, lr, q, 1.0);
-      b = adamw_step(b, g, q.ab + E2 + 2 * i + 1, q.ab + 2 * E2 + 2 * i + 1, t, lr, q, 0.0);
+      a = adamw_step(a, Z0 * g, q.ab + E2 + 2 * i, q.ab + 2 * E2 + 2 * i, c1, c2, lr, q, 1.0);
+      b = adamw_step(b, g, q.ab + E2 + 2 * i + 1, q.ab + 2 * E2 + 2 * i + 1, c1, c2, lr, q, 0.0);
       q.ab[2 * i] = a; q.ab[2 * i + 1] = b;
     }
     const float Z = (float)(Z0 * a + b);
