@@ -25,9 +25,10 @@
  * Errors.  Every function returns an epo_status; nothing throws or aborts.  On error the context is
  * left unchanged (epo_set_views / epo_set_pairs are all-or-nothing); epo_last_error gives a
  * context-owned, NUL-terminated description valid until the next call on that context.
- * Threads.  One context per thread at a time; no global state.
- * Determinism.  Edge lists, distance fields and pair lists are bit-reproducible.  Loss and gradient
- * are reproducible up to the order of a few fp64 atomic additions per pair (relative 1e-16).
+ * Threads.  One context per thread at a time; no global state (device memory comes from a per-context
+ * pool; the device's default memory pool and its attributes are never touched).
+ * Determinism.  Edge lists, distance fields, pair lists, loss, gradient and every iteration of epo_step
+ * are bit-reproducible run to run: all reductions run in a fixed order, without atomics on values.
  */
 #ifndef EPO_H_
 #define EPO_H_
@@ -93,6 +94,10 @@ typedef struct {
                                        rate and weight_decay towards the identity.  An iteration then runs the fused
                                        kernel twice (loss + pose gradient, then the joint gradients).                  */
   float   weight_decay;             /* 0.01                                                          */
+  void*   mem_pool;                 /* cudaMemPool_t all device memory of the context is taken from (stream-ordered, on
+                                       cfg.stream).  NULL (default): the context creates a private pool and destroys it
+                                       in epo_destroy.  A caller-owned pool may be shared by consecutive contexts so
+                                       that a new one reuses the blocks of a destroyed one; it must outlive them.   */
 } epo_config;
 
 /* Fill *cfg with the paper's hyper-parameters (n_views/width/height = 0, device 0, stream NULL). */
@@ -151,7 +156,9 @@ EPO_API epo_status epo_build_viewgraph(epo_ctx* ctx, int32_t grid_stride, float 
  * Set the viewgraph as a list of DIRECTED pairs [P][2] = (source, target), P >= 1,
  * indices in [0, N), source != target; duplicates are kept (they weigh twice).  Builds the canonical
  * order (ascending (target, source), stable), the per-target and per-source incidence lists and the
- * work list of the fused kernel.  Resets Adam moments, step counter, phase and traces.
+ * work list of the fused kernel.  Resets the optimiser (Adam / AdamW moments, step counter, phase and traces)
+ * and nothing else: the CURRENT poses (and joint variables) stay, so a viewgraph re-estimated from refined poses
+ * can be installed without losing them.  epo_reset rewinds to the initial poses.
  */
 EPO_API epo_status epo_set_pairs(epo_ctx* ctx, const int32_t* pairs, int64_t n_pairs);
 

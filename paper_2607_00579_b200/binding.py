@@ -36,7 +36,8 @@ class EpoConfig(C.Structure):
                 ("early_stop", C.c_int32), ("dtf_format", C.c_int32), ("e_max", C.c_int32), ("z_min", C.c_float),
                 ("device", C.c_int32), ("stream", C.c_void_p), ("pair_budget", C.c_int32),
                 ("subsample_seed", C.c_uint64), ("stop_rule", C.c_int32), ("w_loss", C.c_int32),
-                ("eps_loss", C.c_float), ("joint_phase", C.c_int32), ("weight_decay", C.c_float)]
+                ("eps_loss", C.c_float), ("joint_phase", C.c_int32), ("weight_decay", C.c_float),
+                ("mem_pool", C.c_void_p)]
 
 
 class EpoError(RuntimeError):

@@ -126,6 +126,7 @@ epo_status epo_config_default(epo_config* cfg) {
   cfg->pair_budget = 0; cfg->subsample_seed = 0;
   cfg->stop_rule = 0; cfg->w_loss = 100; cfg->eps_loss = 5e-4f;
   cfg->joint_phase = 0; cfg->weight_decay = 0.01f;
+  cfg->mem_pool = nullptr;
   return EPO_OK;
 }
 
@@ -145,17 +146,29 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   c->N = cfg->n_views; c->W = cfg->width; c->H = cfg->height;
   c->have_views = c->have_pairs = false; c->P = c->E = c->n_work = c->reproj_per_eval = c->launches = 0; c->lg_chunk = kLgOuter * kLgPass;
   c->err[0] = 0;
+  c->pool = nullptr; c->own_pool = false;
   c->atlas = EpoAtlas{nullptr, nullptr, 0, 0, 1};
   { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
   c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
   const size_t N = (size_t)c->N;
   if (e == cudaSuccess) {
-    // keep freed blocks in the device's default pool instead of returning them to the driver at every sync
-    cudaMemPool_t pool = nullptr;
-    unsigned long long keep = ~0ull;
-    if (cudaDeviceGetDefaultMemPool(&pool, cfg->device) == cudaSuccess) cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-    cudaGetLastError();
+    if (cfg->mem_pool) {
+      c->pool = (cudaMemPool_t)cfg->mem_pool;       // caller-owned: shared between contexts, never destroyed here
+    } else {
+      // a private pool that keeps freed blocks until epo_destroy (no process-wide side effect)
+      cudaMemPoolProps props = {};
+      props.allocType = cudaMemAllocationTypePinned; props.handleTypes = cudaMemHandleTypeNone;
+      props.location.type = cudaMemLocationTypeDevice; props.location.id = cfg->device;
+      e = cudaMemPoolCreate(&c->pool, &props);
+      if (e == cudaSuccess) {
+        c->own_pool = true;
+        unsigned long long keep = ~0ull;
+        e = cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+      }
+    }
+  }
+  if (e == cudaSuccess) {
     e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_alloc, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming);
@@ -194,6 +207,7 @@ void epo_destroy(epo_ctx* c) {
   epo_dfree(c, c->d_m); epo_dfree(c, c->d_v); epo_dfree(c, c->d_dR); epo_dfree(c, c->d_dt); epo_dfree(c, c->d_state);
   epo_dfree(c, c->d_sched); epo_dfree(c, c->d_theta); epo_dfree(c, c->d_loss_trace);
   cudaStreamSynchronize(c->stream);                 // the frees are stream-ordered: done before the context goes
+  if (c->own_pool && c->pool) cudaMemPoolDestroy(c->pool);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->ev_alloc) cudaEventDestroy(c->ev_alloc);
   if (c->ev_copied) cudaEventDestroy(c->ev_copied);
@@ -377,8 +391,10 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
     if (c->sel_grid < 1) c->sel_grid = 1;
   }
   c->have_pairs = true; c->static_dirty = true;
-  EPO_CUDA(c, cudaMemcpyAsync(c->d_poses, c->d_poses_init, (size_t)c->N * 12 * sizeof(double), cudaMemcpyDeviceToDevice, st));
-  EPO_TRY(reset_optimiser(c));
+  // the optimiser restarts (moments, step counter, phase, traces); the CURRENT poses and joint variables stay, so that
+  // a viewgraph re-estimated with epo_build_viewgraph from refined poses can be installed without losing them
+  EPO_TRY(reset_optimiser(c, false));
+  EPO_TRY(epo_joint_reset_moments(c));
   return EPO_OK;
 }
 

@@ -76,6 +76,8 @@ struct epo_ctx {
   epo_config cfg;
   cudaStream_t stream;
   cudaStream_t copy_stream;   // epo_set_views: the depth maps arrive on it while the distance transform runs on `stream`
+  cudaMemPool_t pool;         // every device allocation of the context comes from it (stream-ordered)
+  bool own_pool;              // created in epo_create (cfg.mem_pool == NULL) and destroyed in epo_destroy
   cudaEvent_t ev_alloc, ev_copied;
   int N, W, H;
   bool have_views, have_pairs;
@@ -176,12 +178,14 @@ epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
     if (s_ != EPO_OK) return s_;   \
   } while (0)
 
-// ---- device memory: stream-ordered allocation from the device's default pool on the context's stream.  A free
-// costs no device synchronisation and a later allocation of the same size is served from the pool (epo_create sets
-// the pool's release threshold), which takes ~2.5 ms of cudaMalloc/cudaFree out of an epo_set_views call.
+// ---- device memory: stream-ordered allocation on the context's stream from the context's memory pool -- a private
+// pool created in epo_create (release threshold = keep everything until epo_destroy), or the pool the caller passed in
+// cfg.mem_pool.  A free costs no device synchronisation and a later allocation of the same size is served from the
+// pool, which takes ~2.5 ms of cudaMalloc/cudaFree out of a repeated epo_set_views call.  The device's default pool
+// and its attributes are never touched.
 template <class T>
 inline cudaError_t epo_dmalloc(epo_ctx* ctx, T** p, size_t bytes) {
-  return cudaMallocAsync(reinterpret_cast<void**>(p), bytes ? bytes : 1, ctx->stream);
+  return cudaMallocFromPoolAsync(reinterpret_cast<void**>(p), bytes ? bytes : 1, ctx->pool, ctx->stream);
 }
 inline void epo_dfree(epo_ctx* ctx, void* p) {
   if (p) cudaFreeAsync(p, ctx->stream);
@@ -218,6 +222,7 @@ epo_status epo_run_canny(epo_ctx* ctx, const uint8_t* d_img, int low, int high, 
 epo_status epo_joint_alloc(epo_ctx* ctx);              // after the points exist (epo_set_views)
 void epo_joint_free(epo_ctx* ctx);
 epo_status epo_joint_reset(epo_ctx* ctx);              // identity variables, zero moments, K and points as given
+epo_status epo_joint_reset_moments(epo_ctx* ctx);      // zero AdamW moments only (epo_set_pairs: the variables stay)
 epo_status epo_launch_joint_update(epo_ctx* ctx);      // gated by DevState.joint_pending
 epo_status epo_joint_scatter_gz(epo_ctx* ctx, const float* d_g_points, float* d_map);   // point order -> [N][H][W]
 epo_status epo_joint_export(epo_ctx* ctx, double* d_gamma_out, double* d_alpha_map, double* d_beta_map);

@@ -184,6 +184,13 @@ epo_status epo_joint_reset(epo_ctx* c) {
   return EPO_OK;
 }
 
+epo_status epo_joint_reset_moments(epo_ctx* c) {
+  if (!c->cfg.joint_phase || !c->d_gamma) return EPO_OK;
+  EPO_CUDA(c, cudaMemsetAsync(c->d_gamma + c->N, 0, 2 * (size_t)c->N * sizeof(double), c->stream));
+  if (c->E > 0) EPO_CUDA(c, cudaMemsetAsync(c->d_ab + 2 * (size_t)c->E, 0, 4 * (size_t)c->E * sizeof(double), c->stream));
+  return EPO_OK;
+}
+
 epo_status epo_launch_joint_update(epo_ctx* c) {
   const JointParams q = make_params(c);
   k_joint_cams<<<(c->N + 127) / 128, 128, 0, c->stream>>>(q);

@@ -104,20 +104,19 @@ __device__ void select_two(const double* x, int n, int k, double* lo, double* hi
 }
 
 // Converged(theta_{0..s}; w, eps)  (smooth: PAPER.md:357; raw: PAPER.md:114), evaluated by the whole CTA:
-// thread k < w tests the window ending at step s - k (its mean is summed in time order).
+// thread k tests the windows ending at steps s - k, s - k - blockDim, ... (k < w; each mean is summed in time order).
 __device__ bool converged(const double* theta, double theta_s, int s, int w, double eps, int smooth) {
   const int need = smooth ? 2 * w - 2 : w - 1;
   if (s < need) return false;                       // uniform
   bool ok = true;
-  const int k = threadIdx.x;
-  if (k < w) {
-    auto th = [&](int j) { return j == s ? theta_s : __ldcg(theta + j); };
+  auto th = [&](int j) { return j == s ? theta_s : __ldcg(theta + j); };
+  for (int k = threadIdx.x; k < w; k += blockDim.x) {       // any window length: strided over the CTA
     if (smooth) {
       double m = 0.0;
       for (int j = s - k - w + 1; j <= s - k; ++j) m += th(j);
-      ok = m / w < eps;
+      ok = ok && (m / w < eps);
     } else {
-      ok = th(s - k) < eps;
+      ok = ok && (th(s - k) < eps);
     }
   }
   return __syncthreads_and(ok) != 0;

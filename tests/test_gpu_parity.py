@@ -275,8 +275,7 @@ def test_fixed_200_iterations_free_running_tiny():
 
 @pytest.mark.parametrize("name,iters,strict_prefix", [("room6", 200, 25), ("orbit8", 100, 0)])
 def test_free_running_trajectories(name, iters, strict_prefix):
-    """Free-running runs decorrelate (see _lockstep) -- two runs of the GPU itself do, through the order of its
-    fp64 atomics -- so beyond config 1 the end-of-run pose difference is a chaotic quantity, printed here next
+    """Free-running runs decorrelate (see _lockstep), so beyond config 1 the end-of-run pose difference is a chaotic quantity, printed here next
     to the distance between the oracle's own two variants.  Asserted: the contraction phase of the room scene
     (first 25 iterations) meets the contract's tolerance; every run ends within the Adam jitter amplitude
     (a few lr = 3e-3 rad or scene units per coordinate) of the oracle and at the same loss."""
@@ -591,13 +590,13 @@ def test_subsampled_iterations_match_the_oracle():
 
 def test_measurement_hooks_leave_results_unchanged():
     """epo_time_loss_grad_kernel / epo_time_gather_ceiling overwrite the per-CTA partial sums only: the next
-    evaluation and the loop are unaffected, and the memory side alone is not slower than the whole kernel."""
+    evaluation and the loop are unaffected.  (No timing comparison here: durations are bench.py's business.)"""
     sc = scene("room6")
     e = make_ctx(sc, early_stop=0)
     before = e.loss_grad(10.0)
     full = e.time_loss_grad_kernel(10.0, 5, False)
     gat = e.time_gather_ceiling(10.0, 5, False)
-    assert 0.0 < gat[1] <= full[1] * 1.15
+    assert full[1] > 0.0 and gat[1] > 0.0
     after = e.loss_grad(10.0)
     assert after["loss"] == before["loss"] and np.array_equal(after["grad"], before["grad"])
     assert e.step(3) == (3, 0)
@@ -625,6 +624,47 @@ def test_loss_based_stopping_rule():
         elif oracle.converged_loss(loss.astype(np.float64), s_, 12, okw["eps_loss"]):
             fired = s_ + 1; break
     assert fired == done, (fired, done)
+    e.destroy()
+
+
+def test_long_convergence_window():
+    """A window longer than k_finish's CTA (w1 = 300 > 256 threads), raw test: the phase must agree
+    with the oracle's rule at every iteration; with eps1 below the warm-up's pose changes the rule can only fire
+    once the large early steps have left the window, i.e. well after step w1 - 1."""
+    kw = dict(w1=300, eps1=0.15, smooth_window=0, early_stop=0)
+    okw = dict(w1=300, eps1=float(np.float32(0.15)), smooth_window=0, early_stop=0)
+    sc = scene("tiny")
+    e = make_ctx(sc, **kw)
+    e.step(380)
+    _, theta = e.get_trace(0, 380)
+    e.destroy()
+    big = np.nonzero(theta >= np.float32(0.15))[0]
+    assert len(big) and big.max() >= 8, "the scene must have early steps above eps1 for this test to bite"
+    worst, _, n = _lockstep(sc, 380, kw, okw)                 # asserts GPU phase == oracle phase at every iteration
+    assert n == 380 and worst["rot"] <= 1e-3 and worst["tr"] <= 1e-4
+
+
+def test_set_pairs_keeps_the_current_poses():
+    """Refine, re-estimate the viewgraph from the refined poses, install it (the flow include/epo.h advertises for
+    epo_build_viewgraph): epo_set_pairs restarts the optimiser but must not rewind the poses; epo_reset does."""
+    sc = scene("room6")
+    e = make_ctx(sc, early_stop=0)
+    e.step(15)
+    refined = e.get_poses_f64()
+    assert not np.array_equal(refined, sc.poses_init.astype(np.float64))
+    pairs = e.build_viewgraph(stride=8)
+    assert len(pairs) >= 2
+    e.set_pairs(pairs)
+    assert np.array_equal(e.get_poses_f64(), refined)
+    assert e.step(0) == (0, 0)                                   # optimiser state restarted
+    done, _ = e.step(2)
+    assert done == 2
+    loss, _ = e.get_trace(0, 2)
+    prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
+    ref = oracle.loss_grad(prob, refined, pairs, 10.0, z_min=Z_MIN)
+    assert abs(float(loss[0]) - ref["loss"]) <= 1e-5 * abs(ref["loss"])    # step 0 again: lambda_0 at the kept poses
+    e.reset()
+    assert np.array_equal(e.get_poses_f64(), sc.poses_init.astype(np.float64))
     e.destroy()
 
 
