@@ -110,6 +110,15 @@ def lib():
                                     C.c_double, C.c_double, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int32),
                                     C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_double),
                                     C.POINTER(C.c_double)]
+        L.orc_pair_event_slack.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_uint16), C.POINTER(C.c_float),
+                                           C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                           C.POINTER(C.c_double), C.POINTER(C.c_float), C.c_double, C.c_double,
+                                           C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.orc_event_slack.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
+                                      C.POINTER(C.c_int32), C.POINTER(C.c_uint16), C.POINTER(C.c_float),
+                                      C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_int32), C.c_double, C.c_double,
+                                      C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_double),
+                                      C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
         L.orc_joint_grad.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
                                      C.POINTER(C.c_int32), C.POINTER(C.c_uint16), C.POINTER(C.c_float),
                                      C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_int32), C.c_double, C.c_double,
@@ -291,6 +300,40 @@ def loss_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, want_pair
                         _p(pl, C.c_double), _p(pv, C.c_int32), _p(pG, C.c_double), _p(near, C.c_int32),
                         _p(grad, C.c_double), C.byref(L))
     return dict(loss=L.value, pair_loss=pl, pair_valid=pv, grad=grad, near=near, pair_G=pG)
+
+
+def pair_event_slack(uv, z, Ks, Kt, Ts, Tt, dtf_t, lam, delta=1.0, z_min=1e-6):
+    """One directed pair: what a correct binary32 evaluation may decide differently (see orc_pair_event_slack).
+    Returns dict(E_t, E_s, E_rho, k_out, k_in, flagged, check [14] = S, n, G[12] through the slack routine)."""
+    H, W = dtf_t.shape
+    uv = np.ascontiguousarray(uv, np.uint16); z = np.ascontiguousarray(z, np.float32)
+    dtf_t = np.ascontiguousarray(dtf_t, np.float32)
+    out = np.zeros(8); chk = np.zeros(14)
+    lib().orc_pair_event_slack(W, H, len(z), _p(uv, C.c_uint16), _p(z, C.c_float), _p(_d(Ks, 4), C.c_double),
+                               _p(_d(Kt, 4), C.c_double), _p(_d(Ts, 12), C.c_double), _p(_d(Tt, 12), C.c_double),
+                               _p(dtf_t, C.c_float), lam, delta, z_min, _p(out, C.c_double), _p(chk, C.c_double))
+    return dict(E_t=out[0], E_s=out[1], E_rho=out[2], k_out=int(out[3]), k_in=int(out[4]), flagged=int(out[5]), Q_t=out[6],
+                Q_s=out[7], check=chk)
+
+
+def event_slack(prob: Problem, poses, pairs, lam, ref=None, delta=1.0, z_min=1e-6):
+    """Bounds on what a correct binary32 evaluation may differ by from `ref` = loss_grad(..., want_pair_G=True) (all
+    double) through its discrete decisions: dict(cam [N] on the 2-norm of each camera's gradient, pair_loss [P],
+    k_out [P], k_in [P] on the valid counts, flagged [P], rss [N] = root-sum-square of the terms of each camera's
+    gradient: its scale before cancellation, reading T2)."""
+    N = prob.n_views
+    poses = np.ascontiguousarray(np.asarray(poses, np.float64).reshape(N, 12))
+    pairs = np.ascontiguousarray(pairs, np.int32); P = pairs.shape[0]
+    if ref is None or ref.get("pair_G") is None:
+        ref = loss_grad(prob, poses, pairs, lam, delta, z_min, want_pair_G=True)
+    cam = np.zeros(N); pls = np.zeros(P); fl = np.zeros((P, 3), np.int32); rss = np.zeros(N)
+    pl = np.ascontiguousarray(ref["pair_loss"], np.float64); pv = np.ascontiguousarray(ref["pair_valid"], np.int32)
+    pG = np.ascontiguousarray(ref["pair_G"], np.float64)
+    lib().orc_event_slack(N, prob.W, prob.H, _p(prob.K, C.c_float), _p(poses, C.c_double), _p(prob.edge_off, C.c_int32),
+                          _p(prob.uv, C.c_uint16), _p(prob.z, C.c_float), _p(prob.dtf, C.c_float), P, _p(pairs, C.c_int32),
+                          C.c_double(lam), C.c_double(delta), C.c_double(z_min), _p(pl, C.c_double), _p(pv, C.c_int32),
+                          _p(pG, C.c_double), _p(cam, C.c_double), _p(pls, C.c_double), _p(fl, C.c_int32), _p(rss, C.c_double))
+    return dict(cam=cam, pair_loss=pls, k_out=fl[:, 0].copy(), k_in=fl[:, 1].copy(), flagged=fl[:, 2].copy(), rss=rss)
 
 
 def joint_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, coord_fp32=0):

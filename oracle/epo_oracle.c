@@ -467,9 +467,200 @@ void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, con
 }
 
 /* =================================================================================================
- * O7  Schedules, Adam, SE(3) exponential  (PAPER.md:121, 429, 462-463; readings S4, S10, S11)
+ * Event slack: how far may a CORRECT binary32 evaluation of the same loss be from this all-double one?
+ * (SURVEY.md 8(c) "Tolerance realism" (2); reading T1.)
+ *
+ * The paper computes the geometry in FP32.  The loss is continuous in the projected position, but
+ * three decisions per sample are discrete: valid or not (z > z_min, 0 <= x <= W-1, 0 <= y <= H-1: a sample
+ * enters or leaves the pair's mean), the bilinear cell (x0, y0) (the spatial gradient of the interpolant
+ * jumps at a cell border), and the clamp test d <= lambda (rho' jumps from min(d, delta) to 0).  A binary32
+ * evaluation places the sample up to its own rounding error away from where double places it, and so may decide
+ * differently for samples that lie that close to a boundary.  This function bounds, from the double side alone
+ * and without reference to any particular binary32 program, what those decisions can change.
+ *
+ * Position error of ANY evaluation that rounds every operation of rows a-2..a-4 to binary32 (u = 2^-24), for the
+ * natural formulas  x_s = Z (u - cx_s)/fx_s,  X = r00 x_s + r01 y_s + r02 z_s + t_x,  x = fx_t X / Z + cx_t:
+ *   |dX| <= 8 u S_X,  S_X = |r00 x_s| + |r01 y_s| + |r02 z_s| + |t_x|      (same for Y, Z)
+ *           [1 u: T_ts rounded to binary32; <= 4 u: the point x_s (difference, reciprocal or division by fx, two
+ *            products); 3 u: the three additions (or FMAs) of the row sum]
+ *   r_x = fx_t |dX| / Z + |x - cx_t| (|dZ| / Z + 3 u) + u |x|
+ *           [product fx_t X, reciprocal or division by Z, their product, the final addition of cx_t]
+ *   r_d = |dd/dx| r_x + |dd/dy| r_y + 6 u max|D|                            (the interpolated distance)
+ * For every sample the alternatives a binary32 evaluation can reach are enumerated -- valid / not valid if the
+ * position is within (r_x, r_y) of the image border (or Z within |dZ| of z_min), the neighbouring cell in x and/or
+ * y if the position is within r of a cell border, the other clamp branch if |d - lambda| <= r_d -- and the largest
+ * change of the sample's contribution to the pair's un-normalised target sum, source sum (6-vectors, 2-norm)
+ * and loss sum is added to the pair's slack:
+ *   E_t, E_s, E_rho   sums of those largest changes
+ *   k_out, k_in       samples that double counts valid but binary32 may drop / that double drops but binary32
+ *                     may count (they change the pair's n_valid)
+ * With n' in [n - k_out, n + k_in] and n_lo = max(n - k_out, 1):
+ *   | G'/n' - G/n | <= E / n_lo + |G| max(k_out, k_in) / (n n_lo)          (loss sums likewise)
+ * and per camera  slack_c = (1/P) [ sum_{t = c} (target bound) + sum_{s = c} (source bound) ].
+ * A parity test then asserts  | g_gpu,c - g_oracle,c | <= 1e-4 | g_oracle,c | + slack_c : the contract's tolerance
+ * for everything that is continuous, plus exactly what the flagged samples can move.
+ * `check` (nullable, [14] per pair) receives S, n and the 12 sums accumulated through THIS function's per-sample
+ * routine for the nominal decisions, so that a test can tie it to orc_pair_loss_grad.
  * ================================================================================================= */
-/* clamp lambda: clamp_start -> clamp_end linearly over the first clamp_steps steps  (PAPER.md:462) */
+#define ORC_U32 5.9604644775390625e-08 /* 2^-24 */
+
+/* contribution of one sample at position (x, y), evaluated in cell (x0, y0) with the clamp branch `inside`
+ * (1: d <= lambda taken as true): rho, target 6-vector, source 6-vector.  Same formulas as the pair routine above. */
+static void orc_sample_terms(int W, const float* dtf_t, const double Kt[4], const double Tts[12], const double xs[3],
+                             const double xt[3], double x, double y, int x0, int y0, int inside, double lambda,
+                             double delta, double* rho, double gt[6], double gs[6], double* d_out, double dd[2],
+                             double* Dmax) {
+  double wx = x - x0, wy = y - y0;
+  double D00 = dtf_t[(size_t)y0 * W + x0], D01 = dtf_t[(size_t)y0 * W + x0 + 1];
+  double D10 = dtf_t[(size_t)(y0 + 1) * W + x0], D11 = dtf_t[(size_t)(y0 + 1) * W + x0 + 1];
+  double d = (1.0 - wy) * ((1.0 - wx) * D00 + wx * D01) + wy * ((1.0 - wx) * D10 + wx * D11);
+  double ddx = (1.0 - wy) * (D01 - D00) + wy * (D11 - D10);
+  double ddy = (1.0 - wx) * (D10 - D00) + wx * (D11 - D01);
+  double dhat = d < lambda ? d : lambda;
+  *rho = dhat <= delta ? 0.5 * dhat * dhat : delta * (dhat - 0.5 * delta);
+  double drho = inside ? (d < delta ? d : delta) : 0.0;
+  double iz = 1.0 / xt[2], a[3], b[3];
+  a[0] = drho * ddx * Kt[0] * iz;
+  a[1] = drho * ddy * Kt[1] * iz;
+  a[2] = -drho * (ddx * Kt[0] * xt[0] + ddy * Kt[1] * xt[1]) * iz * iz;
+  gt[0] = a[0]; gt[1] = a[1]; gt[2] = a[2];
+  gt[3] = xt[1] * a[2] - xt[2] * a[1];
+  gt[4] = xt[2] * a[0] - xt[0] * a[2];
+  gt[5] = xt[0] * a[1] - xt[1] * a[0];
+  for (int i = 0; i < 3; ++i) b[i] = Tts[i] * a[0] + Tts[4 + i] * a[1] + Tts[8 + i] * a[2];
+  gs[0] = -b[0]; gs[1] = -b[1]; gs[2] = -b[2];
+  gs[3] = -(xs[1] * b[2] - xs[2] * b[1]);
+  gs[4] = -(xs[2] * b[0] - xs[0] * b[2]);
+  gs[5] = -(xs[0] * b[1] - xs[1] * b[0]);
+  *d_out = d; dd[0] = ddx; dd[1] = ddy;
+  double m = fabs(D00);
+  if (fabs(D01) > m) m = fabs(D01);
+  if (fabs(D10) > m) m = fabs(D10);
+  if (fabs(D11) > m) m = fabs(D11);
+  *Dmax = m;
+}
+
+static double orc_norm6(const double a[6], const double b[6] /* nullable: norm of a - b */) {
+  double q = 0.0;
+  for (int i = 0; i < 6; ++i) { double v = b ? a[i] - b[i] : a[i]; q += v * v; }
+  return sqrt(q);
+}
+
+/* One pair.  out[8] = { E_t, E_s, E_rho, k_out, k_in, flagged samples, Q_t, Q_s }; check[14] nullable.
+ * Q_t, Q_s = sums over the valid samples of the SQUARED 2-norm of the sample's target / source 6-vector: the scale of
+ * the pair's gradient before its terms cancel (reading T2: near a minimum |G| -> 0 while the terms do not, and an
+ * error "relative to |G|" loses its meaning; a tolerance is then taken relative to max(|g|, root-sum-square)). */
+void orc_pair_event_slack(int W, int H, int n_edges, const uint16_t* uv, const float* z, const double Ks[4],
+                          const double Kt[4], const double Ts[12], const double Tt[12], const float* dtf_t,
+                          double lambda, double delta, double z_min, double out[8], double* check) {
+  double Tts[12];
+  orc_relative_pose(Ts, Tt, Tts);
+  double Et = 0.0, Es = 0.0, Er = 0.0, Qt = 0.0, Qs = 0.0; int k_out = 0, k_in = 0, flagged = 0;
+  if (check) for (int i = 0; i < 14; ++i) check[i] = 0.0;
+  const double xmax = (double)(W - 1), ymax = (double)(H - 1);
+  for (int e = 0; e < n_edges; ++e) {
+    double xs[3], xt[3], S3[3];
+    orc_backproject_cam(Ks, (double)uv[2 * e], (double)uv[2 * e + 1], (double)z[e], xs);
+    for (int i = 0; i < 3; ++i) {
+      xt[i] = Tts[4 * i] * xs[0] + Tts[4 * i + 1] * xs[1] + Tts[4 * i + 2] * xs[2] + Tts[4 * i + 3];
+      S3[i] = fabs(Tts[4 * i] * xs[0]) + fabs(Tts[4 * i + 1] * xs[1]) + fabs(Tts[4 * i + 2] * xs[2]) + fabs(Tts[4 * i + 3]);
+    }
+    const double eX = 8.0 * ORC_U32 * S3[0], eY = 8.0 * ORC_U32 * S3[1], eZ = 8.0 * ORC_U32 * S3[2];
+    const int z_ok = xt[2] > z_min, z_unsure = fabs(xt[2] - z_min) <= eZ;
+    if (!z_ok && !z_unsure) continue;                  /* behind the camera on both sides */
+    /* a depth within rounding of z_min gives an unbounded position: only the count can be bounded */
+    if (z_unsure) { flagged++; if (z_ok) k_out++; else k_in++; Et = Es = Er = INFINITY; continue; }
+    double px[2];
+    orc_project_px(Kt, xt, px);
+    const double x = px[0], y = px[1];
+    const double rx = (Kt[0] * eX + fabs(x - Kt[2]) * eZ) / xt[2] + ORC_U32 * (3.0 * fabs(x - Kt[2]) + fabs(x));
+    const double ry = (Kt[1] * eY + fabs(y - Kt[3]) * eZ) / xt[2] + ORC_U32 * (3.0 * fabs(y - Kt[3]) + fabs(y));
+    const int valid = x >= 0.0 && x <= xmax && y >= 0.0 && y <= ymax;
+    const int reach = x >= -rx && x <= xmax + rx && y >= -ry && y <= ymax + ry;   /* binary32 may find it inside */
+    if (!reach) continue;
+    const int edge_near = x < rx || x > xmax - rx || y < ry || y > ymax - ry;     /* binary32 may decide the other way */
+    /* where the alternatives are evaluated: the position itself, moved onto the image if it is just outside */
+    const double xe = x < 0.0 ? 0.0 : (x > xmax ? xmax : x), ye = y < 0.0 ? 0.0 : (y > ymax ? ymax : y);
+    int x0 = (int)floor(xe), y0 = (int)floor(ye);
+    if (x0 > W - 2) x0 = W - 2;
+    if (y0 > H - 2) y0 = H - 2;
+    /* neighbouring cells a binary32 position may fall into */
+    int cxs[2] = { x0, x0 }, cys[2] = { y0, y0 }, ncx = 1, ncy = 1;
+    if (xe - x0 < rx && x0 >= 1) { cxs[1] = x0 - 1; ncx = 2; }
+    else if (x0 + 1 - xe < rx && x0 + 1 <= W - 2) { cxs[1] = x0 + 1; ncx = 2; }
+    if (ye - y0 < ry && y0 >= 1) { cys[1] = y0 - 1; ncy = 2; }
+    else if (y0 + 1 - ye < ry && y0 + 1 <= H - 2) { cys[1] = y0 + 1; ncy = 2; }
+    /* nominal terms (only meaningful if valid) */
+    double rho0 = 0.0, gt0[6] = {0, 0, 0, 0, 0, 0}, gs0[6] = {0, 0, 0, 0, 0, 0}, d0, dd0[2], Dm;
+    orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, x0, y0, 1, lambda, delta, &rho0, gt0, gs0, &d0, dd0, &Dm);
+    const int inside0 = d0 <= lambda;
+    if (!inside0) orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, x0, y0, 0, lambda, delta, &rho0, gt0, gs0, &d0, dd0, &Dm);
+    const double rd = fabs(dd0[0]) * rx + fabs(dd0[1]) * ry + 6.0 * ORC_U32 * Dm;
+    const int lam_unsure = fabs(d0 - lambda) <= rd;
+    if (valid && check) {
+      check[0] += rho0; check[1] += 1.0;
+      for (int i = 0; i < 6; ++i) { check[2 + i] += gt0[i]; check[8 + i] += gs0[i]; }
+    }
+    if (valid) { double a = orc_norm6(gt0, NULL), b = orc_norm6(gs0, NULL); Qt += a * a; Qs += b * b; }
+    if (!valid) { rho0 = 0.0; for (int i = 0; i < 6; ++i) gt0[i] = gs0[i] = 0.0; }
+    if (!edge_near && ncx == 1 && ncy == 1 && !lam_unsure) continue;               /* nothing discrete in reach */
+    flagged++;
+    if (edge_near) { if (valid) k_out++; else k_in++; }
+    double wt = 0.0, ws = 0.0, wr = 0.0;
+    if (valid && edge_near) { wt = orc_norm6(gt0, NULL); ws = orc_norm6(gs0, NULL); wr = rho0; }   /* dropped */
+    for (int ix = 0; ix < ncx; ++ix)
+      for (int iy = 0; iy < ncy; ++iy)
+        for (int br = 0; br < 2; ++br) {
+          const int inside = br == 0 ? inside0 : !inside0;
+          if (br == 1 && !lam_unsure) continue;
+          double rho1, gt1[6], gs1[6], d1, dd1[2], Dm1;
+          orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, cxs[ix], cys[iy], inside, lambda, delta, &rho1, gt1, gs1, &d1, dd1, &Dm1);
+          double a = orc_norm6(gt1, gt0), b = orc_norm6(gs1, gs0), c = fabs(rho1 - rho0);
+          if (a > wt) wt = a;
+          if (b > ws) ws = b;
+          if (c > wr) wr = c;
+        }
+    Et += wt; Es += ws; Er += wr;
+  }
+  out[0] = Et; out[1] = Es; out[2] = Er; out[3] = k_out; out[4] = k_in; out[5] = flagged; out[6] = Qt; out[7] = Qs;
+}
+
+/* Whole list: per-camera gradient slack [N], per-pair loss slack [P], per-pair (k_out, k_in, flagged) [P][3].
+ * pair_valid / pair_G are the nominal results of orc_loss_grad on the same inputs (pair_G [P][12] un-normalised). */
+void orc_event_slack(int N, int W, int H, const float* K, const double* poses, const int32_t* edge_off,
+                     const uint16_t* uv, const float* z, const float* dtf, int64_t P, const int32_t* pairs,
+                     double lambda, double delta, double z_min, const double* pair_loss, const int32_t* pair_valid,
+                     const double* pair_G, double* cam_slack, double* pair_loss_slack, int32_t* pair_flags,
+                     double* cam_rss /* [N]: root-sum-square of the terms of each camera's gradient (reading T2) */) {
+  double* bt = (double*)malloc((size_t)P * sizeof(double));
+  double* bs = (double*)malloc((size_t)P * sizeof(double));
+  double* qt = (double*)malloc((size_t)P * sizeof(double));
+  double* qs = (double*)malloc((size_t)P * sizeof(double));
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t p = 0; p < P; ++p) {
+    int s = pairs[2 * p], t = pairs[2 * p + 1];
+    double Ks[4], Kt[4], o[8];
+    for (int i = 0; i < 4; ++i) { Ks[i] = K[4 * s + i]; Kt[i] = K[4 * t + i]; }
+    orc_pair_event_slack(W, H, edge_off[s + 1] - edge_off[s], uv + 2 * (size_t)edge_off[s], z + edge_off[s], Ks, Kt,
+                         poses + 12 * (size_t)s, poses + 12 * (size_t)t, dtf + (size_t)t * W * H, lambda, delta, z_min, o, NULL);
+    const double n = (double)pair_valid[p], k_out = o[3], k_in = o[4], kmax = k_out > k_in ? k_out : k_in;
+    const double n_lo = n - k_out >= 1.0 ? n - k_out : 1.0;
+    const double Gt = orc_norm6(pair_G + 12 * p, NULL), Gs = orc_norm6(pair_G + 12 * p + 6, NULL);
+    bt[p] = o[0] / n_lo + (n > 0.0 ? Gt * kmax / (n * n_lo) : 0.0);
+    bs[p] = o[1] / n_lo + (n > 0.0 ? Gs * kmax / (n * n_lo) : 0.0);
+    pair_loss_slack[p] = o[2] / n_lo + (n > 0.0 ? pair_loss[p] * kmax / n_lo : 0.0);
+    pair_flags[3 * p] = (int32_t)k_out; pair_flags[3 * p + 1] = (int32_t)k_in; pair_flags[3 * p + 2] = (int32_t)o[5];
+    qt[p] = n > 0.0 ? o[6] / (n * n) : 0.0; qs[p] = n > 0.0 ? o[7] / (n * n) : 0.0;
+  }
+  for (int i = 0; i < N; ++i) cam_slack[i] = cam_rss[i] = 0.0;
+  for (int64_t p = 0; p < P; ++p) {
+    cam_slack[pairs[2 * p + 1]] += bt[p]; cam_slack[pairs[2 * p]] += bs[p];
+    cam_rss[pairs[2 * p + 1]] += qt[p]; cam_rss[pairs[2 * p]] += qs[p];
+  }
+  for (int i = 0; i < N; ++i) { cam_slack[i] /= (double)P; cam_rss[i] = sqrt(cam_rss[i]) / (double)P; }
+  free(bt); free(bs); free(qt); free(qs);
+}
+
 /* =================================================================================================
  * Edge extraction: "the edge map E_i via the Canny edge detector [4]" (Alg. 1 l.6).
  * The paper names the detector and nothing else; this is Canny's scheme [4] -- smooth, gradient, non-maximum
@@ -727,6 +918,10 @@ int64_t orc_pair_subset(uint64_t seed, int step, int64_t P, int64_t M, uint8_t* 
   return M;
 }
 
+/* =================================================================================================
+ * O7  Schedules, Adam, SE(3) exponential  (PAPER.md:121, 429, 462-463; readings S4, S10, S11)
+ * ================================================================================================= */
+/* clamp lambda: clamp_start -> clamp_end linearly over the first clamp_steps steps  (PAPER.md:462) */
 double orc_lambda(int s, double clamp_start, double clamp_end, int clamp_steps) {
   int m = s < clamp_steps ? s : clamp_steps;
   return clamp_start + (clamp_end - clamp_start) * (double)m / (double)clamp_steps;

@@ -1,7 +1,8 @@
 #!/usr/bin/env python
 """Writes tests/golden/tiny_expected.txt: loss, per-pair losses / valid counts and per-camera gradients of
 BASELINE.json config 1 (seeded Tiny scene) at its initial poses, for lambda = 10 and 6, and the poses after 200
-fixed iterations -- as computed by the CPU ORACLE (fp32-position variant, reading P1).
+fixed iterations -- as computed by the all-double CPU ORACLE, with the oracle's own event slack (reading T1:
+what a binary32 evaluation may decide differently; for this scene a handful of samples).
 
 Calls only `oracle/` and `epo_scenes/` (never the CUDA path).  Re-run after a justified change of the oracle:
     python tests/golden/make_golden.py
@@ -22,18 +23,23 @@ def main():
     sc = make_scene(1)
     zmin = f32(1e-6)
     prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=zmin)
-    out = ["# written by tests/golden/make_golden.py from oracle/ only (config 1, fp32-position variant)"]
+    out = ["# written by tests/golden/make_golden.py from oracle/ only (config 1, all-double oracle + its event slack)"]
     out.append("edge_off " + " ".join(str(int(x)) for x in prob.edge_off))
     for lam in (10.0, 6.0):
-        r = oracle.loss_grad(prob, sc.poses_init.astype(np.float64), sc.pairs, lam, z_min=zmin, coord_fp32=1)
+        r = oracle.loss_grad(prob, sc.poses_init.astype(np.float64), sc.pairs, lam, z_min=zmin, want_pair_G=True)
+        sl = oracle.event_slack(prob, sc.poses_init.astype(np.float64), sc.pairs, lam, r, z_min=zmin)
         out.append(f"lambda {lam!r}")
         out.append("loss " + repr(float(r["loss"])))
         out.append("pair_valid " + " ".join(str(int(x)) for x in r["pair_valid"]))
         out.append("pair_loss " + " ".join(repr(float(x)) for x in r["pair_loss"]))
         for c in range(sc.n_views):
             out.append(f"grad {c} " + " ".join(repr(float(x)) for x in r["grad"][c]))
+        out.append("slack_k_out " + " ".join(str(int(x)) for x in sl["k_out"]))
+        out.append("slack_k_in " + " ".join(str(int(x)) for x in sl["k_in"]))
+        out.append("slack_pair_loss " + " ".join(repr(float(x)) for x in sl["pair_loss"]))
+        out.append("slack_cam " + " ".join(repr(float(x)) for x in sl["cam"]))
     cfg = oracle.Config(lr_max=f32(3e-3), beta1=f32(0.9), beta2=f32(0.999), adam_eps=f32(1e-8), eps1=f32(0.5),
-                        eps2=f32(0.1), z_min=zmin, early_stop=0, coord_fp32=1)
+                        eps2=f32(0.1), z_min=zmin, early_stop=0)
     opt = oracle.Optimizer(prob, sc.poses_init, sc.pairs, cfg)
     assert opt.run(200)[0] == 200
     for c in range(sc.n_views):

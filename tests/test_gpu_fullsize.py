@@ -7,7 +7,8 @@ import pytest
 
 import oracle
 from epo_scenes import make_scene
-from parity_utils import Z_MIN, check_camera_grads, check_pair_losses, make_ctx, oracle_config, pose_errors
+from parity_utils import (Z_MIN, check_loss_grad, fmt_lockstep, fmt_report, lockstep, make_ctx, oracle_config, oracle_eval,
+                          pose_errors)
 
 pytestmark = pytest.mark.gpu
 
@@ -43,38 +44,39 @@ def test_full_size_loss_gradient_and_preprocessing(config):
     cp, perm = e.get_pair_order()
     ocp, operm = oracle.canonical_pairs(sc.pairs)
     assert np.array_equal(cp, ocp) and np.array_equal(perm, operm)
-    # loss + gradient, all pairs, all cameras
+    # loss + gradient, all pairs, all cameras, against the all-double oracle (+ its event slack, parity_utils)
     poses = sc.poses_init.astype(np.float64)
     for lam in (10.0, 6.0):
         got = e.loss_grad(lam)
-        ref32 = oracle.loss_grad(prob, poses, sc.pairs, lam, z_min=Z_MIN, coord_fp32=1)
-        assert np.array_equal(got["pair_valid"], ref32["pair_valid"])
-        w32 = check_pair_losses(got["pair_loss"], got["pair_valid"], ref32, lam, max_event_frac=0.0)
-        assert abs(got["loss"] - ref32["loss"]) <= 1e-5 * abs(ref32["loss"])
-        g32 = check_camera_grads(got["grad"], ref32["grad"])
-        print(f"config {config} full size lam={lam}: {len(sc.pairs)} pairs, {int(got['pair_valid'].sum())} valid samples; "
-              f"pair loss rel err {w32:.2e}, camera grad rel err {g32:.2e}")
-    ref64 = oracle.loss_grad(prob, poses, sc.pairs, 10.0, z_min=Z_MIN)
-    got = e.loss_grad(10.0)
-    check_pair_losses(got["pair_loss"], got["pair_valid"], ref64, 10.0)
+        ref, sl = oracle_eval(prob, poses, sc.pairs, lam)
+        rep = check_loss_grad(got, ref, sl, what=f"config {config} lam={lam}")
+        print(f"config {config} full size lam={lam}: {len(sc.pairs)} pairs, {int(got['pair_valid'].sum())} valid samples; {fmt_report(rep)}")
+        assert rep["flagged_frac"] <= 1e-2 and rep["slack_rel_median"] <= 1e-1
     # three lock-step iterations of the loop at full size
-    ocfg = oracle_config(coord_fp32=1, early_stop=0)
-    m = np.zeros((N, 6)); v = np.zeros((N, 6))
-    P = e.get_poses_f64()
-    for k in range(3):
-        ref = oracle.loss_grad(prob, P, sc.pairs, oracle.lam_schedule(k, ocfg), z_min=Z_MIN, coord_fp32=1)
-        inc = oracle.adam(ref["grad"].reshape(-1), m.reshape(-1), v.reshape(-1), k, oracle.lr_schedule(k, ocfg),
-                          ocfg.beta1, ocfg.beta2, ocfg.adam_eps).reshape(N, 6)
-        pred = np.stack([oracle.se3_compose(oracle.se3_exp(inc[c]), P[c]) for c in range(N)])
-        assert e.step(1)[0] == 1
-        new = e.get_poses_f64()
-        rot, tr = pose_errors(new, pred)
-        loss, theta = e.get_trace(k, 1)
-        assert rot <= 1e-3 and tr <= 1e-4, (k, rot, tr)
-        assert abs(float(loss[0]) - ref["loss"]) <= 1e-5 * abs(ref["loss"])
-        th = oracle.theta95(pred, P)
-        assert abs(float(theta[0]) - th) <= 1e-3 * th + 1e-7
-        P = new
+    worst, _, n = lockstep(sc, e, 3, oracle_config(early_stop=0), prob=prob, label=f"config {config}")
+    assert n == 3
+    print(f"config {config} full size, 3 lock-step iterations: {fmt_lockstep(worst)}")
+    e.destroy()
+
+
+@pytest.mark.parametrize("config", [2, 3, 4, 5])
+def test_full_size_free_running_prefix(config):
+    """The first 25 iterations, free-running on both sides (no re-synchronisation), at full size, against the all-double
+    oracle: final poses within the contract's 1e-3 degrees / 1e-4 scene units where binary32 can meet that at all --
+    else within 3x the distance at which the oracle's own binary32-position variant ends (one-step differences of a
+    few 1e-4 degrees, see the lock-step test above, accumulate over 25 steps); the loss trace within 1e-4."""
+    sc, e, prob = _full(config, early_stop=0)
+    opt = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0))
+    o32 = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0, coord_fp32=1))
+    assert e.step(25)[0] == 25 and opt.run(25)[0] == 25 and o32.run(25)[0] == 25
+    rot, tr = pose_errors(e.get_poses_f64(), opt.poses)
+    orot, otr = pose_errors(o32.poses, opt.poses)
+    loss, _ = e.get_trace(0, 25)
+    lrel = float(np.max(np.abs(loss - opt.loss[:25]) / opt.loss[:25]))
+    print(f"config {config} full size, 25 free-running iterations vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e}, "
+          f"loss trace rel {lrel:.2e} (the oracle's own binary32-position variant: rot {orot:.2e}, trans {otr:.2e})")
+    assert rot <= max(1e-3, 3 * orot) and tr <= max(1e-4, 3 * otr)
+    assert lrel <= 1e-4
     e.destroy()
 
 
@@ -83,14 +85,19 @@ def test_full_size_config4_fp16_fields():
     sc, e, prob = _full(4, dtf_format=1)
     poses = sc.poses_init.astype(np.float64)
     got = e.loss_grad(10.0)
-    ref = oracle.loss_grad(prob, poses, sc.pairs, 10.0, z_min=Z_MIN)
-    check_pair_losses(got["pair_loss"], got["pair_valid"], ref, 10.0, rtol=1e-3)
+    ref, sl = oracle_eval(prob, poses, sc.pairs, 10.0)
+    assert np.all(got["pair_valid"] >= ref["pair_valid"] - sl["k_out"]) and np.all(got["pair_valid"] <= ref["pair_valid"] + sl["k_in"])
+    assert np.all(np.abs(got["pair_loss"] - ref["pair_loss"]) <= 1e-3 * ref["pair_loss"] + sl["pair_loss"])
     assert abs(got["loss"] - ref["loss"]) <= 1e-3 * abs(ref["loss"])
     err = np.linalg.norm(got["grad"] - ref["grad"], axis=1) / np.linalg.norm(ref["grad"], axis=1)
-    print(f"config 4 fp16 fields: loss rel err {abs(got['loss'] - ref['loss']) / ref['loss']:.2e}, camera grad rel err max {err.max():.2e}")
-    # the fp16 field's gradient differs from the fp32 field's by the rounding of neighbouring taps (2^-11 relative
-    # on values up to ~100 px against differences of ~1 px): reported, bounded loosely
-    assert err.max() <= 5e-2
+    # parity of the fp16 PATH: the all-double oracle on the RNE-rounded field (what the kernel samples), standard
+    # tolerances.  How far the rounded field's gradient is from the fp32 field's is a property of the variant
+    # (2^-11 relative on taps of up to ~100 px against tap differences of ~1 px), reported, not a parity claim.
+    prob_h = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN, half=True)
+    ref_h, sl_h = oracle_eval(prob_h, poses, sc.pairs, 10.0)
+    rep = check_loss_grad(got, ref_h, sl_h, what="config 4 fp16 fields")
+    print(f"config 4 fp16 fields: vs the oracle on the rounded field: {fmt_report(rep)}; vs the fp32-field oracle: loss rel err "
+          f"{abs(got['loss'] - ref['loss']) / ref['loss']:.2e}, camera grad rel err max {err.max():.2e} (the variant's own deviation)")
     e.destroy()
 
 
@@ -125,23 +132,9 @@ def test_full_size_config4_stochastic_pair_subsampling():
     for step in (0, 1, 500):
         got = e.get_pair_subset(step)
         assert got.sum() == M and np.array_equal(got, oracle.pair_subset(seed, step, Pn, M)), step
-    ocfg = oracle_config(coord_fp32=1, early_stop=0)
-    N = sc.n_views
-    m = np.zeros((N, 6)); v = np.zeros((N, 6))
-    P = e.get_poses_f64()
-    for k in range(3):
-        pairs_k = sc.pairs[oracle.pair_subset(seed, k, Pn, M)]
-        ref = oracle.loss_grad(prob, P, pairs_k, oracle.lam_schedule(k, ocfg), z_min=Z_MIN, coord_fp32=1)
-        inc = oracle.adam(ref["grad"].reshape(-1), m.reshape(-1), v.reshape(-1), k, oracle.lr_schedule(k, ocfg),
-                          ocfg.beta1, ocfg.beta2, ocfg.adam_eps).reshape(N, 6)
-        pred = np.stack([oracle.se3_compose(oracle.se3_exp(inc[c]), P[c]) for c in range(N)])
-        assert e.step(1)[0] == 1
-        new = e.get_poses_f64()
-        rot, tr = pose_errors(new, pred)
-        loss, _ = e.get_trace(k, 1)
-        assert rot <= 1e-3 and tr <= 1e-4, (k, rot, tr)
-        assert abs(float(loss[0]) - ref["loss"]) <= 1e-5 * abs(ref["loss"]), (k, float(loss[0]), ref["loss"])
-        P = new
+    worst, _, n = lockstep(sc, e, 3, oracle_config(early_stop=0), budget=M, seed=seed, prob=prob, label="config 4, M = 1024")
+    assert n == 3
+    print(f"config 4 with M = 1024, 3 lock-step iterations: {fmt_lockstep(worst)}")
     e.destroy()
 
 
