@@ -568,8 +568,20 @@ void orc_pair_event_slack(int W, int H, int n_edges, const uint16_t* uv, const f
     const double eX = 8.0 * ORC_U32 * S3[0], eY = 8.0 * ORC_U32 * S3[1], eZ = 8.0 * ORC_U32 * S3[2];
     const int z_ok = xt[2] > z_min, z_unsure = fabs(xt[2] - z_min) <= eZ;
     if (!z_ok && !z_unsure) continue;                  /* behind the camera on both sides */
-    /* a depth within rounding of z_min gives an unbounded position: only the count can be bounded */
-    if (z_unsure) { flagged++; if (z_ok) k_out++; else k_in++; Et = Es = Er = INFINITY; continue; }
+    /* A depth within rounding of z_min: with z' <= z + |dZ| the projection is at least fx (|X| - |dX|) / (z + |dZ|) away
+     * from the principal point -- far outside the image unless the point sits on the optical centre itself.  Then the
+     * sample is invalid on both sides whatever z' is; otherwise nothing bounds its position and the slack is infinite. */
+    if (z_unsure) {
+      const double z_hi = xt[2] + eZ;
+      const double ax = fabs(xt[0]) - eX, ay = fabs(xt[1]) - eY;
+      const double far_x = fabs(Kt[2]) + fabs(xmax - Kt[2]) + 1.0, far_y = fabs(Kt[3]) + fabs(ymax - Kt[3]) + 1.0;
+      if (z_hi > 0.0 && ((ax > 0.0 && Kt[0] * ax / z_hi > far_x) || (ay > 0.0 && Kt[1] * ay / z_hi > far_y))) {
+        if (!z_ok) continue;                           /* invalid here, and outside the image for any z' > z_min */
+        /* valid-by-depth here: it continues below and is found outside the image */
+      } else {
+        flagged++; if (z_ok) k_out++; else k_in++; Et = Es = Er = INFINITY; continue;
+      }
+    }
     double px[2];
     orc_project_px(Kt, xt, px);
     const double x = px[0], y = px[1];

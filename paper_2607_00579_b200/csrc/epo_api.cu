@@ -62,6 +62,7 @@ void free_views(epo_ctx* c) {
   epo_dfree(c, c->d_edge_off); epo_dfree(c, c->d_edges); epo_dfree(c, c->d_pts); epo_dfree(c, c->d_depth);
   c->d_depth = nullptr;
   epo_free_atlas(&c->atlas);
+  epo_free_packed(c, &c->packed);
   epo_joint_free(c);
   c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_pts = nullptr;
   c->have_views = false;
@@ -148,6 +149,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   c->err[0] = 0;
   c->pool = nullptr; c->own_pool = false;
   c->atlas = EpoAtlas{nullptr, nullptr, 0, 0, 1};
+  c->packed.xyz = nullptr; c->packed.d_off = nullptr;
   { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
   c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
@@ -271,6 +273,9 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff, &subsampled);
   tr.mark("edge lists");
   if (rc == EPO_OK) rc = epo_build_points(c, d_small, off, rec, E, hoff, d_e, d_depth, subsampled, &pts);
+  EpoPacked packed = {nullptr, nullptr, {}};
+  if (rc == EPO_OK) rc = epo_alloc_packed(c, hoff, &packed);
+  if (rc == EPO_OK) rc = epo_launch_pack_points(c, pts, off, packed);
   if (rc == EPO_OK) {
     // commit the small state on the stream, then drain it once
     e = cudaMemcpyAsync(c->d_K, d_small, N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, st);
@@ -293,12 +298,12 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
     // d_K / d_poses may have been overwritten only if every build step succeeded and the final drain failed
     // (a sticky CUDA error: the context is unusable anyway)
     cudaGetLastError();
-    epo_dfree(c, off); epo_dfree(c, rec); epo_dfree(c, pts); epo_free_atlas(&atlas);
+    epo_dfree(c, off); epo_dfree(c, rec); epo_dfree(c, pts); epo_free_atlas(&atlas); epo_free_packed(c, &packed);
     return rc;
   }
   free_pairs(c); free_views(c);
   c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff;
-  c->d_pts = pts; c->atlas = atlas; c->d_depth = d_depth;
+  c->d_pts = pts; c->atlas = atlas; c->d_depth = d_depth; c->packed = packed;
   c->have_views = true; c->static_dirty = true;
   EPO_TRY(epo_joint_alloc(c));                      // joint loop: variables at the identity, Z0 and K0 kept
   tr.mark("free temporaries");
@@ -780,16 +785,25 @@ static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flu
   cudaStream_t st = c->stream;
   const size_t flush_bytes = (size_t)256 << 20;   // > 126 MB L2
   void* flush = nullptr;
+  uint2* taps = nullptr; unsigned* gout = nullptr;
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (flush_l2) EPO_CUDA(c, epo_dmalloc(c, &flush, flush_bytes));
   cudaError_t e = cudaEventCreate(&e0);
   if (e == cudaSuccess) e = cudaEventCreate(&e1);
-  double sum = 0.0; float mn = 1e30f;
   epo_status rc = EPO_OK;
+  const size_t n_items = (size_t)(c->n_work > 0 ? c->n_work : 1);
+  if (gather_only && e == cudaSuccess) {
+    // the tap stream of this evaluation, recorded once by the fused kernel's own position arithmetic
+    e = epo_dmalloc(c, &taps, n_items * (size_t)(c->lg_chunk / 2) * sizeof(uint2));
+    if (e == cudaSuccess) e = epo_dmalloc(c, &gout, n_items * sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemsetAsync(gout, 0, n_items * sizeof(unsigned), st);
+    if (e == cudaSuccess) rc = epo_launch_record_taps(c, lambda, taps);
+  }
+  double sum = 0.0; float mn = 1e30f;
   for (int r = 0; r < reps && e == cudaSuccess && rc == EPO_OK; ++r) {
     if (flush) e = cudaMemsetAsync(flush, r & 0xff, flush_bytes, st);
     if (e == cudaSuccess) e = cudaEventRecord(e0, st);
-    if (e == cudaSuccess) rc = epo_launch_fused_only(c, lambda, gather_only);
+    if (e == cudaSuccess) rc = gather_only ? epo_launch_gather_taps(c, lambda, taps, gout) : epo_launch_fused_only(c, lambda);
     if (e == cudaSuccess) e = cudaEventRecord(e1, st);
     if (e == cudaSuccess) e = cudaEventSynchronize(e1);
     float ms = 0.f;
@@ -797,11 +811,11 @@ static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flu
     sum += ms; if (ms < mn) mn = ms;
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  epo_dfree(c, flush);
+  epo_dfree(c, flush); epo_dfree(c, taps); epo_dfree(c, gout);
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
   if (rc != EPO_OK) return rc;
-  if (e != cudaSuccess) return epo_fail(c, EPO_ERR_CUDA, "epo_time_loss_grad_kernel: %s", cudaGetErrorString(e));
+  if (e != cudaSuccess) return epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_time_loss_grad_kernel: %s", cudaGetErrorString(e));
   if (ms_mean) *ms_mean = (float)(sum / reps);
   if (ms_min) *ms_min = mn;
   return EPO_OK;

@@ -34,6 +34,9 @@ constexpr int kAccStride = 8;
 #ifndef EPO_LG_MINBLOCKS
 #define EPO_LG_MINBLOCKS 7
 #endif
+#ifndef EPO_LG_L2PF
+#define EPO_LG_L2PF 2                         // passes ahead the fused kernel prefetches its points into L2 (0 = off)
+#endif
 constexpr int kLgThreads = EPO_LG_THREADS;
 constexpr int kLgPerThread = EPO_LG_PER_THREAD;
 constexpr int kLgOuter = EPO_LG_OUTER;        // most passes per work item (epo_ctx::lg_chunk is what runs)
@@ -72,6 +75,20 @@ struct EpoAtlas {
 };
 constexpr float kU8LambdaMax = 14.5f;
 
+// The camera-frame points as the packed fused kernel reads them.  "Slot" j holds two samples; view i owns the slots
+// [off[i] / 2, off[i+1] / 2), off[i+1] - off[i] = its edge count rounded up to a multiple of kLgPass (padding = zero
+// points, never counted), and inside a view slot j = 32 g + l holds the samples 64 g + l and 64 g + 32 + l of the
+// tile-major list: a warp's load is one contiguous 256-byte row and each of its two gathers covers 32 CONSECUTIVE
+// points.  The three coordinates of a block of kLgThreads slots are stored as three consecutive planes,
+//   float2 index of (slot j, coordinate c) = (j / kLgThreads) * 3 * kLgThreads + c * kLgThreads + j % kLgThreads,
+// so that a CTA's pass is three loads at immediate offsets from ONE running pointer.  kLgPad / 2 zero slots follow the
+// last view (the first-pass loads of a short last work item read past its list).
+struct EpoPacked {
+  float2* xyz;
+  int32_t* d_off;               // [N+1] device copy of h_off
+  std::vector<int32_t> h_off;   // [N+1] in samples, multiples of kLgPass
+};
+
 struct epo_ctx {
   epo_config cfg;
   cudaStream_t stream;
@@ -102,7 +119,8 @@ struct epo_ctx {
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
   float* d_depth;         // [N][H][W] the depth maps as given (kept for epo_build_viewgraph)
-  float4* d_pts;          // [E] camera-frame points (x_s, y_s, z_s, 0): K and Z are fixed, so row a-2 is hoisted
+  float4* d_pts;          // [E] camera-frame points (x_s, y_s, z_s, pixel index): K and Z are fixed, so row a-2 is hoisted
+  EpoPacked packed;       // the same points in the fused kernel's layout (rebuilt whenever d_pts changes)
   EpoAtlas atlas;         // the distance fields as the fused kernel samples them (see EpoAtlas)
   std::vector<int32_t> h_edge_off;
 
@@ -203,6 +221,9 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
                             const std::vector<int32_t>& h_off, const uint8_t* d_edges_u8, const float* d_depth,
                             bool subsampled, float4** out_pts);
 void epo_free_atlas(EpoAtlas* atlas);
+epo_status epo_alloc_packed(epo_ctx* ctx, const std::vector<int32_t>& h_edge_off, EpoPacked* out);
+void epo_free_packed(epo_ctx* ctx, EpoPacked* pk);
+epo_status epo_launch_pack_points(epo_ctx* ctx, const float4* d_pts, const int32_t* d_edge_off, const EpoPacked& pk);
 // pairs.cu
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
@@ -232,7 +253,9 @@ epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_f
 // lossgrad.cu
 epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);
 epo_status epo_launch_fused_joint(epo_ctx* ctx, float lambda, double* d_g_logf, float* d_g_depth, bool in_loop);   // joint-phase pass
-epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda, bool gather_only);   // the fused kernel alone (measurement hooks)
+epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)
+epo_status epo_launch_record_taps(epo_ctx* ctx, float lambda, uint2* d_taps);                  // gather ceiling: the tap stream
+epo_status epo_launch_gather_taps(epo_ctx* ctx, float lambda, const uint2* d_taps, unsigned* d_out);   // ... replayed alone
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
 epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset);
 epo_status epo_launch_fill_schedule(epo_ctx* ctx);     // d_sched from the configuration (once, in epo_create)

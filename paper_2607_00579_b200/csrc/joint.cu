@@ -179,6 +179,7 @@ epo_status epo_joint_reset(epo_ctx* c) {
     dim3 grid((unsigned)std::min((m + 255) / 256, 64), (unsigned)c->N);
     k_joint_points<<<grid, 256, 0, c->stream>>>(q);
     c->launches += 2;
+    EPO_TRY(epo_launch_pack_points(c, c->d_pts, c->d_edge_off, c->packed));
   }
   EPO_CUDA(c, cudaGetLastError());
   return EPO_OK;
@@ -198,6 +199,7 @@ epo_status epo_launch_joint_update(epo_ctx* c) {
   dim3 grid((unsigned)std::min((m + 255) / 256, 64), (unsigned)c->N);
   k_joint_points<<<grid, 256, 0, c->stream>>>(q);
   c->launches += 2;
+  EPO_TRY(epo_launch_pack_points(c, c->d_pts, c->d_edge_off, c->packed));    // the fused kernel's copy of the points
   EPO_CUDA(c, cudaGetLastError());
   return EPO_OK;
 }

@@ -90,17 +90,19 @@ __global__ void k_chunk_counts(const int2* __restrict__ canon, const int32_t* __
   cnt[p] = (n + chunk - 1) / chunk;
 }
 
-// work item = {source | target << 16, canonical pair index, first point of the chunk (absolute index into the point
-// list), samples of the source's list from there on}: the fused kernel needs no other table before it can start
+// work item = {source | target << 16, canonical pair index, first slot of the chunk in the packed point array
+// (absolute, a multiple of kLgThreads: EpoPacked), samples of the source's list from there on}: the fused kernel needs no other table before it can start
 // loading points (N <= 65535 is checked in epo_create)
 __global__ void k_fill_work(const int32_t* __restrict__ work_off, const int2* __restrict__ canon,
-                            const int32_t* __restrict__ edge_off, int64_t P, int chunk, int4* __restrict__ work) {
+                            const int32_t* __restrict__ edge_off, const int32_t* __restrict__ pk_off, int64_t P, int chunk,
+                            int4* __restrict__ work) {
   int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= P) return;
   const int2 st = canon[p];
-  const int e0 = edge_off[st.x], n = edge_off[st.x + 1] - e0;
+  const int n = edge_off[st.x + 1] - edge_off[st.x];
+  const int e0 = pk_off[st.x] / 2;                   // slots of the packed point array (EpoPacked)
   int lo = work_off[p], hi = work_off[p + 1];
-  for (int w = lo; w < hi; ++w) work[w] = make_int4(st.x | (st.y << 16), (int)p, e0 + (w - lo) * chunk, n - (w - lo) * chunk);
+  for (int w = lo; w < hi; ++w) work[w] = make_int4(st.x | (st.y << 16), (int)p, e0 + (w - lo) * (chunk / 2), n - (w - lo) * chunk);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -353,7 +355,7 @@ epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user, int64_t P, int2*
   PR_CUDA(cudaMemcpyAsync(&n_work, work_off + P, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   PR_CUDA(cudaStreamSynchronize(st));
   PR_CUDA(epo_dmalloc(ctx, &work, (size_t)(n_work > 0 ? n_work : 1) * sizeof(int4)));
-  k_fill_work<<<gridP, 256, 0, st>>>(work_off, canon, ctx->d_edge_off, P, chunk, work);
+  k_fill_work<<<gridP, 256, 0, st>>>(work_off, canon, ctx->d_edge_off, ctx->packed.d_off, P, chunk, work);
   ctx->launches += 1;
   PR_CUDA(cudaGetLastError());
   free_tmp();

@@ -5,6 +5,8 @@
 #include <climits>
 #include <cstring>
 
+#include <algorithm>
+
 #include "epo_internal.h"
 
 namespace {
@@ -294,7 +296,58 @@ __global__ void k_tile_points(const uint8_t* __restrict__ edges, const float* __
 }
 
 
+// tile-major float4 points -> the packed layout (EpoPacked): thread = one slot (two samples) of one view
+__global__ void k_pack_points(const float4* __restrict__ pts, const int32_t* __restrict__ edge_off,
+                              const int32_t* __restrict__ pk_off, float2* __restrict__ xyz) {
+  const int view = blockIdx.y;
+  const int lo = edge_off[view], n = edge_off[view + 1] - lo;
+  const int slots = (pk_off[view + 1] - pk_off[view]) / 2;
+  const size_t base = (size_t)pk_off[view] / 2;
+  for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < slots; j += gridDim.x * blockDim.x) {
+    const int a = 64 * (j >> 5) + (j & 31), b = a + 32;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 pa = a < n ? pts[(size_t)lo + a] : zero, pb = b < n ? pts[(size_t)lo + b] : zero;
+    const size_t s = base + j, o = s / kLgThreads * (3 * kLgThreads) + s % kLgThreads;
+    xyz[o] = make_float2(pa.x, pb.x); xyz[o + kLgThreads] = make_float2(pa.y, pb.y); xyz[o + 2 * kLgThreads] = make_float2(pa.z, pb.z);
+  }
+}
+
 }  // namespace
+
+epo_status epo_alloc_packed(epo_ctx* ctx, const std::vector<int32_t>& h_edge_off, EpoPacked* out) {
+  EpoPacked pk = {nullptr, nullptr, {}};
+  const int N = ctx->N;
+  pk.h_off.assign((size_t)N + 1, 0);
+  for (int i = 0; i < N; ++i) pk.h_off[i + 1] = pk.h_off[i] + (h_edge_off[i + 1] - h_edge_off[i] + kLgPass - 1) / kLgPass * kLgPass;
+  const size_t used = (size_t)pk.h_off[N] / 2 * 3, all = used + (size_t)kLgPad / 2 * 3;     // float2 entries
+  cudaError_t e = epo_dmalloc(ctx, &pk.xyz, all * sizeof(float2));
+  if (e == cudaSuccess) e = epo_dmalloc(ctx, &pk.d_off, ((size_t)N + 1) * sizeof(int32_t));
+  if (e == cudaSuccess) e = cudaMemsetAsync(pk.xyz + used, 0, (all - used) * sizeof(float2), ctx->stream);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(pk.d_off, pk.h_off.data(), ((size_t)N + 1) * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);      // h_off is copied from this frame
+  if (e != cudaSuccess) {
+    epo_free_packed(ctx, &pk);
+    return epo_fail(ctx, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "packed points: %s", cudaGetErrorString(e));
+  }
+  *out = pk;
+  return EPO_OK;
+}
+
+void epo_free_packed(epo_ctx* ctx, EpoPacked* pk) {
+  epo_dfree(ctx, pk->xyz); epo_dfree(ctx, pk->d_off);
+  pk->xyz = nullptr; pk->d_off = nullptr; pk->h_off.clear();
+}
+
+epo_status epo_launch_pack_points(epo_ctx* ctx, const float4* d_pts, const int32_t* d_edge_off, const EpoPacked& pk) {
+  int max_slots = 1;
+  for (int i = 0; i < ctx->N; ++i) max_slots = std::max(max_slots, (pk.h_off[i + 1] - pk.h_off[i]) / 2);
+  dim3 grid((unsigned)std::min((max_slots + 255) / 256, 64), (unsigned)ctx->N);
+  k_pack_points<<<grid, 256, 0, ctx->stream>>>(d_pts, d_edge_off, pk.d_off, pk.xyz);
+  ctx->launches += 1;
+  EPO_CUDA(ctx, cudaGetLastError());
+  return EPO_OK;
+}
 
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
                                 int32_t** out_off, EdgeRec** out_rec, int64_t* out_E,
