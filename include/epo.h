@@ -91,8 +91,9 @@ typedef struct {
                                        (PAPER.md:64, 78-87): a focal scale per camera, f = f0 (1 + gamma) (Eq. 4), from the
                                        first iteration, and the affine depth Z = Z0 alpha + beta (Eq. 5) of every listed
                                        edge pixel in iterations that start in phase >= 1; AdamW with the loop's learning
-                                       rate and weight_decay towards the identity.  An iteration then runs the fused
-                                       kernel twice (loss + pose gradient, then the joint gradients).                  */
+                                       rate and weight_decay towards the identity.  An iteration is then three launches:
+                                       the fused kernel (which also emits the joint derivatives), the per-camera
+                                       reduction (+ gamma), the per-pixel depth update.  May be combined with pair_budget. */
   float   weight_decay;             /* 0.01                                                          */
   void*   mem_pool;                 /* cudaMemPool_t all device memory of the context is taken from (stream-ordered, on
                                        cfg.stream).  NULL (default): the context creates a private pool and destroys it
@@ -181,8 +182,9 @@ EPO_API epo_status epo_loss_grad(epo_ctx* ctx, float lambda, float* loss, float*
  *   g_depth [N][H][W]  d loss / d Z_c(u, v) at the edge pixels of the lists (0 elsewhere); with Eq. 5, Z = Z0 alpha + beta:
  *                      d loss / d alpha = Z0 g_depth, d loss / d beta = g_depth
  *   loss [1]           nullable: the loss of this evaluation
- * Evaluates all pairs (no sub-sampling).  Sums are accumulated with atomics (run-to-run differences at rounding
- * level).  Does not change poses or optimiser state: this library does not optimise f or Z.
+ * Evaluates all pairs (no sub-sampling), in ONE pass of the fused kernel; every edge pixel's pairs are then summed in a
+ * fixed order (no atomics: bit-reproducible).  Does not change poses, variables or optimiser state (the loop that
+ * optimises f and Z is cfg.joint_phase = 1, see epo_step).
  */
 EPO_API epo_status epo_loss_grad_joint(epo_ctx* ctx, float lambda, float* loss, float* g_logf, float* g_depth);
 

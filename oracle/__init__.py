@@ -119,6 +119,10 @@ def lib():
                                       C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_int32), C.c_double, C.c_double,
                                       C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_double),
                                       C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_double)]
+        L.orc_joint_slack.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
+                                      C.POINTER(C.c_int32), C.POINTER(C.c_uint16), C.POINTER(C.c_float),
+                                      C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_int32), C.c_double, C.c_double,
+                                      C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.orc_joint_grad.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
                                      C.POINTER(C.c_int32), C.POINTER(C.c_uint16), C.POINTER(C.c_float),
                                      C.POINTER(C.c_float), C.c_int64, C.POINTER(C.c_int32), C.c_double, C.c_double,
@@ -347,6 +351,19 @@ def joint_grad(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6, coord_fp
                          C.c_double(lam), C.c_double(delta), C.c_double(z_min), int(coord_fp32), _p(g_f, C.c_double),
                          _p(g_z, C.c_double))
     return g_f, g_z
+
+
+def joint_slack(prob: Problem, poses, pairs, lam, delta=1.0, z_min=1e-6):
+    """Event slack of the joint-phase gradients (see orc_joint_slack): dict(logf [N], logf_rss [N], gz [E])."""
+    N = prob.n_views
+    poses = np.ascontiguousarray(np.asarray(poses, np.float64).reshape(N, 12))
+    pairs = np.ascontiguousarray(pairs, np.int32); P = pairs.shape[0]
+    sf = np.zeros(N); rf = np.zeros(N); sz = np.zeros(int(prob.edge_off[-1]))
+    lib().orc_joint_slack(N, prob.W, prob.H, _p(prob.K, C.c_float), _p(poses, C.c_double), _p(prob.edge_off, C.c_int32),
+                          _p(prob.uv, C.c_uint16), _p(prob.z, C.c_float), _p(prob.dtf, C.c_float), P, _p(pairs, C.c_int32),
+                          C.c_double(lam), C.c_double(delta), C.c_double(z_min), _p(sf, C.c_double), _p(rf, C.c_double),
+                          _p(sz, C.c_double))
+    return dict(logf=sf, logf_rss=rf, gz=sz)
 
 
 # ---------------------------------------------------------------------------------------------- O7

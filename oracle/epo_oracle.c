@@ -509,7 +509,7 @@ void orc_loss_grad(int N, int W, int H, const float* K, const double* poses, con
 static void orc_sample_terms(int W, const float* dtf_t, const double Kt[4], const double Tts[12], const double xs[3],
                              const double xt[3], double x, double y, int x0, int y0, int inside, double lambda,
                              double delta, double* rho, double gt[6], double gs[6], double* d_out, double dd[2],
-                             double* Dmax) {
+                             double* Dmax, double jz[3] /* nullable: d rho / d ln f_t, d rho / d ln f_s, d rho / d Z_s */) {
   double wx = x - x0, wy = y - y0;
   double D00 = dtf_t[(size_t)y0 * W + x0], D01 = dtf_t[(size_t)y0 * W + x0 + 1];
   double D10 = dtf_t[(size_t)(y0 + 1) * W + x0], D11 = dtf_t[(size_t)(y0 + 1) * W + x0 + 1];
@@ -532,6 +532,11 @@ static void orc_sample_terms(int W, const float* dtf_t, const double Kt[4], cons
   gs[3] = -(xs[1] * b[2] - xs[2] * b[1]);
   gs[4] = -(xs[2] * b[0] - xs[0] * b[2]);
   gs[5] = -(xs[0] * b[1] - xs[1] * b[0]);
+  if (jz) {   /* the joint phase's terms, as in orc_pair_loss_grad_joint */
+    jz[0] = drho * (ddx * (x - Kt[2]) + ddy * (y - Kt[3]));
+    jz[1] = -(b[0] * xs[0] + b[1] * xs[1]);
+    jz[2] = (b[0] * xs[0] + b[1] * xs[1] + b[2] * xs[2]) / xs[2];
+  }
   *d_out = d; dd[0] = ddx; dd[1] = ddy;
   double m = fabs(D00);
   if (fabs(D01) > m) m = fabs(D01);
@@ -550,13 +555,17 @@ static double orc_norm6(const double a[6], const double b[6] /* nullable: norm o
  * Q_t, Q_s = sums over the valid samples of the SQUARED 2-norm of the sample's target / source 6-vector: the scale of
  * the pair's gradient before its terms cancel (reading T2: near a minimum |G| -> 0 while the terms do not, and an
  * error "relative to |G|" loses its meaning; a tolerance is then taken relative to max(|g|, root-sum-square)). */
-void orc_pair_event_slack(int W, int H, int n_edges, const uint16_t* uv, const float* z, const double Ks[4],
-                          const double Kt[4], const double Ts[12], const double Tt[12], const float* dtf_t,
-                          double lambda, double delta, double z_min, double out[8], double* check) {
+void orc_pair_event_slack_joint(int W, int H, int n_edges, const uint16_t* uv, const float* z, const double Ks[4],
+                                const double Kt[4], const double Ts[12], const double Tt[12], const float* dtf_t,
+                                double lambda, double delta, double z_min, double out[8], double* check,
+                                double* jout /* nullable [4]: E_Jt, E_Js, Q_Jt, Q_Js (joint phase: the focal sums) */,
+                                double* dz_slack /* nullable [n_edges]: largest change of d rho / d Z_s of each sample */) {
   double Tts[12];
   orc_relative_pose(Ts, Tt, Tts);
   double Et = 0.0, Es = 0.0, Er = 0.0, Qt = 0.0, Qs = 0.0; int k_out = 0, k_in = 0, flagged = 0;
+  double EJt = 0.0, EJs = 0.0, QJt = 0.0, QJs = 0.0;
   if (check) for (int i = 0; i < 14; ++i) check[i] = 0.0;
+  if (dz_slack) for (int e = 0; e < n_edges; ++e) dz_slack[e] = 0.0;
   const double xmax = (double)(W - 1), ymax = (double)(H - 1);
   for (int e = 0; e < n_edges; ++e) {
     double xs[3], xt[3], S3[3];
@@ -579,7 +588,9 @@ void orc_pair_event_slack(int W, int H, int n_edges, const uint16_t* uv, const f
         if (!z_ok) continue;                           /* invalid here, and outside the image for any z' > z_min */
         /* valid-by-depth here: it continues below and is found outside the image */
       } else {
-        flagged++; if (z_ok) k_out++; else k_in++; Et = Es = Er = INFINITY; continue;
+        flagged++; if (z_ok) k_out++; else k_in++; Et = Es = Er = EJt = EJs = INFINITY;
+        if (dz_slack) dz_slack[e] = INFINITY;
+        continue;
       }
     }
     double px[2];
@@ -603,38 +614,82 @@ void orc_pair_event_slack(int W, int H, int n_edges, const uint16_t* uv, const f
     if (ye - y0 < ry && y0 >= 1) { cys[1] = y0 - 1; ncy = 2; }
     else if (y0 + 1 - ye < ry && y0 + 1 <= H - 2) { cys[1] = y0 + 1; ncy = 2; }
     /* nominal terms (only meaningful if valid) */
-    double rho0 = 0.0, gt0[6] = {0, 0, 0, 0, 0, 0}, gs0[6] = {0, 0, 0, 0, 0, 0}, d0, dd0[2], Dm;
-    orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, x0, y0, 1, lambda, delta, &rho0, gt0, gs0, &d0, dd0, &Dm);
+    double rho0 = 0.0, gt0[6] = {0, 0, 0, 0, 0, 0}, gs0[6] = {0, 0, 0, 0, 0, 0}, d0, dd0[2], Dm, jz0[3] = {0, 0, 0};
+    orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, x0, y0, 1, lambda, delta, &rho0, gt0, gs0, &d0, dd0, &Dm, jz0);
     const int inside0 = d0 <= lambda;
-    if (!inside0) orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, x0, y0, 0, lambda, delta, &rho0, gt0, gs0, &d0, dd0, &Dm);
+    if (!inside0) orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, x0, y0, 0, lambda, delta, &rho0, gt0, gs0, &d0, dd0, &Dm, jz0);
     const double rd = fabs(dd0[0]) * rx + fabs(dd0[1]) * ry + 6.0 * ORC_U32 * Dm;
     const int lam_unsure = fabs(d0 - lambda) <= rd;
     if (valid && check) {
       check[0] += rho0; check[1] += 1.0;
       for (int i = 0; i < 6; ++i) { check[2 + i] += gt0[i]; check[8 + i] += gs0[i]; }
     }
-    if (valid) { double a = orc_norm6(gt0, NULL), b = orc_norm6(gs0, NULL); Qt += a * a; Qs += b * b; }
-    if (!valid) { rho0 = 0.0; for (int i = 0; i < 6; ++i) gt0[i] = gs0[i] = 0.0; }
+    if (valid) { double a = orc_norm6(gt0, NULL), b = orc_norm6(gs0, NULL); Qt += a * a; Qs += b * b; QJt += jz0[0] * jz0[0]; QJs += jz0[1] * jz0[1]; }
+    if (!valid) { rho0 = 0.0; for (int i = 0; i < 6; ++i) gt0[i] = gs0[i] = 0.0; jz0[0] = jz0[1] = jz0[2] = 0.0; }
     if (!edge_near && ncx == 1 && ncy == 1 && !lam_unsure) continue;               /* nothing discrete in reach */
     flagged++;
     if (edge_near) { if (valid) k_out++; else k_in++; }
-    double wt = 0.0, ws = 0.0, wr = 0.0;
-    if (valid && edge_near) { wt = orc_norm6(gt0, NULL); ws = orc_norm6(gs0, NULL); wr = rho0; }   /* dropped */
+    double wt = 0.0, ws = 0.0, wr = 0.0, wj[3] = {0, 0, 0};
+    if (valid && edge_near) {   /* dropped */
+      wt = orc_norm6(gt0, NULL); ws = orc_norm6(gs0, NULL); wr = rho0;
+      for (int i = 0; i < 3; ++i) wj[i] = fabs(jz0[i]);
+    }
     for (int ix = 0; ix < ncx; ++ix)
       for (int iy = 0; iy < ncy; ++iy)
         for (int br = 0; br < 2; ++br) {
           const int inside = br == 0 ? inside0 : !inside0;
           if (br == 1 && !lam_unsure) continue;
-          double rho1, gt1[6], gs1[6], d1, dd1[2], Dm1;
-          orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, cxs[ix], cys[iy], inside, lambda, delta, &rho1, gt1, gs1, &d1, dd1, &Dm1);
+          double rho1, gt1[6], gs1[6], d1, dd1[2], Dm1, jz1[3];
+          orc_sample_terms(W, dtf_t, Kt, Tts, xs, xt, xe, ye, cxs[ix], cys[iy], inside, lambda, delta, &rho1, gt1, gs1, &d1, dd1, &Dm1, jz1);
           double a = orc_norm6(gt1, gt0), b = orc_norm6(gs1, gs0), c = fabs(rho1 - rho0);
           if (a > wt) wt = a;
           if (b > ws) ws = b;
           if (c > wr) wr = c;
+          for (int i = 0; i < 3; ++i) if (fabs(jz1[i] - jz0[i]) > wj[i]) wj[i] = fabs(jz1[i] - jz0[i]);
         }
-    Et += wt; Es += ws; Er += wr;
+    Et += wt; Es += ws; Er += wr; EJt += wj[0]; EJs += wj[1];
+    if (dz_slack) dz_slack[e] = wj[2];
   }
+  if (jout) { jout[0] = EJt; jout[1] = EJs; jout[2] = QJt; jout[3] = QJs; }
   out[0] = Et; out[1] = Es; out[2] = Er; out[3] = k_out; out[4] = k_in; out[5] = flagged; out[6] = Qt; out[7] = Qs;
+}
+
+void orc_pair_event_slack(int W, int H, int n_edges, const uint16_t* uv, const float* z, const double Ks[4],
+                          const double Kt[4], const double Ts[12], const double Tt[12], const float* dtf_t,
+                          double lambda, double delta, double z_min, double out[8], double* check) {
+  orc_pair_event_slack_joint(W, H, n_edges, uv, z, Ks, Kt, Ts, Tt, dtf_t, lambda, delta, z_min, out, check, NULL, NULL);
+}
+
+/* The same bound for the joint phase's gradients (orc_joint_grad): logf_slack [N] on d L / d ln f_c, logf_rss [N] its
+ * root-sum-square scale (reading T2), gz_slack [E] on d L / d Z of every edge-list entry.  Serial over pairs. */
+void orc_joint_slack(int N, int W, int H, const float* K, const double* poses, const int32_t* edge_off,
+                     const uint16_t* uv, const float* z, const float* dtf, int64_t P, const int32_t* pairs,
+                     double lambda, double delta, double z_min, double* logf_slack, double* logf_rss, double* gz_slack) {
+  int max_n = 1;
+  for (int i = 0; i < N; ++i) if (edge_off[i + 1] - edge_off[i] > max_n) max_n = edge_off[i + 1] - edge_off[i];
+  double* dzs = (double*)malloc((size_t)max_n * sizeof(double));
+  double* dZ = (double*)malloc((size_t)max_n * sizeof(double));
+  for (int i = 0; i < N; ++i) logf_slack[i] = logf_rss[i] = 0.0;
+  for (int64_t e = 0; e < edge_off[N]; ++e) gz_slack[e] = 0.0;
+  for (int64_t p = 0; p < P; ++p) {
+    const int s = pairs[2 * p], t = pairs[2 * p + 1], n_e = edge_off[s + 1] - edge_off[s];
+    double Ks[4], Kt[4], S, G[12], J[2], o[8], jo[4]; int32_t nv, nr[2];
+    for (int i = 0; i < 4; ++i) { Ks[i] = K[4 * s + i]; Kt[i] = K[4 * t + i]; }
+    orc_pair_loss_grad_joint(W, H, n_e, uv + 2 * (size_t)edge_off[s], z + edge_off[s], Ks, Kt, poses + 12 * (size_t)s,
+                             poses + 12 * (size_t)t, dtf + (size_t)t * W * H, lambda, delta, z_min, 0, &S, &nv, G, nr, J, dZ);
+    orc_pair_event_slack_joint(W, H, n_e, uv + 2 * (size_t)edge_off[s], z + edge_off[s], Ks, Kt, poses + 12 * (size_t)s,
+                               poses + 12 * (size_t)t, dtf + (size_t)t * W * H, lambda, delta, z_min, o, NULL, jo, dzs);
+    const double n = (double)nv, k_out = o[3], k_in = o[4], kmax = k_out > k_in ? k_out : k_in;
+    const double n_lo = n - k_out >= 1.0 ? n - k_out : 1.0;
+    logf_slack[t] += jo[0] / n_lo + (n > 0.0 ? fabs(J[0]) * kmax / (n * n_lo) : 0.0);
+    logf_slack[s] += jo[1] / n_lo + (n > 0.0 ? fabs(J[1]) * kmax / (n * n_lo) : 0.0);
+    if (n > 0.0) { logf_rss[t] += jo[2] / (n * n); logf_rss[s] += jo[3] / (n * n); }
+    for (int e = 0; e < n_e; ++e)
+      gz_slack[edge_off[s] + e] += dzs[e] / n_lo + (n > 0.0 ? fabs(dZ[e]) * kmax / (n * n_lo) : 0.0);
+  }
+  for (int i = 0; i < N; ++i) { logf_slack[i] /= (double)P; logf_rss[i] = sqrt(logf_rss[i]) / (double)P; }
+  for (int64_t e = 0; e < edge_off[N]; ++e) gz_slack[e] /= (double)P;
+  free(dzs); free(dZ);
 }
 
 /* Whole list: per-camera gradient slack [N], per-pair loss slack [P], per-pair (k_out, k_in, flagged) [P][3].
@@ -653,8 +708,9 @@ void orc_event_slack(int N, int W, int H, const float* K, const double* poses, c
     int s = pairs[2 * p], t = pairs[2 * p + 1];
     double Ks[4], Kt[4], o[8];
     for (int i = 0; i < 4; ++i) { Ks[i] = K[4 * s + i]; Kt[i] = K[4 * t + i]; }
-    orc_pair_event_slack(W, H, edge_off[s + 1] - edge_off[s], uv + 2 * (size_t)edge_off[s], z + edge_off[s], Ks, Kt,
-                         poses + 12 * (size_t)s, poses + 12 * (size_t)t, dtf + (size_t)t * W * H, lambda, delta, z_min, o, NULL);
+    orc_pair_event_slack_joint(W, H, edge_off[s + 1] - edge_off[s], uv + 2 * (size_t)edge_off[s], z + edge_off[s], Ks, Kt,
+                               poses + 12 * (size_t)s, poses + 12 * (size_t)t, dtf + (size_t)t * W * H, lambda, delta, z_min, o, NULL,
+                               NULL, NULL);
     const double n = (double)pair_valid[p], k_out = o[3], k_in = o[4], kmax = k_out > k_in ? k_out : k_in;
     const double n_lo = n - k_out >= 1.0 ? n - k_out : 1.0;
     const double Gt = orc_norm6(pair_G + 12 * p, NULL), Gs = orc_norm6(pair_G + 12 * p + 6, NULL);

@@ -59,17 +59,18 @@ cudaError_t copy_out(void* dst, const void* src, size_t bytes, cudaStream_t st, 
 }
 
 void free_views(epo_ctx* c) {
-  epo_dfree(c, c->d_edge_off); epo_dfree(c, c->d_edges); epo_dfree(c, c->d_pts); epo_dfree(c, c->d_depth);
+  epo_dfree(c, c->d_edge_off); epo_dfree(c, c->d_edges); epo_dfree(c, c->d_depth);
   c->d_depth = nullptr;
   epo_free_atlas(&c->atlas);
   epo_free_packed(c, &c->packed);
   epo_joint_free(c);
-  c->d_edge_off = nullptr; c->d_edges = nullptr; c->d_pts = nullptr;
+  c->d_edge_off = nullptr; c->d_edges = nullptr;
   c->have_views = false;
 }
 void free_pairs(epo_ctx* c) {
   epo_dfree(c, c->d_pairs); epo_dfree(c, c->d_perm); epo_dfree(c, c->d_tgt_off); epo_dfree(c, c->d_src_off); epo_dfree(c, c->d_src_inc);
   epo_dfree(c, c->d_work); epo_dfree(c, c->d_work_off); epo_dfree(c, c->d_part); epo_dfree(c, c->d_pair_loss); epo_dfree(c, c->d_pair_valid); epo_dfree(c, c->d_out_f);
+  epo_dfree(c, c->d_dz); c->d_dz = nullptr;
   epo_dfree(c, c->d_out_i); epo_dfree(c, c->d_sel_flag); epo_dfree(c, c->d_sel_work); epo_dfree(c, c->d_sel_info); epo_dfree(c, c->d_sel_scratch);
   c->d_sel_scratch = nullptr; c->d_sel_flag = nullptr; c->d_sel_work = nullptr; c->d_sel_info = nullptr; c->subsample = false; c->sel_grid = 0;
   c->d_pairs = nullptr; c->d_perm = nullptr; c->d_tgt_off = nullptr; c->d_src_off = nullptr; c->d_src_inc = nullptr;
@@ -139,7 +140,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   if (!(cfg->huber_delta > 0.f) || cfg->clamp_steps < 1 || cfg->warmup_steps < 0 || cfg->max_steps <= cfg->warmup_steps ||
       cfg->w1 < 1 || cfg->w2 < 1 || (cfg->dtf_format != 0 && cfg->dtf_format != 1) || cfg->e_max < 0 ||
       cfg->pair_budget < 0 || (cfg->joint_phase != 0 && cfg->joint_phase != 1) || !(cfg->weight_decay >= 0.f) ||
-      (cfg->joint_phase && cfg->pair_budget > 0) || (cfg->stop_rule != 0 && cfg->stop_rule != 1) || cfg->w_loss < 1 || !(cfg->eps_loss >= 0.f) || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
+      (cfg->stop_rule != 0 && cfg->stop_rule != 1) || cfg->w_loss < 1 || !(cfg->eps_loss >= 0.f) || !(cfg->beta1 >= 0.f && cfg->beta1 < 1.f) || !(cfg->beta2 >= 0.f && cfg->beta2 < 1.f) || !(cfg->z_min >= 0.f))
     return EPO_ERR_INVALID_ARG;
   epo_ctx* c = new (std::nothrow) epo_ctx();
   if (!c) return EPO_ERR_OUT_OF_MEMORY;
@@ -149,7 +150,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   c->err[0] = 0;
   c->pool = nullptr; c->own_pool = false;
   c->atlas = EpoAtlas{nullptr, nullptr, 0, 0, 1};
-  c->packed.xyz = nullptr; c->packed.d_off = nullptr;
+  c->packed.xyz = nullptr; c->packed.pix = nullptr; c->packed.d_off = nullptr;
   { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
   c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
@@ -240,7 +241,8 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   PhaseTrace tr(st, "epo_set_views");
   float* d_depth = nullptr; uint8_t* d_e = nullptr; float* d_small = nullptr;
   int32_t* off = nullptr; EdgeRec* rec = nullptr; int64_t E = 0;
-  float4* pts = nullptr; EpoAtlas atlas = {nullptr, nullptr, 0, 0, 1};
+  EpoAtlas atlas = {nullptr, nullptr, 0, 0, 1};
+  EpoPacked packed = {nullptr, nullptr, nullptr, {}};
   EpoDtfScratch scratch = {nullptr, 0, 0};
   std::vector<int32_t> hoff;
   bool subsampled = false;
@@ -272,10 +274,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
   tr.mark("copy depth");
   if (rc == EPO_OK) rc = epo_build_edge_lists(c, d_e, d_depth, &off, &rec, &E, &hoff, &subsampled);
   tr.mark("edge lists");
-  if (rc == EPO_OK) rc = epo_build_points(c, d_small, off, rec, E, hoff, d_e, d_depth, subsampled, &pts);
-  EpoPacked packed = {nullptr, nullptr, {}};
-  if (rc == EPO_OK) rc = epo_alloc_packed(c, hoff, &packed);
-  if (rc == EPO_OK) rc = epo_launch_pack_points(c, pts, off, packed);
+  if (rc == EPO_OK) rc = epo_build_points(c, d_small, off, rec, E, hoff, d_e, d_depth, subsampled, &packed);
   if (rc == EPO_OK) {
     // commit the small state on the stream, then drain it once
     e = cudaMemcpyAsync(c->d_K, d_small, N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, st);
@@ -298,12 +297,12 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
     // d_K / d_poses may have been overwritten only if every build step succeeded and the final drain failed
     // (a sticky CUDA error: the context is unusable anyway)
     cudaGetLastError();
-    epo_dfree(c, off); epo_dfree(c, rec); epo_dfree(c, pts); epo_free_atlas(&atlas); epo_free_packed(c, &packed);
+    epo_dfree(c, off); epo_dfree(c, rec); epo_free_atlas(&atlas); epo_free_packed(c, &packed);
     return rc;
   }
   free_pairs(c); free_views(c);
   c->d_edge_off = off; c->d_edges = rec; c->E = E; c->h_edge_off = hoff;
-  c->d_pts = pts; c->atlas = atlas; c->d_depth = d_depth; c->packed = packed;
+  c->atlas = atlas; c->d_depth = d_depth; c->packed = packed;
   c->have_views = true; c->static_dirty = true;
   EPO_TRY(epo_joint_alloc(c));                      // joint loop: variables at the identity, Z0 and K0 kept
   tr.mark("free temporaries");
@@ -335,7 +334,7 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   epo_status rc = (e == cudaSuccess) ? epo_build_pairs(c, d_user, P, &canon, &perm, &toff, &soff, &sinc, &work, &woff, &n_work, chunk)
                                      : epo_fail(c, EPO_ERR_CUDA, "epo_set_pairs: %s", cudaGetErrorString(e));
   epo_dfree(c, d_user);
-  double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr;
+  double* acc = nullptr; float* pl = nullptr; int32_t* pv = nullptr; float* of = nullptr; int32_t* oi = nullptr; float2* dz = nullptr;
   uint8_t* sflag = nullptr; int32_t* swork = nullptr; int32_t* sinfo = nullptr; int32_t* sscr = nullptr;
   if (rc == EPO_OK && c->cfg.pair_budget > 0 && P > c->cfg.pair_budget) {
     // k_select_pairs meets at grid barriers: all its CTAs (4096 pairs each) must be resident at once, one per SM
@@ -361,7 +360,9 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   if (rc == EPO_OK) {
     // output staging: [loss | grad 6N | pair_loss P | loss trace | theta trace]
     size_t nf = 1 + (size_t)c->N * 6 + (size_t)P + (size_t)c->cfg.max_steps * 2;
-    e = epo_dmalloc(c, &acc, (size_t)(n_work > 0 ? n_work : 1) * kAccStride * sizeof(double));
+    // partial records at the joint phase's stride (epo_loss_grad_joint works in every context)
+    e = epo_dmalloc(c, &acc, (size_t)(n_work > 0 ? n_work : 1) * kAccStrideJoint * sizeof(double));
+    if (e == cudaSuccess && c->cfg.joint_phase) e = epo_dmalloc(c, &dz, (size_t)(n_work > 0 ? n_work : 1) * (size_t)(chunk / 2) * sizeof(float2));
     if (e == cudaSuccess) e = epo_dmalloc(c, &pl, (size_t)P * sizeof(float));
     if (e == cudaSuccess) e = epo_dmalloc(c, &pv, (size_t)P * sizeof(int32_t));
     if (e == cudaSuccess) e = epo_dmalloc(c, &of, nf * sizeof(float));
@@ -373,7 +374,7 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   if (rc != EPO_OK) {
     cudaGetLastError();
     epo_dfree(c, canon); epo_dfree(c, work); epo_dfree(c, perm); epo_dfree(c, toff); epo_dfree(c, soff); epo_dfree(c, sinc); epo_dfree(c, woff);
-    epo_dfree(c, acc); epo_dfree(c, pl); epo_dfree(c, pv); epo_dfree(c, of); epo_dfree(c, oi);
+    epo_dfree(c, acc); epo_dfree(c, pl); epo_dfree(c, pv); epo_dfree(c, of); epo_dfree(c, oi); epo_dfree(c, dz);
     epo_dfree(c, sflag); epo_dfree(c, swork); epo_dfree(c, sinfo); epo_dfree(c, sscr);
     return rc;
   }
@@ -381,7 +382,7 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   c->d_pairs = canon; c->d_perm = perm; c->d_tgt_off = toff; c->d_src_off = soff; c->d_src_inc = sinc; c->d_work = work;
   c->d_work_off = woff; c->n_work = n_work; c->P = P; c->d_part = acc; c->d_pair_loss = pl; c->d_pair_valid = pv; c->d_out_f = of; c->d_out_i = oi;
   c->h_pairs.swap(hp); c->reproj_per_eval = reproj; c->lg_chunk = chunk;
-  c->d_sel_flag = sflag; c->d_sel_work = swork; c->d_sel_info = sinfo; c->d_sel_scratch = sscr;
+  c->d_sel_flag = sflag; c->d_sel_work = swork; c->d_sel_info = sinfo; c->d_sel_scratch = sscr; c->d_dz = dz;
   // stochastic pair sub-sampling: only when the list is longer than the budget (Alg. 3 l.3-6)
   c->subsample = c->cfg.pair_budget > 0 && P > c->cfg.pair_budget;
   {
@@ -409,8 +410,8 @@ epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss
   if (!loss || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_loss_grad: NULL loss or negative lambda");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
-  EPO_TRY(epo_launch_fused(c, lambda, false, false));
-  EPO_TRY(epo_launch_finish(c, false, false, false, false));
+  EPO_TRY(epo_launch_fused(c, lambda, false, false, false));
+  EPO_TRY(epo_launch_finish(c, false, false, false, false, false));
   bool sync = false;
   // loss: DevState.loss (double) -> float
   epo_launch_f64_to_f32(st, &c->d_state->loss, c->d_out_f, 1);
@@ -443,27 +444,30 @@ epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_l
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
   const size_t N = (size_t)c->N, px = N * c->W * c->H;
-  // the evaluation first: per-pair valid counts (and the loss), then the joint pass over the same samples
-  EPO_TRY(epo_launch_fused(c, lambda, false, false));
-  EPO_TRY(epo_launch_finish(c, false, false, false, false));
-  double* d_gf = nullptr; float* d_gf32 = nullptr; float* d_gz = nullptr; float* d_gpt = nullptr;
+  // one pass of the fused kernel in joint mode (loss, pose gradient, the focal sums and a . t_ts of every sample), the
+  // per-camera reduction (valid counts, d L / d ln f), then every edge pixel's pairs summed into the dense map
+  float2* dz = c->d_dz; float2* dz_tmp = nullptr; float* d_gf32 = nullptr; float* d_gz = nullptr;
   const bool gz_dev = is_device_ptr(g_depth);
-  const size_t E = (size_t)(c->E > 0 ? c->E : 1);
-  cudaError_t e = epo_dmalloc(c, &d_gf, N * sizeof(double));
-  if (e == cudaSuccess) e = epo_dmalloc(c, &d_gf32, N * sizeof(float));
-  if (e == cudaSuccess) e = epo_dmalloc(c, &d_gpt, E * sizeof(float));
+  cudaError_t e = epo_dmalloc(c, &d_gf32, N * sizeof(float));
+  if (e == cudaSuccess && !dz) {
+    e = epo_dmalloc(c, &dz_tmp, (size_t)(c->n_work > 0 ? c->n_work : 1) * (size_t)(c->lg_chunk / 2) * sizeof(float2));
+    dz = dz_tmp;
+  }
   if (e == cudaSuccess && !gz_dev) e = epo_dmalloc(c, &d_gz, px * sizeof(float));
-  float* gz = gz_dev ? g_depth : d_gz;
-  if (e == cudaSuccess) e = cudaMemsetAsync(d_gf, 0, N * sizeof(double), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(d_gpt, 0, E * sizeof(float), st);
-  if (e == cudaSuccess) e = cudaMemsetAsync(gz, 0, px * sizeof(float), st);
-  epo_status rc = e == cudaSuccess ? epo_launch_fused_joint(c, lambda, d_gf, d_gpt, false)
-                                   : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
-                                              "epo_loss_grad_joint: %s", cudaGetErrorString(e));
-  if (rc == EPO_OK) rc = epo_joint_scatter_gz(c, d_gpt, gz);     // point order -> the dense map
+  epo_status rc = e == cudaSuccess ? EPO_OK : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
+                                                        "epo_loss_grad_joint: %s", cudaGetErrorString(e));
+  if (rc == EPO_OK) {
+    float2* keep = c->d_dz;
+    c->d_dz = dz;
+    rc = epo_launch_fused(c, lambda, false, false, true);
+    c->d_dz = keep;
+    c->static_dirty = true;                          // (the launch above was not the loop's: keep the next one serialised)
+  }
+  if (rc == EPO_OK) rc = epo_launch_finish(c, false, false, false, false, true);
+  if (rc == EPO_OK) rc = epo_joint_gather_gz(c, dz, gz_dev ? g_depth : d_gz);
   bool sync = false;
   if (rc == EPO_OK) {
-    epo_launch_f64_to_f32(st, d_gf, d_gf32, (int64_t)N);
+    epo_launch_f64_to_f32(st, c->d_glogf, d_gf32, (int64_t)N);
     c->launches += 1;
     e = copy_out(g_logf, d_gf32, N * sizeof(float), st, &sync);
     if (e == cudaSuccess && !gz_dev) e = copy_out(g_depth, d_gz, px * sizeof(float), st, &sync);
@@ -475,7 +479,7 @@ epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_l
     if (e == cudaSuccess && sync) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) rc = epo_fail(c, EPO_ERR_CUDA, "epo_loss_grad_joint: %s", cudaGetErrorString(e));
   }
-  epo_dfree(c, d_gf); epo_dfree(c, d_gf32); epo_dfree(c, d_gz); epo_dfree(c, d_gpt);
+  epo_dfree(c, d_gf32); epo_dfree(c, d_gz); epo_dfree(c, dz_tmp);
   return rc;
 }
 
@@ -511,19 +515,14 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
   if (n_iters == 0) EPO_TRY(epo_launch_begin_step_call(c));
+  const bool joint = c->cfg.joint_phase != 0;
   for (int i = 0; i < n_iters; ++i) {
     if (c->subsample) EPO_TRY(epo_launch_select_pairs(c, -1, true, true));
-    EPO_TRY(epo_launch_fused(c, -1.0f, true, c->subsample));
-    EPO_TRY(epo_launch_finish(c, true, true, i == 0, c->subsample));
-    if (c->cfg.joint_phase) {
-      // the joint gradients at the state this iteration's loss was evaluated at, then AdamW on gamma / alpha / beta
-      // and the new intrinsics and points (all three self-gated by DevState.joint_pending)
-      EPO_CUDA(c, cudaMemsetAsync(c->d_glogf, 0, (size_t)c->N * sizeof(double), st));
-      EPO_CUDA(c, cudaMemsetAsync(c->d_gz, 0, (size_t)(c->E > 0 ? c->E : 1) * sizeof(float), st));
-      EPO_TRY(epo_launch_fused_joint(c, -1.0f, c->d_glogf, c->d_gz, true));
-      EPO_TRY(epo_launch_joint_update(c));
-      c->static_dirty = true;                       // the points were rewritten: the next fused launch is serialised
-    }
+    EPO_TRY(epo_launch_fused(c, -1.0f, true, c->subsample, joint));
+    EPO_TRY(epo_launch_finish(c, true, true, i == 0, c->subsample, joint));
+    // joint phase: AdamW on (alpha, beta) where due and the points again from the new K and Z (gamma was stepped in
+    // k_finish); self-gated by DevState.joint_pending
+    if (joint) EPO_TRY(epo_launch_joint_points(c, c->subsample));
   }
   bool sync = false;
   if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));

@@ -19,6 +19,9 @@ struct __align__(8) EdgeRec {
 // Partial sums written by each CTA of the fused kernel (row a-8): S = sum rho, n = valid count,
 // A = sum a, M = sum x_t x a (six-accumulator identity I1).  fp64, 64 bytes per work item.
 constexpr int kAccStride = 8;
+// Joint phase: the record also carries the pair's focal-length sums (slot 8: sum d rho / d ln f_t, slot 9: sum
+// d rho / d ln f_s); 16 slots so that k_finish reads it with two chunk classes per warp round.
+constexpr int kAccStrideJoint = 16;
 
 // Edge pixels handled by one CTA of the fused kernel: kLgOuter passes of kLgThreads threads x kLgPerThread
 // (unrolled) samples.  The point list is padded by kLgChunk entries so that tail lanes may read past a list.
@@ -85,6 +88,7 @@ constexpr float kU8LambdaMax = 14.5f;
 // last view (the first-pass loads of a short last work item read past its list).
 struct EpoPacked {
   float2* xyz;
+  int2* pix;                    // [slots] pixel index v W + u of both samples of a slot (-1: padding)
   int32_t* d_off;               // [N+1] device copy of h_off
   std::vector<int32_t> h_off;   // [N+1] in samples, multiples of kLgPass
 };
@@ -108,19 +112,21 @@ struct epo_ctx {
   double* d_poses;        // [N][12] current (fp64: T_ts is formed without fp32 cancellation)
   double* d_poses_next;   // [N][12] poses after the update in flight (published by the last CTA of k_finish)
   double* d_poses_init;   // [N][12] as given to epo_set_views / epo_reset
-  // joint loop (cfg.joint_phase): focal scale gamma per camera, depth affine (alpha, beta) per point
-  double* d_poses_prev;   // [N][12] poses at the start of the iteration just completed (the joint pass evaluates there)
+  // joint loop (cfg.joint_phase): focal scale gamma per camera, depth affine (alpha, beta) per edge pixel;
+  // everything per edge pixel lives in the packed slot order (EpoPacked), two samples per slot
   float* d_K0;            // [N][4] intrinsics as given
-  double* d_gamma;        // [3][N] gamma, Adam m, v
-  double* d_ab;           // [3][E][2] (alpha, beta), Adam m, v, point order
-  float* d_z0;            // [E] depth as given, point order
-  float* d_gz;            // [E] d L / d Z of the joint pass, point order
-  double* d_glogf;        // [N] d L / d ln f
+  double* d_gamma;        // [3][N] gamma, AdamW m, v
+  float2* d_z0;           // [slots] depth as given
+  double4* d_ab;          // [slots] (alpha_a, beta_a, alpha_b, beta_b)
+  float4* d_abm;          // [slots][2] AdamW moments (m_alpha, v_alpha, m_beta, v_beta) of sample a, then b
+  float2* d_dz;           // [n_work][chunk / 2] a . t_ts of both samples of every slot of every work item (the fused
+                          // kernel's joint output of the iteration in flight; allocated with the pair list)
+  double* d_glogf;        // [N] d L / d ln f (k_finish)
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
   float* d_depth;         // [N][H][W] the depth maps as given (kept for epo_build_viewgraph)
-  float4* d_pts;          // [E] camera-frame points (x_s, y_s, z_s, pixel index): K and Z are fixed, so row a-2 is hoisted
-  EpoPacked packed;       // the same points in the fused kernel's layout (rebuilt whenever d_pts changes)
+  EpoPacked packed;       // [E] camera-frame points (x_s, y_s, z_s) in the fused kernel's layout: K and Z are fixed outside
+                          // the joint phase, so row a-2 is hoisted; + the pixel index of every point
   EpoAtlas atlas;         // the distance fields as the fused kernel samples them (see EpoAtlas)
   std::vector<int32_t> h_edge_off;
 
@@ -219,11 +225,9 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, EpoAtlas
 void epo_free_dtf_scratch(epo_ctx* ctx, EpoDtfScratch* s);
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
                             const std::vector<int32_t>& h_off, const uint8_t* d_edges_u8, const float* d_depth,
-                            bool subsampled, float4** out_pts);
+                            bool subsampled, EpoPacked* out);   // tile-major points, packed (EpoPacked) + pixel indices
 void epo_free_atlas(EpoAtlas* atlas);
-epo_status epo_alloc_packed(epo_ctx* ctx, const std::vector<int32_t>& h_edge_off, EpoPacked* out);
 void epo_free_packed(epo_ctx* ctx, EpoPacked* pk);
-epo_status epo_launch_pack_points(epo_ctx* ctx, const float4* d_pts, const int32_t* d_edge_off, const EpoPacked& pk);
 // pairs.cu
 epo_status epo_build_pairs(epo_ctx* ctx, const int32_t* d_user_pairs, int64_t P, int2** out_pairs,
                            int32_t** out_perm, int32_t** out_tgt_off, int32_t** out_src_off,
@@ -239,25 +243,27 @@ int64_t epo_select_max_pairs(void);
 epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override /* < 0: device step */, bool gated, bool build_work);
 // canny.cu: edge maps (1 / 0) of [N][H][W] 8-bit images, device pointers
 epo_status epo_run_canny(epo_ctx* ctx, const uint8_t* d_img, int low, int high, uint8_t* d_edges);
-// joint.cu: the joint loop's variable update (AdamW on gamma, alpha, beta; new K and points) and its state
+// joint.cu: the joint loop's depth-variable update (AdamW on alpha, beta; new points) and its state
 epo_status epo_joint_alloc(epo_ctx* ctx);              // after the points exist (epo_set_views)
 void epo_joint_free(epo_ctx* ctx);
 epo_status epo_joint_reset(epo_ctx* ctx);              // identity variables, zero moments, K and points as given
 epo_status epo_joint_reset_moments(epo_ctx* ctx);      // zero AdamW moments only (epo_set_pairs: the variables stay)
-epo_status epo_launch_joint_update(epo_ctx* ctx);      // gated by DevState.joint_pending
-epo_status epo_joint_scatter_gz(epo_ctx* ctx, const float* d_g_points, float* d_map);   // point order -> [N][H][W]
+epo_status epo_launch_joint_points(epo_ctx* ctx, bool subset);   // gated by DevState.joint_pending
+// d L / d Z of every listed edge pixel from the joint pass's per-slot output (d_dz) and the per-pair valid counts:
+// written into the dense [N][H][W] map (zeroed here first)
+epo_status epo_joint_gather_gz(epo_ctx* ctx, const float2* d_dz, float* d_map);
 epo_status epo_joint_export(epo_ctx* ctx, double* d_gamma_out, double* d_alpha_map, double* d_beta_map);
 // viewgraph.cu: cycle counts of all ordered pairs + ordered emission of the valid pairs
 epo_status epo_launch_viewgraph(epo_ctx* ctx, int stride, float tau, float min_frac, int2* d_counts, int2* d_pairs,
                                 long long* d_n);
 // lossgrad.cu
-epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset);
-epo_status epo_launch_fused_joint(epo_ctx* ctx, float lambda, double* d_g_logf, float* d_g_depth, bool in_loop);   // joint-phase pass
+epo_status epo_launch_fused(epo_ctx* ctx, float lambda_override /* < 0: device schedule */, bool gated, bool subset,
+                            bool joint /* also the joint-phase derivatives: d_dz, 16-slot partial records */);
 epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused kernel alone (measurement hook)
 epo_status epo_launch_record_taps(epo_ctx* ctx, float lambda, uint2* d_taps);                  // gather ceiling: the tap stream
 epo_status epo_launch_gather_taps(epo_ctx* ctx, float lambda, const uint2* d_taps, unsigned* d_out);   // ... replayed alone
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
-epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset);
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset, bool joint);
 epo_status epo_launch_fill_schedule(epo_ctx* ctx);     // d_sched from the configuration (once, in epo_create)
 epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done (an epo_step call of zero iterations)
 void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n);

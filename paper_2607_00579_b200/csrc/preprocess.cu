@@ -296,31 +296,33 @@ __global__ void k_tile_points(const uint8_t* __restrict__ edges, const float* __
 }
 
 
-// tile-major float4 points -> the packed layout (EpoPacked): thread = one slot (two samples) of one view
+// tile-major float4 points (.w = pixel index) -> the packed layout (EpoPacked): thread = one slot (two samples) of a view
 __global__ void k_pack_points(const float4* __restrict__ pts, const int32_t* __restrict__ edge_off,
-                              const int32_t* __restrict__ pk_off, float2* __restrict__ xyz) {
+                              const int32_t* __restrict__ pk_off, float2* __restrict__ xyz, int2* __restrict__ pix) {
   const int view = blockIdx.y;
   const int lo = edge_off[view], n = edge_off[view + 1] - lo;
   const int slots = (pk_off[view + 1] - pk_off[view]) / 2;
   const size_t base = (size_t)pk_off[view] / 2;
   for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < slots; j += gridDim.x * blockDim.x) {
     const int a = 64 * (j >> 5) + (j & 31), b = a + 32;
-    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-    const float4 pa = a < n ? pts[(size_t)lo + a] : zero, pb = b < n ? pts[(size_t)lo + b] : zero;
+    const float4 none = make_float4(0.f, 0.f, 0.f, __int_as_float(-1));
+    const float4 pa = a < n ? pts[(size_t)lo + a] : none, pb = b < n ? pts[(size_t)lo + b] : none;
     const size_t s = base + j, o = s / kLgThreads * (3 * kLgThreads) + s % kLgThreads;
     xyz[o] = make_float2(pa.x, pb.x); xyz[o + kLgThreads] = make_float2(pa.y, pb.y); xyz[o + 2 * kLgThreads] = make_float2(pa.z, pb.z);
+    pix[s] = make_int2(__float_as_int(pa.w), __float_as_int(pb.w));
   }
 }
 
 }  // namespace
 
-epo_status epo_alloc_packed(epo_ctx* ctx, const std::vector<int32_t>& h_edge_off, EpoPacked* out) {
-  EpoPacked pk = {nullptr, nullptr, {}};
+static epo_status alloc_packed(epo_ctx* ctx, const std::vector<int32_t>& h_edge_off, EpoPacked* out) {
+  EpoPacked pk = {nullptr, nullptr, nullptr, {}};
   const int N = ctx->N;
   pk.h_off.assign((size_t)N + 1, 0);
   for (int i = 0; i < N; ++i) pk.h_off[i + 1] = pk.h_off[i] + (h_edge_off[i + 1] - h_edge_off[i] + kLgPass - 1) / kLgPass * kLgPass;
-  const size_t used = (size_t)pk.h_off[N] / 2 * 3, all = used + (size_t)kLgPad / 2 * 3;     // float2 entries
+  const size_t slots = (size_t)pk.h_off[N] / 2, used = slots * 3, all = used + (size_t)kLgPad / 2 * 3;     // float2 entries
   cudaError_t e = epo_dmalloc(ctx, &pk.xyz, all * sizeof(float2));
+  if (e == cudaSuccess) e = epo_dmalloc(ctx, &pk.pix, (slots ? slots : 1) * sizeof(int2));
   if (e == cudaSuccess) e = epo_dmalloc(ctx, &pk.d_off, ((size_t)N + 1) * sizeof(int32_t));
   if (e == cudaSuccess) e = cudaMemsetAsync(pk.xyz + used, 0, (all - used) * sizeof(float2), ctx->stream);
   if (e == cudaSuccess)
@@ -335,18 +337,8 @@ epo_status epo_alloc_packed(epo_ctx* ctx, const std::vector<int32_t>& h_edge_off
 }
 
 void epo_free_packed(epo_ctx* ctx, EpoPacked* pk) {
-  epo_dfree(ctx, pk->xyz); epo_dfree(ctx, pk->d_off);
-  pk->xyz = nullptr; pk->d_off = nullptr; pk->h_off.clear();
-}
-
-epo_status epo_launch_pack_points(epo_ctx* ctx, const float4* d_pts, const int32_t* d_edge_off, const EpoPacked& pk) {
-  int max_slots = 1;
-  for (int i = 0; i < ctx->N; ++i) max_slots = std::max(max_slots, (pk.h_off[i + 1] - pk.h_off[i]) / 2);
-  dim3 grid((unsigned)std::min((max_slots + 255) / 256, 64), (unsigned)ctx->N);
-  k_pack_points<<<grid, 256, 0, ctx->stream>>>(d_pts, d_edge_off, pk.d_off, pk.xyz);
-  ctx->launches += 1;
-  EPO_CUDA(ctx, cudaGetLastError());
-  return EPO_OK;
+  epo_dfree(ctx, pk->xyz); epo_dfree(ctx, pk->pix); epo_dfree(ctx, pk->d_off);
+  pk->xyz = nullptr; pk->pix = nullptr; pk->d_off = nullptr; pk->h_off.clear();
 }
 
 epo_status epo_build_edge_lists(epo_ctx* ctx, const uint8_t* d_edges_u8, const float* d_depth,
@@ -501,12 +493,10 @@ epo_status epo_build_dtf_atlas(epo_ctx* ctx, const uint8_t* d_edges_u8, EpoAtlas
 
 epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off, const EdgeRec* d_rec, int64_t E,
                             const std::vector<int32_t>& h_off, const uint8_t* d_edges_u8, const float* d_depth,
-                            bool subsampled, float4** out_pts) {
-  float4* pts = nullptr;
+                            bool subsampled, EpoPacked* out) {
+  float4* pts = nullptr;                             // tile-major (x_s, y_s, z_s, pixel index), packed at the end
   cudaStream_t st = ctx->stream;
-  // padded by one chunk of zeros: the fused kernel's tail lanes read past the end of a list and discard
-  EPO_CUDA(ctx, epo_dmalloc(ctx, &pts, (size_t)(E + kLgPad) * sizeof(float4)));
-  EPO_CUDA(ctx, cudaMemsetAsync(pts + E, 0, (size_t)kLgPad * sizeof(float4), st));
+  EPO_CUDA(ctx, epo_dmalloc(ctx, &pts, (size_t)(E > 0 ? E : 1) * sizeof(float4)));
   cudaError_t e = cudaSuccess;
   if (subsampled) {
     // an E_max sub-sample is defined on the raster list (reading S6): keep its order
@@ -537,6 +527,17 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
     epo_dfree(ctx, tile_cnt); epo_dfree(ctx, tile_off);
   }
   if (e != cudaSuccess) { epo_dfree(ctx, pts); return epo_fail(ctx, EPO_ERR_CUDA, "point list: %s", cudaGetErrorString(e)); }
-  *out_pts = pts;
-  return EPO_OK;
+  EpoPacked pk = {nullptr, nullptr, nullptr, {}};
+  epo_status rc = alloc_packed(ctx, h_off, &pk);
+  if (rc == EPO_OK) {
+    int max_slots = 1;
+    for (int i = 0; i < ctx->N; ++i) max_slots = std::max(max_slots, (pk.h_off[i + 1] - pk.h_off[i]) / 2);
+    dim3 grid((unsigned)std::min((max_slots + 255) / 256, 64), (unsigned)ctx->N);
+    k_pack_points<<<grid, 256, 0, st>>>(pts, d_off, pk.d_off, pk.xyz, pk.pix);
+    ctx->launches += 1;
+    if (cudaGetLastError() != cudaSuccess) { epo_free_packed(ctx, &pk); rc = epo_fail(ctx, EPO_ERR_CUDA, "packed points: launch failed"); }
+  }
+  epo_dfree(ctx, pts);                               // stream-ordered: after the packing kernel
+  if (rc == EPO_OK) *out = pk;
+  return rc;
 }

@@ -26,7 +26,12 @@ struct FinParams {
   int32_t* pair_valid;
   double *grad, *loss_part;
   // optimiser state
-  double *poses, *poses_next, *poses_prev /* nullable */;
+  double *poses, *poses_next;
+  // joint phase (kJoint): per-camera focal scale gamma (AdamW, Eq. 4, 121) and the intrinsics it rescales
+  double *gamma /* [3][N] gamma, m, v */, *glogf /* [N] d L / d ln f */;
+  const float* K0;
+  float* K;
+  double wd;
   double *m, *v, *dR, *dt, *theta, *loss_trace;
   DevState* state;
   int N;
@@ -145,10 +150,14 @@ __device__ bool converged_loss(const double* trace, double loss_s, int s, int w,
   return __syncthreads_and(ok) != 0;
 }
 
+template <bool kJoint>
 __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
+  // partial records: 8 values x 4 chunk classes per warp round, or (joint phase) 16 slots x 2 classes
+  constexpr int kVal = kJoint ? kAccStrideJoint : kAccStride, kCls = 32 / kVal;
   DevState* st = p.state;
   extern __shared__ double sdyn[];                 // last CTA: dR[N], dt[N]
   __shared__ double sg[kFinThreads / 32][8];
+  __shared__ double sj[kFinThreads / 32];
   __shared__ double sel[4];
   __shared__ int s_last;
   const int c = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, N = p.N;
@@ -194,10 +203,14 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
       // per-pair sums: lane l adds value (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... (independent loads), then
       // the four chunk classes are combined by two xor-shuffles: a fixed order
       double v = 0.0;
-      for (int w = wa + (lane >> 3); w < wb; w += 4) v += __ldcg(p.part + (size_t)w * kAccStride + (lane & 7));
-      v += __shfl_xor_sync(0xffffffffu, v, 8);
+      for (int w = wa + lane / kVal; w < wb; w += kCls) v += __ldcg(p.part + (size_t)w * kVal + (lane % kVal));
+      if (!kJoint) v += __shfl_xor_sync(0xffffffffu, v, 8);
       v += __shfl_xor_sync(0xffffffffu, v, 16);
       const double n = __shfl_sync(0xffffffffu, v, 1);
+      // joint phase: lane 8 accumulates d L / d ln f of this camera -- the pair's target sum (slot 8) when the camera
+      // is the pair's target, its source sum (slot 9) when it is the source
+      const double js = kJoint ? __shfl_sync(0xffffffffu, v, 9) : 0.0;
+      if (kJoint && lane == 8 && n > 0.0) acc += (tgt ? v : js) / n;
       if (tgt) {
         const double S = __shfl_sync(0xffffffffu, v, 0);
         const double L = n > 0.0 ? S / n : 0.0;
@@ -222,6 +235,7 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     }
   }
   if (lane < 8) sg[warp][lane] = acc;
+  if (kJoint && lane == 8) sj[warp] = acc;
   __syncthreads();
   double g = 0.0;                                    // warp 0, lane k < 8: sum over warps in a fixed order
   if (tid < 8) {
@@ -229,6 +243,11 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     for (int w = 0; w < kFinThreads / 32; ++w) g += sg[w][tid];
     if (tid == 0) p.loss_part[c] = g;
     else if (tid >= 2) { g /= (double)p.P; p.grad[6 * (size_t)c + tid - 2] = g; }
+  } else if (kJoint && tid == 8) {
+#pragma unroll
+    for (int w = 0; w < kFinThreads / 32; ++w) g += sj[w];
+    g /= (double)p.P;
+    p.glogf[c] = g;
   }
   if (!p.step_mode) {
     // evaluation only (epo_loss_grad): the last CTA adds the per-target loss sums
@@ -274,6 +293,22 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
       for (int k = 0; k < 12; ++k) { sT[k] = Tn[k]; sT[12 + k] = T[k]; }
     }
   }
+  if (kJoint && tid == 8) {
+    // focal scale (Eq. 4): f_c = f0_c (1 + gamma_c), stepped in every iteration ("the first phase ...
+    // drives updates to the camera intrinsics K and poses P").  AdamW [PAPER.md:121] with the loop's
+    // learning rate, decay towards the identity value 0; d L / d gamma = (d L / d ln f) / (1 + gamma); step number s + 1.
+    const int N_ = p.N;
+    const double lr = p.sched[4 * (size_t)s], c1 = p.sched[4 * (size_t)s + 1], c2 = p.sched[4 * (size_t)s + 2];
+    double gm = p.gamma[c];
+    const double gg = g / (1.0 + gm);
+    gm -= lr * p.wd * gm;
+    const double mm = p.beta1 * p.gamma[N_ + c] + (1.0 - p.beta1) * gg, vv = p.beta2 * p.gamma[2 * N_ + c] + (1.0 - p.beta2) * gg * gg;
+    p.gamma[N_ + c] = mm; p.gamma[2 * N_ + c] = vv;
+    gm -= lr * (mm / c1) / (sqrt(vv / c2) + p.adam_eps);
+    p.gamma[c] = gm;
+    p.K[4 * c] = (float)((double)p.K0[4 * c] * (1.0 + gm));
+    p.K[4 * c + 1] = (float)((double)p.K0[4 * c + 1] * (1.0 + gm));
+  }
   __syncthreads();
   // ---- a-11 pose change of this camera: three warps side by side
   if (tid == 0) {
@@ -308,10 +343,7 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     sdR[i] = __ldcg(p.dR + i); sdt[i] = __ldcg(p.dt + i);
     lv += __ldcg(p.loss_part + i);
   }
-  for (int i = tid; i < 12 * N; i += kFinThreads) {
-    if (p.poses_prev) p.poses_prev[i] = p.poses[i];
-    p.poses[i] = __ldcg(p.poses_next + i);
-  }
+  for (int i = tid; i < 12 * N; i += kFinThreads) p.poses[i] = __ldcg(p.poses_next + i);
   const double loss = block_sum(lv, &sg[0][0]) / (double)p.P;     // (contains the barrier that publishes sdR / sdt)
   // 95th percentiles, linear interpolation at rank 0.95 (N-1) (reading S12)
   const double rank = 95.0 / 100.0 * (double)(N - 1);
@@ -374,13 +406,15 @@ __global__ void k_f32_to_f64(const float* __restrict__ in, double* __restrict__ 
 
 }  // namespace
 
-epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset) {
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset, bool joint) {
   FinParams p;
+  p.gamma = ctx->d_gamma; p.glogf = ctx->d_glogf; p.K0 = ctx->d_K0; p.K = ctx->d_K; p.wd = ctx->cfg.weight_decay;
+  if (joint && !ctx->d_glogf) return epo_fail(ctx, EPO_ERR_BAD_STATE, "joint-phase reduction without joint state");
   p.sel_flag = subset ? ctx->d_sel_flag : nullptr;
   p.pairs = ctx->d_pairs; p.tgt_off = ctx->d_tgt_off; p.src_off = ctx->d_src_off; p.src_inc = ctx->d_src_inc;
   p.work_off = ctx->d_work_off; p.part = ctx->d_part; p.pair_loss = ctx->d_pair_loss; p.pair_valid = ctx->d_pair_valid;
   p.grad = ctx->d_grad; p.loss_part = ctx->d_loss_part;
-  p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.poses_prev = ctx->cfg.joint_phase ? ctx->d_poses_prev : nullptr; p.m = ctx->d_m; p.v = ctx->d_v;
+  p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.m = ctx->d_m; p.v = ctx->d_v;
   p.dR = ctx->d_dR; p.dt = ctx->d_dt; p.theta = ctx->d_theta; p.loss_trace = ctx->d_loss_trace;
   p.state = ctx->d_state; p.N = ctx->N;
   p.P = subset ? (int64_t)ctx->cfg.pair_budget : ctx->P;     // the mean runs over the pairs that were evaluated
@@ -391,8 +425,10 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   p.gated = gated ? 1 : 0; p.step_mode = step_mode ? 1 : 0; p.call_first = call_first ? 1 : 0;
   const size_t smem = (size_t)2 * ctx->N * sizeof(double);   // the last CTA's copy of dR, dt
   if (smem > 200 * 1024) return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "more than %d views", 200 * 1024 / 16);
-  if (smem > 48 * 1024)
-    EPO_CUDA(ctx, cudaFuncSetAttribute(k_finish, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  if (smem > 48 * 1024) {
+    EPO_CUDA(ctx, cudaFuncSetAttribute(k_finish<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    EPO_CUDA(ctx, cudaFuncSetAttribute(k_finish<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  }
   // programmatic dependent launch: the CTAs may become resident while the fused kernel drains; they wait in
   // cudaGridDependencySynchronize() before touching anything it (or an earlier kernel) wrote
   cudaLaunchConfig_t lc = {};
@@ -400,7 +436,7 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at; lc.numAttrs = ctx->pdl ? 1 : 0;
-  EPO_CUDA(ctx, cudaLaunchKernelEx(&lc, k_finish, p));
+  EPO_CUDA(ctx, joint ? cudaLaunchKernelEx(&lc, k_finish<true>, p) : cudaLaunchKernelEx(&lc, k_finish<false>, p));
   ctx->launches += 1;
   EPO_CUDA(ctx, cudaGetLastError());
   return EPO_OK;

@@ -175,22 +175,17 @@ def test_full_size_edge_extraction_config3_shape():
 
 
 def test_full_size_config3_joint_phase_gradients():
-    """Config 3 at full size: d L / d ln f of all 100 cameras and d L / d Z of all 1.6 M edge pixels against the oracle."""
+    """Config 3 at full size: d L / d ln f of all 100 cameras and d L / d Z of all 1.6 M edge pixels against the
+    all-double oracle (tolerances and slack: test_gpu_parity._check_joint_grads)."""
     import time
+    from test_gpu_parity import _check_joint_grads
     sc, e, prob = _full(3)
     e.loss_grad_joint(10.0)
     t0 = time.perf_counter(); got = e.loss_grad_joint(10.0); t_gpu = time.perf_counter() - t0
     t0 = time.perf_counter()
-    gf, gz = oracle.joint_grad(prob, sc.poses_init.astype(np.float64), sc.pairs, 10.0, z_min=Z_MIN, coord_fp32=1)
+    rep = _check_joint_grads(got, prob, sc.poses_init.astype(np.float64), sc.pairs, 10.0, "config 3")
     t_cpu = time.perf_counter() - t0
-    assert np.all(np.abs(got["g_logf"] - gf) <= 1e-4 * np.abs(gf) + 1e-9)
-    worst = 0.0
-    for i in range(sc.n_views):
-        lo, hi = prob.edge_off[i], prob.edge_off[i + 1]
-        u, v = prob.uv[lo:hi, 0].astype(int), prob.uv[lo:hi, 1].astype(int)
-        mine, ref = got["g_depth"][i, v, u].astype(np.float64), gz[lo:hi]
-        worst = max(worst, np.linalg.norm(mine - ref) / np.linalg.norm(ref))
-    assert worst <= 1e-4
-    print(f"config 3 joint gradients: d/dZ per-view rel err max {worst:.2e}; library call {1e3 * t_gpu:.1f} ms (incl. the D2H of "
-          f"the 81 MB map), oracle {t_cpu:.1f} s (serial over pairs)")
+    print(f"config 3 joint gradients: d/dlnf err {rep['logf']:.1e} of its scale; d/dZ per-view rel err max {rep['gz_view']:.1e}, worst entry "
+          f"{rep['gz_entry']:.1e} of the largest; library call {1e3 * t_gpu:.1f} ms (incl. the D2H of the 81 MB map), oracle + slack "
+          f"{t_cpu:.1f} s (serial over pairs)")
     e.destroy()

@@ -146,3 +146,42 @@ def test_T1d_slack_is_small_where_it_should_be():
         bt, bs, _ = _bounds(ref, oracle.pair_event_slack(uv, z, Ks, Kt, poses[s], poses[t], prob.dtf[t], 10.0), p)
         cam[t] += bt; cam[s] += bs
     assert np.allclose(cam / len(sc.pairs), sl["cam"], rtol=1e-12, atol=0)
+
+
+def test_T1e_joint_phase_slack_holds_for_displaced_and_binary32_evaluations():
+    """The same bound for the joint phase's gradients (orc_joint_slack): d L / d ln f per camera and d L / d Z per edge
+    pixel of evaluations whose projected positions are displaced by less than the binary32 position error (all
+    principal points shifted by a few 1e-6 px) and of the oracle's binary32-position variant stay within
+    2e-5 relative + slack of the nominal all-double result; entries without any event in reach have zero slack."""
+    import copy
+    sc = make_scene(2, n_views=5)
+    prob = oracle.preprocess(sc.K, sc.depth, sc.edges)
+    poses = sc.poses_init.astype(np.float64)
+    lam = 8.0
+    gf, gz = oracle.joint_grad(prob, poses, sc.pairs, lam)
+    sl = oracle.joint_slack(prob, poses, sc.pairs, lam)
+    assert np.all(np.isfinite(sl["logf"])) and np.all(np.isfinite(sl["gz"]))
+    assert (sl["gz"] == 0).mean() > 0.95 and (sl["gz"] > 0).sum() > 10
+    scale_f = np.maximum(np.abs(gf), sl["logf_rss"])
+    cases = [oracle.joint_grad(prob, poses, sc.pairs, lam, coord_fp32=1)]
+    for dx, dy in ((3e-6, 0.0), (-3e-6, 3e-6), (3e-6, -3e-6)):
+        p2 = copy.copy(prob); p2.K = prob.K.astype(np.float64)
+        # float32 intrinsics cannot carry a 1e-6 px shift: displace through the (double) poses instead -- a rotation
+        # of every camera about its own y / x axis by dx / fx, dy / fy moves every projection by about (dx, dy)
+        P2 = poses.reshape(-1, 3, 4).copy()
+        for c in range(sc.n_views):
+            ax, ay = dy / sc.K[c, 1], -dx / sc.K[c, 0]
+            R = np.array([[1, 0, -ay], [0, 1, ax], [ay, -ax, 1.0]])          # first order: Exp of a 1e-8 rad twist
+            P2[c] = R @ P2[c]
+        cases.append(oracle.joint_grad(prob, P2.reshape(-1, 12), sc.pairs, lam))
+    moved = 0
+    for k, (f2, z2) in enumerate(cases):
+        # what the displacement itself moves the continuous part by: a binary32 position is off by up to ~1e-4 px, and a
+        # single edge pixel's derivative (a sum over a handful of pairs, nothing averages) follows the interpolant's
+        # curvature with it -- 1e-3 relative per entry, 1e-4 on a camera's sum; the 3e-6 px displacements: 2e-5
+        rel_z, rel_f = (1e-3, 1e-4) if k == 0 else (2e-5, 2e-5)
+        assert np.all(np.abs(f2 - gf) <= rel_f * scale_f + sl["logf"])
+        tol = rel_z * np.abs(gz) + rel_z * 0.1 * np.abs(gz).max() + sl["gz"]
+        assert np.all(np.abs(z2 - gz) <= tol), float(np.max(np.abs(z2 - gz) - tol))
+        moved += int(np.sum((sl["gz"] > 0) & (np.abs(z2 - gz) > 0.2 * sl["gz"])))     # a flagged entry really flipped
+    assert moved >= 1                                   # a flagged sample did change cell / branch, inside its slack
