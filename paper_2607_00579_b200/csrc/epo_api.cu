@@ -67,7 +67,9 @@ void free_views(epo_ctx* c) {
   c->d_edge_off = nullptr; c->d_edges = nullptr;
   c->have_views = false;
 }
+void destroy_step_graph(epo_ctx* c);
 void free_pairs(epo_ctx* c) {
+  destroy_step_graph(c);
   epo_dfree(c, c->d_pairs); epo_dfree(c, c->d_perm); epo_dfree(c, c->d_tgt_off); epo_dfree(c, c->d_src_off); epo_dfree(c, c->d_src_inc);
   epo_dfree(c, c->d_work); epo_dfree(c, c->d_work_off); epo_dfree(c, c->d_part); epo_dfree(c, c->d_pair_loss); epo_dfree(c, c->d_pair_valid); epo_dfree(c, c->d_out_f);
   epo_dfree(c, c->d_dz); c->d_dz = nullptr;
@@ -94,6 +96,77 @@ int choose_chunk(const epo_ctx* c, const std::vector<int32_t>& pairs, int64_t P)
   if (passes > kLgOuter) passes = kLgOuter;
   if (const char* v = std::getenv("EPO_LG_PASSES")) { int k = std::atoi(v); if (k >= 1 && k <= kLgMaxOuter) passes = k; }
   return (int)passes * kLgPass;
+}
+
+void destroy_step_graph(epo_ctx* c) {
+  if (c->step_exec) cudaGraphExecDestroy(c->step_exec);
+  if (c->step_graph) cudaGraphDestroy(c->step_graph);
+  c->step_exec = nullptr; c->step_graph = nullptr; c->step_begin_node = nullptr; c->step_cond = 0;
+}
+
+// One iteration as the loop enqueues it: [select pairs] -> fused -> finish -> [joint points], every kernel self-gated
+// by DevState.halt, chained by programmatic dependent launch.
+epo_status enqueue_iteration(epo_ctx* c, cudaGraphConditionalHandle cond) {
+  const bool joint = c->cfg.joint_phase != 0;
+  if (c->subsample) EPO_TRY(epo_launch_select_pairs(c, -1, true, true));
+  EPO_TRY(epo_launch_fused(c, -1.0f, true, c->subsample, joint));
+  EPO_TRY(epo_launch_finish(c, true, true, c->subsample, joint, cond));
+  // joint phase: AdamW on (alpha, beta) where due and the points again from the new K and Z (gamma was stepped in
+  // k_finish); self-gated by DevState.joint_pending
+  if (joint) EPO_TRY(epo_launch_joint_points(c, c->subsample));
+  return EPO_OK;
+}
+
+// The whole epo_step call as one graph: k_begin_step_call (iteration budget, initial condition) -> WHILE(condition)
+// { graph_unroll iterations }.  The body is captured from the very launches the host loop would issue, so the
+// programmatic-dependent-launch edges between its kernels are kept; k_finish sets the condition, and once it is 0
+// nothing more is launched (PAPER.md:436-446 is a host `break`; SURVEY.md section 3 "a CUDA-graph conditional loop").
+// On any failure the context falls back to the host loop (use_graph = false).
+epo_status build_step_graph(epo_ctx* c) {
+  destroy_step_graph(c);
+  cudaError_t e = cudaGraphCreate(&c->step_graph, 0);
+  if (e == cudaSuccess) e = cudaGraphConditionalHandleCreate(&c->step_cond, c->step_graph, 0, 0);
+  EpoBeginArgs ba;
+  if (e == cudaSuccess) {
+    epo_begin_step_call_args(c, 0, c->step_cond, &ba);
+    cudaKernelNodeParams kp = {};
+    kp.func = ba.func; kp.gridDim = dim3(1); kp.blockDim = dim3(1); kp.sharedMemBytes = 0; kp.kernelParams = ba.ptrs; kp.extra = nullptr;
+    e = cudaGraphAddKernelNode(&c->step_begin_node, c->step_graph, nullptr, 0, &kp);
+  }
+  cudaGraph_t body = nullptr;
+  if (e == cudaSuccess) {
+    cudaGraphNodeParams cp = {};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = c->step_cond; cp.conditional.type = cudaGraphCondTypeWhile; cp.conditional.size = 1;
+    cudaGraphNode_t cnode = nullptr;
+    e = cudaGraphAddNode(&cnode, c->step_graph, &c->step_begin_node, 1, &cp);
+    if (e == cudaSuccess) body = cp.conditional.phGraph_out[0];
+  }
+  epo_status rc = EPO_OK;
+  if (e == cudaSuccess) {
+    // capture the iterations on a private stream (the caller's may be the legacy default stream, which cannot capture)
+    cudaStream_t user = c->stream;
+    const int64_t launches = c->launches;
+    const bool dirty = c->static_dirty;
+    c->static_dirty = false;                         // inside the graph every launch follows the loop's own kernels
+    e = cudaStreamBeginCaptureToGraph(c->capture_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+    if (e == cudaSuccess) {
+      c->stream = c->capture_stream;
+      for (int u = 0; u < c->graph_unroll && rc == EPO_OK; ++u) rc = enqueue_iteration(c, c->step_cond);
+      c->stream = user;
+      cudaGraph_t got = nullptr;
+      e = cudaStreamEndCapture(c->capture_stream, &got);
+    }
+    c->launches = launches; c->static_dirty = dirty;
+  }
+  if (e == cudaSuccess && rc == EPO_OK) e = cudaGraphInstantiate(&c->step_exec, c->step_graph, 0);
+  if (e != cudaSuccess || rc != EPO_OK) {
+    cudaGetLastError();
+    destroy_step_graph(c);
+    c->use_graph = false;
+    if (std::getenv("EPO_TRACE")) fprintf(stderr, "[epo trace] loop graph unavailable (%s): host launch loop\n", cudaGetErrorString(e));
+  }
+  return EPO_OK;
 }
 
 epo_status reset_optimiser(epo_ctx* c, bool joint = true) {
@@ -151,6 +224,10 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   c->pool = nullptr; c->own_pool = false;
   c->atlas = EpoAtlas{nullptr, nullptr, 0, 0, 1};
   c->packed.xyz = nullptr; c->packed.pix = nullptr; c->packed.d_off = nullptr;
+  { const char* v = std::getenv("EPO_NO_GRAPH"); c->use_graph = !(v && v[0] && v[0] != '0'); }
+  c->graph_unroll = 8;
+  if (const char* v = std::getenv("EPO_GRAPH_UNROLL")) { const int k = std::atoi(v); if (k >= 1 && k <= 64) c->graph_unroll = k; }
+  c->capture_stream = nullptr; c->step_graph = nullptr; c->step_exec = nullptr; c->step_begin_node = nullptr; c->step_cond = 0;
   { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
   c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
@@ -173,6 +250,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   }
   if (e == cudaSuccess) {
     e = cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_alloc, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming);
   }
@@ -212,6 +290,7 @@ void epo_destroy(epo_ctx* c) {
   cudaStreamSynchronize(c->stream);                 // the frees are stream-ordered: done before the context goes
   if (c->own_pool && c->pool) cudaMemPoolDestroy(c->pool);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
   if (c->ev_alloc) cudaEventDestroy(c->ev_alloc);
   if (c->ev_copied) cudaEventDestroy(c->ev_copied);
   cudaGetLastError();
@@ -411,7 +490,7 @@ epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
   EPO_TRY(epo_launch_fused(c, lambda, false, false, false));
-  EPO_TRY(epo_launch_finish(c, false, false, false, false, false));
+  EPO_TRY(epo_launch_finish(c, false, false, false, false, 0));
   bool sync = false;
   // loss: DevState.loss (double) -> float
   epo_launch_f64_to_f32(st, &c->d_state->loss, c->d_out_f, 1);
@@ -463,7 +542,7 @@ epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_l
     c->d_dz = keep;
     c->static_dirty = true;                          // (the launch above was not the loop's: keep the next one serialised)
   }
-  if (rc == EPO_OK) rc = epo_launch_finish(c, false, false, false, false, true);
+  if (rc == EPO_OK) rc = epo_launch_finish(c, false, false, false, true, 0);
   if (rc == EPO_OK) rc = epo_joint_gather_gz(c, dz, gz_dev ? g_depth : d_gz);
   bool sync = false;
   if (rc == EPO_OK) {
@@ -514,15 +593,23 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
   if (n_iters < 0) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_step: negative iteration count");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
-  if (n_iters == 0) EPO_TRY(epo_launch_begin_step_call(c));
-  const bool joint = c->cfg.joint_phase != 0;
-  for (int i = 0; i < n_iters; ++i) {
-    if (c->subsample) EPO_TRY(epo_launch_select_pairs(c, -1, true, true));
-    EPO_TRY(epo_launch_fused(c, -1.0f, true, c->subsample, joint));
-    EPO_TRY(epo_launch_finish(c, true, true, i == 0, c->subsample, joint));
-    // joint phase: AdamW on (alpha, beta) where due and the points again from the new K and Z (gamma was stepped in
-    // k_finish); self-gated by DevState.joint_pending
-    if (joint) EPO_TRY(epo_launch_joint_points(c, c->subsample));
+  if (n_iters > 0 && c->use_graph && !c->step_exec) EPO_TRY(build_step_graph(c));
+  if (n_iters > 0 && c->use_graph && c->step_exec) {
+    // one launch for the whole call: the graph loops on the device until the budget is used up or the rule stops it.
+    // Its first launch after the static data changed must not overlap the kernels that wrote them: the graph is
+    // launched into the stream after them, and its first node is the (serialised) begin kernel.
+    EpoBeginArgs ba;
+    epo_begin_step_call_args(c, n_iters, c->step_cond, &ba);
+    cudaKernelNodeParams kp = {};
+    kp.func = ba.func; kp.gridDim = dim3(1); kp.blockDim = dim3(1); kp.sharedMemBytes = 0; kp.kernelParams = ba.ptrs; kp.extra = nullptr;
+    EPO_CUDA(c, cudaGraphExecKernelNodeSetParams(c->step_exec, c->step_begin_node, &kp));
+    EPO_CUDA(c, cudaGraphLaunch(c->step_exec, st));
+    c->static_dirty = false;
+    // kernels the call runs if no rule stops it (what the host loop would have launched)
+    c->launches += 1 + (int64_t)n_iters * (2 + (c->subsample ? 1 : 0) + (c->cfg.joint_phase ? 1 : 0));
+  } else {
+    EPO_TRY(epo_launch_begin_step_call(c, n_iters));
+    for (int i = 0; i < n_iters; ++i) EPO_TRY(enqueue_iteration(c, 0));
   }
   bool sync = false;
   if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));

@@ -48,7 +48,7 @@ constexpr int kLgMaxOuter = 32;
 constexpr int kLgPad = kLgPass * kLgMaxOuter;  // zero points appended to the list: tail lanes / prefetches read past a list
 
 // Device-resident control block of the optimisation loop (rows a-10..a-12): lets epo_step enqueue
-// n iterations without any host synchronisation; every kernel of an iteration checks `stopped`.
+// n iterations without any host synchronisation; every kernel of an iteration checks `halt`.
 struct DevState {
   int32_t step;        // optimiser step counter s (0-based index of the NEXT update)
   int32_t phase;       // 0, 1, 2 (Alg. 2 l.13-17)
@@ -58,6 +58,9 @@ struct DevState {
   int32_t joint_pending;   // joint loop: an iteration has completed and its joint pass / variable update are due
   int32_t phase1_step; // joint loop: iteration index at which phase 0 -> 1 happened (depth steps from the next one)
   int32_t ticket;      // CTAs of k_finish that have finished (the last one runs the serial tail and re-zeroes it)
+  int32_t budget;      // iterations the epo_step call in flight may still run at most (set by k_begin_step_call)
+  int32_t halt;        // stopped || iters_done >= budget: what the kernels of an iteration test, and the negation of
+                       // the loop graph's WHILE condition
   int32_t pad_;
   double loss;         // loss of the last evaluation
 };
@@ -103,6 +106,16 @@ struct epo_ctx {
   int N, W, H;
   bool have_views, have_pairs;
   bool pdl;            // programmatic dependent launch between the kernels of the loop (EPO_NO_PDL=1 turns it off)
+  // The loop as ONE graph launch per epo_step call (epo_api.cu: build_step_graph): k_begin_step_call, then a conditional
+  // WHILE node whose body is `unroll` iterations captured with their programmatic dependencies; k_finish sets the
+  // condition.  Rebuilt whenever the pair list (and with it the kernels' arguments) changes.  EPO_NO_GRAPH=1: host loop.
+  bool use_graph;
+  int graph_unroll;
+  cudaStream_t capture_stream;
+  cudaGraph_t step_graph;
+  cudaGraphExec_t step_exec;
+  cudaGraphNode_t step_begin_node;
+  cudaGraphConditionalHandle step_cond;
   bool static_dirty;   // work list / points / fields were (re)built since the last fused launch: launch it serialised
   int64_t P, E, n_work, reproj_per_eval, launches;
   int lg_chunk;        // samples per work item of the fused kernel (a multiple of kLgPass), chosen in epo_set_pairs
@@ -263,9 +276,14 @@ epo_status epo_launch_fused_only(epo_ctx* ctx, float lambda);   // the fused ker
 epo_status epo_launch_record_taps(epo_ctx* ctx, float lambda, uint2* d_taps);                  // gather ceiling: the tap stream
 epo_status epo_launch_gather_taps(epo_ctx* ctx, float lambda, const uint2* d_taps, unsigned* d_out);   // ... replayed alone
 // update.cu: k_finish = per-camera reduction (+ Adam, retraction, pose change, stop test when step_mode)
-epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset, bool joint);
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool subset, bool joint,
+                             cudaGraphConditionalHandle cond /* 0: not inside the loop graph */);
 epo_status epo_launch_fill_schedule(epo_ctx* ctx);     // d_sched from the configuration (once, in epo_create)
-epo_status epo_launch_begin_step_call(epo_ctx* ctx);   // zero iters_done (an epo_step call of zero iterations)
+// first kernel of every epo_step call: iters_done = 0, budget = n_iters, stopped / halt from the current state
+epo_status epo_launch_begin_step_call(epo_ctx* ctx, int n_iters);
+// the same kernel as a graph node (epo_api.cu builds the node and updates n_iters before every graph launch)
+struct EpoBeginArgs { DevState* st; int n_iters, max_steps, early_stop; cudaGraphConditionalHandle cond; void* ptrs[5]; void* func; };
+void epo_begin_step_call_args(epo_ctx* ctx, int n_iters, cudaGraphConditionalHandle cond, EpoBeginArgs* a);
 void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n);
 void epo_launch_f32_to_f64(cudaStream_t st, const float* in, double* out, int64_t n);
 void epo_launch_scatter_pair_outputs(cudaStream_t st, const float* pl, const int32_t* pv, const int32_t* perm,

@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(kSelThreads, 1) k_select_pairs(const SelParams
   for (int i = tid; i < kSelBins; i += kSelThreads) hist[i] = 0;
   cudaTriggerProgrammaticLaunchCompletion();
   cudaGridDependencySynchronize();
-  if (p.gated && p.state->stopped) return;
+  if (p.gated && p.state->halt) return;
   const int step = p.step_override >= 0 ? p.step_override : p.state->step;
   unsigned long long key[kSelUnroll];
 #pragma unroll

@@ -40,7 +40,8 @@ struct FinParams {
   const double* sched;          // [max_steps][4] {lr_s, 1 - beta1^(s+1), 1 - beta2^(s+1), lambda_s}
   int max_steps, w1, w2, smooth, early_stop, stop_rule, w_loss;
   double eps_loss;
-  int gated, step_mode, call_first;
+  int gated, step_mode;
+  cudaGraphConditionalHandle cond;   // the loop graph's WHILE condition (0 outside the graph)
 };
 
 // sum over the CTA in a fixed order (xor tree inside each warp, then the warps in index order); every thread
@@ -181,8 +182,11 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   fetch(j0, &q, &w0, &w1);
   cudaTriggerProgrammaticLaunchCompletion();       // the next fused kernel may start its own static prologue
   cudaGridDependencySynchronize();                 // partial sums, poses and the control block are final now
-  if (p.gated && st->stopped) {
-    if (blockIdx.x == 0 && threadIdx.x == 0) { if (p.call_first) st->iters_done = 0; st->joint_pending = 0; }
+  if (p.gated && st->halt) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+      st->joint_pending = 0;
+      if (p.cond) cudaGraphSetConditional(p.cond, 0);
+    }
     return;
   }
   const double* Pc = p.poses + 12 * (size_t)c;
@@ -370,8 +374,12 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     st->phase_prev = phase0; st->joint_pending = 1;
     if (phase0 == 0 && phase == 1) st->phase1_step = s;
     st->step = s + 1;
-    st->iters_done = p.call_first ? 1 : st->iters_done + 1;
-    st->stopped = (s + 1 >= p.max_steps) || (p.early_stop && phase == 2);
+    const int done = st->iters_done + 1;
+    const int stopped = (s + 1 >= p.max_steps) || (p.early_stop && phase == 2);
+    const int halt = stopped || done >= st->budget;
+    st->iters_done = done; st->stopped = stopped; st->halt = halt;
+    // the loop graph runs its body again only while the call may go on: nothing is launched after the stop
+    if (p.cond) cudaGraphSetConditional(p.cond, halt ? 0u : 1u);
     st->ticket = 0;
   }
 }
@@ -390,9 +398,11 @@ __global__ void k_fill_schedule(double* __restrict__ sched, int max_steps, doubl
   sched[4 * s + 3] = (double)(float)(clamp_start + (clamp_end - clamp_start) * (double)m / (double)clamp_steps);
 }
 
-__global__ void k_begin_step_call(DevState* st, int max_steps, int early_stop) {
-  st->iters_done = 0;
-  st->stopped = (st->step >= max_steps) || (early_stop && st->phase == 2);
+__global__ void k_begin_step_call(DevState* st, int n_iters, int max_steps, int early_stop, cudaGraphConditionalHandle cond) {
+  const int stopped = (st->step >= max_steps) || (early_stop && st->phase == 2);
+  const int halt = stopped || n_iters <= 0;
+  st->iters_done = 0; st->budget = n_iters; st->stopped = stopped; st->halt = halt;
+  if (cond) cudaGraphSetConditional(cond, halt ? 0u : 1u);
 }
 
 __global__ void k_f64_to_f32(const double* __restrict__ in, float* __restrict__ out, int64_t n) {
@@ -406,7 +416,7 @@ __global__ void k_f32_to_f64(const float* __restrict__ in, double* __restrict__ 
 
 }  // namespace
 
-epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call_first, bool subset, bool joint) {
+epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool subset, bool joint, cudaGraphConditionalHandle cond) {
   FinParams p;
   p.gamma = ctx->d_gamma; p.glogf = ctx->d_glogf; p.K0 = ctx->d_K0; p.K = ctx->d_K; p.wd = ctx->cfg.weight_decay;
   if (joint && !ctx->d_glogf) return epo_fail(ctx, EPO_ERR_BAD_STATE, "joint-phase reduction without joint state");
@@ -422,7 +432,7 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool call
   p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.max_steps = ctx->cfg.max_steps;
   p.w1 = ctx->cfg.w1; p.w2 = ctx->cfg.w2; p.smooth = ctx->cfg.smooth_window; p.early_stop = ctx->cfg.early_stop;
   p.stop_rule = ctx->cfg.stop_rule; p.w_loss = ctx->cfg.w_loss; p.eps_loss = ctx->cfg.eps_loss;
-  p.gated = gated ? 1 : 0; p.step_mode = step_mode ? 1 : 0; p.call_first = call_first ? 1 : 0;
+  p.gated = gated ? 1 : 0; p.step_mode = step_mode ? 1 : 0; p.cond = cond;
   const size_t smem = (size_t)2 * ctx->N * sizeof(double);   // the last CTA's copy of dR, dt
   if (smem > 200 * 1024) return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "more than %d views", 200 * 1024 / 16);
   if (smem > 48 * 1024) {
@@ -451,11 +461,17 @@ epo_status epo_launch_fill_schedule(epo_ctx* ctx) {
   return EPO_OK;
 }
 
-epo_status epo_launch_begin_step_call(epo_ctx* ctx) {
-  k_begin_step_call<<<1, 1, 0, ctx->stream>>>(ctx->d_state, ctx->cfg.max_steps, ctx->cfg.early_stop);
+epo_status epo_launch_begin_step_call(epo_ctx* ctx, int n_iters) {
+  k_begin_step_call<<<1, 1, 0, ctx->stream>>>(ctx->d_state, n_iters, ctx->cfg.max_steps, ctx->cfg.early_stop, 0);
   ctx->launches += 1;
   EPO_CUDA(ctx, cudaGetLastError());
   return EPO_OK;
+}
+
+void epo_begin_step_call_args(epo_ctx* ctx, int n_iters, cudaGraphConditionalHandle cond, EpoBeginArgs* a) {
+  a->st = ctx->d_state; a->n_iters = n_iters; a->max_steps = ctx->cfg.max_steps; a->early_stop = ctx->cfg.early_stop; a->cond = cond;
+  a->ptrs[0] = &a->st; a->ptrs[1] = &a->n_iters; a->ptrs[2] = &a->max_steps; a->ptrs[3] = &a->early_stop; a->ptrs[4] = &a->cond;
+  a->func = (void*)k_begin_step_call;
 }
 
 void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n) {
