@@ -128,7 +128,7 @@ epo_status build_step_graph(epo_ctx* c) {
   if (e == cudaSuccess) e = cudaGraphConditionalHandleCreate(&c->step_cond, c->step_graph, 0, 0);
   EpoBeginArgs ba;
   if (e == cudaSuccess) {
-    epo_begin_step_call_args(c, 0, c->step_cond, &ba);
+    epo_begin_step_call_args(c, 0, 0, c->step_cond, &ba);
     cudaKernelNodeParams kp = {};
     kp.func = ba.func; kp.gridDim = dim3(1); kp.blockDim = dim3(1); kp.sharedMemBytes = 0; kp.kernelParams = ba.ptrs; kp.extra = nullptr;
     e = cudaGraphAddKernelNode(&c->step_begin_node, c->step_graph, nullptr, 0, &kp);
@@ -593,20 +593,22 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
   if (n_iters < 0) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_step: negative iteration count");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
-  if (n_iters > 0 && c->use_graph && !c->step_exec) EPO_TRY(build_step_graph(c));
-  if (n_iters > 0 && c->use_graph && c->step_exec) {
-    // one launch for the whole call: the graph loops on the device until the budget is used up or the rule stops it.
-    // Its first launch after the static data changed must not overlap the kernels that wrote them: the graph is
-    // launched into the stream after them, and its first node is the (serialised) begin kernel.
+  // Whole bodies of the loop graph (graph_unroll iterations each) run as ONE launch that loops on the device until
+  // they are used up or the rule stops the loop; the remainder (and short calls) is enqueued kernel by kernel.  After a
+  // stop at most one body's and one remainder's worth of iterations is launched in vain (their kernels exit at once).
+  const int in_graph = c->use_graph ? n_iters / c->graph_unroll * c->graph_unroll : 0;
+  if (in_graph > 0 && !c->step_exec) EPO_TRY(build_step_graph(c));
+  if (in_graph > 0 && c->step_exec) {
     EpoBeginArgs ba;
-    epo_begin_step_call_args(c, n_iters, c->step_cond, &ba);
+    epo_begin_step_call_args(c, n_iters, in_graph, c->step_cond, &ba);
     cudaKernelNodeParams kp = {};
     kp.func = ba.func; kp.gridDim = dim3(1); kp.blockDim = dim3(1); kp.sharedMemBytes = 0; kp.kernelParams = ba.ptrs; kp.extra = nullptr;
     EPO_CUDA(c, cudaGraphExecKernelNodeSetParams(c->step_exec, c->step_begin_node, &kp));
     EPO_CUDA(c, cudaGraphLaunch(c->step_exec, st));
     c->static_dirty = false;
-    // kernels the call runs if no rule stops it (what the host loop would have launched)
-    c->launches += 1 + (int64_t)n_iters * (2 + (c->subsample ? 1 : 0) + (c->cfg.joint_phase ? 1 : 0));
+    // kernels these iterations run if no rule stops them (what the host loop would have launched)
+    c->launches += 1 + (int64_t)in_graph * (2 + (c->subsample ? 1 : 0) + (c->cfg.joint_phase ? 1 : 0));
+    for (int i = in_graph; i < n_iters; ++i) EPO_TRY(enqueue_iteration(c, 0));
   } else {
     EPO_TRY(epo_launch_begin_step_call(c, n_iters));
     for (int i = 0; i < n_iters; ++i) EPO_TRY(enqueue_iteration(c, 0));

@@ -59,9 +59,9 @@ struct DevState {
   int32_t phase1_step; // joint loop: iteration index at which phase 0 -> 1 happened (depth steps from the next one)
   int32_t ticket;      // CTAs of k_finish that have finished (the last one runs the serial tail and re-zeroes it)
   int32_t budget;      // iterations the epo_step call in flight may still run at most (set by k_begin_step_call)
-  int32_t halt;        // stopped || iters_done >= budget: what the kernels of an iteration test, and the negation of
-                       // the loop graph's WHILE condition
-  int32_t pad_;
+  int32_t halt;        // stopped || iters_done >= budget: what the kernels of an iteration test
+  int32_t graph_limit; // the loop graph runs its body again while !stopped && iters_done < graph_limit (the largest
+                       // multiple of its unroll factor within the budget; the host enqueues the remainder)
   double loss;         // loss of the last evaluation
 };
 
@@ -282,8 +282,8 @@ epo_status epo_launch_fill_schedule(epo_ctx* ctx);     // d_sched from the confi
 // first kernel of every epo_step call: iters_done = 0, budget = n_iters, stopped / halt from the current state
 epo_status epo_launch_begin_step_call(epo_ctx* ctx, int n_iters);
 // the same kernel as a graph node (epo_api.cu builds the node and updates n_iters before every graph launch)
-struct EpoBeginArgs { DevState* st; int n_iters, max_steps, early_stop; cudaGraphConditionalHandle cond; void* ptrs[5]; void* func; };
-void epo_begin_step_call_args(epo_ctx* ctx, int n_iters, cudaGraphConditionalHandle cond, EpoBeginArgs* a);
+struct EpoBeginArgs { DevState* st; int n_iters, graph_limit, max_steps, early_stop; cudaGraphConditionalHandle cond; void* ptrs[6]; void* func; };
+void epo_begin_step_call_args(epo_ctx* ctx, int n_iters, int graph_limit, cudaGraphConditionalHandle cond, EpoBeginArgs* a);
 void epo_launch_f64_to_f32(cudaStream_t st, const double* in, float* out, int64_t n);
 void epo_launch_f32_to_f64(cudaStream_t st, const float* in, double* out, int64_t n);
 void epo_launch_scatter_pair_outputs(cudaStream_t st, const float* pl, const int32_t* pv, const int32_t* perm,

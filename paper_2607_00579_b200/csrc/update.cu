@@ -379,7 +379,7 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
     const int halt = stopped || done >= st->budget;
     st->iters_done = done; st->stopped = stopped; st->halt = halt;
     // the loop graph runs its body again only while the call may go on: nothing is launched after the stop
-    if (p.cond) cudaGraphSetConditional(p.cond, halt ? 0u : 1u);
+    if (p.cond) cudaGraphSetConditional(p.cond, (stopped || done >= st->graph_limit) ? 0u : 1u);
     st->ticket = 0;
   }
 }
@@ -398,11 +398,12 @@ __global__ void k_fill_schedule(double* __restrict__ sched, int max_steps, doubl
   sched[4 * s + 3] = (double)(float)(clamp_start + (clamp_end - clamp_start) * (double)m / (double)clamp_steps);
 }
 
-__global__ void k_begin_step_call(DevState* st, int n_iters, int max_steps, int early_stop, cudaGraphConditionalHandle cond) {
+__global__ void k_begin_step_call(DevState* st, int n_iters, int graph_limit, int max_steps, int early_stop,
+                                  cudaGraphConditionalHandle cond) {
   const int stopped = (st->step >= max_steps) || (early_stop && st->phase == 2);
   const int halt = stopped || n_iters <= 0;
-  st->iters_done = 0; st->budget = n_iters; st->stopped = stopped; st->halt = halt;
-  if (cond) cudaGraphSetConditional(cond, halt ? 0u : 1u);
+  st->iters_done = 0; st->budget = n_iters; st->graph_limit = graph_limit; st->stopped = stopped; st->halt = halt;
+  if (cond) cudaGraphSetConditional(cond, (stopped || graph_limit <= 0) ? 0u : 1u);
 }
 
 __global__ void k_f64_to_f32(const double* __restrict__ in, float* __restrict__ out, int64_t n) {
@@ -462,15 +463,17 @@ epo_status epo_launch_fill_schedule(epo_ctx* ctx) {
 }
 
 epo_status epo_launch_begin_step_call(epo_ctx* ctx, int n_iters) {
-  k_begin_step_call<<<1, 1, 0, ctx->stream>>>(ctx->d_state, n_iters, ctx->cfg.max_steps, ctx->cfg.early_stop, 0);
+  k_begin_step_call<<<1, 1, 0, ctx->stream>>>(ctx->d_state, n_iters, 0, ctx->cfg.max_steps, ctx->cfg.early_stop, 0);
   ctx->launches += 1;
   EPO_CUDA(ctx, cudaGetLastError());
   return EPO_OK;
 }
 
-void epo_begin_step_call_args(epo_ctx* ctx, int n_iters, cudaGraphConditionalHandle cond, EpoBeginArgs* a) {
-  a->st = ctx->d_state; a->n_iters = n_iters; a->max_steps = ctx->cfg.max_steps; a->early_stop = ctx->cfg.early_stop; a->cond = cond;
-  a->ptrs[0] = &a->st; a->ptrs[1] = &a->n_iters; a->ptrs[2] = &a->max_steps; a->ptrs[3] = &a->early_stop; a->ptrs[4] = &a->cond;
+void epo_begin_step_call_args(epo_ctx* ctx, int n_iters, int graph_limit, cudaGraphConditionalHandle cond, EpoBeginArgs* a) {
+  a->st = ctx->d_state; a->n_iters = n_iters; a->graph_limit = graph_limit; a->max_steps = ctx->cfg.max_steps;
+  a->early_stop = ctx->cfg.early_stop; a->cond = cond;
+  a->ptrs[0] = &a->st; a->ptrs[1] = &a->n_iters; a->ptrs[2] = &a->graph_limit; a->ptrs[3] = &a->max_steps; a->ptrs[4] = &a->early_stop;
+  a->ptrs[5] = &a->cond;
   a->func = (void*)k_begin_step_call;
 }
 

@@ -755,6 +755,29 @@ def test_set_pairs_keeps_the_current_poses():
     e.destroy()
 
 
+@pytest.mark.parametrize("kw", [dict(), dict(pair_budget=9, subsample_seed=5), dict(pair_budget=1024, subsample_seed=7, dup=400)])
+def test_loop_is_bit_reproducible(kw):
+    """compute-sanitizer is closed on this GPU pool (profiles/r2_sanitizer.md), so data races are hunted the other way
+    round: the loop has no atomics on values and fixed reduction orders, hence ANY race -- in the fused kernel's block
+    reduction, k_finish's last-CTA ticket, k_select_pairs' grid barriers (the 4,800-pair list spans two of its CTAs) --
+    shows as run-to-run differences.  Three runs of 40 iterations must give bit-identical poses and traces."""
+    kw = dict(kw)
+    dup = kw.pop("dup", 1)
+    sc = scene("tiny") if dup > 1 else scene("room6")
+    pairs = np.ascontiguousarray(np.tile(sc.pairs, (dup, 1)))
+    outs = []
+    for _ in range(3):
+        e = make_ctx(sc, early_stop=0, **kw)
+        if dup > 1:
+            e.set_pairs(pairs)
+        assert e.step(40)[0] == 40
+        outs.append((e.get_poses_f64(),) + e.get_trace(0, 40))
+        e.destroy()
+    for o in outs[1:]:
+        for a, b in zip(outs[0], o):
+            assert np.array_equal(a, b)
+
+
 def test_step_in_pieces_equals_one_call():
     sc = scene("tiny")
     a = make_ctx(sc, early_stop=0); b = make_ctx(sc, early_stop=0)
