@@ -47,6 +47,7 @@ def parse():
     ap.add_argument("--joint-phase", type=int, default=0,
                     help="1: epo_step also optimises focal scale and edge-pixel depth (DESIGN.md 6.7); a step then runs "
                          "the fused kernel twice, value still counts the loss's reprojections once")
+    ap.add_argument("--dtf-format", type=int, default=0, help="1: fp16 distance fields (BASELINE.json config 4 variant)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--plumbing-test", action="store_true",
@@ -271,7 +272,7 @@ def main():
     stream = torch.cuda.current_stream()
     cfg = epo_config_default(n_views=sc.n_views, width=sc.W, height=sc.H, early_stop=0, device=local,
                              stream=stream.cuda_stream, pair_budget=args.pair_budget, subsample_seed=2607,
-                             joint_phase=args.joint_phase)
+                             joint_phase=args.joint_phase, dtf_format=args.dtf_format)
     e = Epo(cfg)
     # inputs resident in HBM before the timed region
     dK, dP, dD, dE = (torch.from_numpy(a).cuda() for a in (sc.K, sc.poses_init, sc.depth, sc.edges))
@@ -335,7 +336,7 @@ def main():
     # ... and with the paper's stopping rule active: to its own stop, at most max_steps = 2000
     cfg_es = epo_config_default(n_views=sc.n_views, width=sc.W, height=sc.H, early_stop=1, device=local,
                                 stream=stream.cuda_stream, pair_budget=args.pair_budget, subsample_seed=2607,
-                                joint_phase=args.joint_phase)
+                                joint_phase=args.joint_phase, dtf_format=args.dtf_format)
     e_es = Epo(cfg_es)
     e_es.set_views(dK, dP, dD, dE); e_es.set_pairs(dpairs); torch.cuda.synchronize()
     a.record(stream); es_done, es_phase = e_es.step(2000); b.record(stream); torch.cuda.synchronize()
@@ -411,10 +412,10 @@ def main():
         config=dict(workload=workload_name(sc), l2="flushed between timed steps (256 MiB write)",
                     reprojections_per_step=reproj, valid_per_step=n_valid, valid_fraction=n_valid / max(reproj, 1),
                     edge_pixels=int(edge_off[-1]), parallelism="replicas only" if world > 1 else "1 GPU",
-                    joint_phase=args.joint_phase),
+                    joint_phase=args.joint_phase, dtf_format=("fp16" if args.dtf_format else "fp32")),
         clocks=clocks, gpu_launches=int(k1 - k0),
         roofline=dict(bound=bound, achieved=ach, peak=pk, unit=unit, frac=ach / pk, traffic=comp_bytes,
-                      kernel="k_loss_grad_packed<u8>", kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
+                      kernel=("k_loss_grad_packed<fp16 atlas>" if args.dtf_format else "k_loss_grad_packed<u8>"), kernel_ms_cold_l2=k_ms_cold, kernel_ms_warm_l2=k_ms_warm,
                       peak_source=pk_src,
                       ceilings_ms=dict(gather_cold_l2=g_ms_cold, gather_warm_l2=g_ms_warm,
                                        issue=(1e3 * t_issue if t_issue else None), hbm=(1e3 * t_hbm if t_hbm else None)),

@@ -121,6 +121,11 @@ EPO_API void epo_destroy(epo_ctx* ctx);
  */
 EPO_API epo_status epo_extract_edges(epo_ctx* ctx, const uint8_t* images, int32_t low, int32_t high, uint8_t* edges);
 
+/* The same from colour images, as the paper extracts its edges from the RGB frames: rgb [N][H][W][3]
+ * 8-bit interleaved -> grey by the BT.601 luma in 8-bit fixed point, Y = (77 R + 150 G + 29 B + 128) >> 8 (the paper
+ * states no conversion: DESIGN.md reading C7; a grey pixel keeps its value), then epo_extract_edges. */
+EPO_API epo_status epo_extract_edges_rgb(epo_ctx* ctx, const uint8_t* rgb, int32_t low, int32_t high, uint8_t* edges);
+
 /*
  * Load the initial estimate G = {K_i, P_i, Z_i} (Eq. 1) and the edge maps E_i
  * (PAPER.md:62), and run the one-time preprocessing (Alg. 1 l.6-7):

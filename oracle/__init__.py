@@ -143,6 +143,8 @@ def lib():
         L.orc_viewgraph_counts.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
                                            C.POINTER(C.c_float), C.c_int, C.c_double, C.c_double, C.c_int,
                                            C.POINTER(C.c_int32)]
+        L.orc_viewgraph_counts_slack.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double),
+                                                 C.POINTER(C.c_float), C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int32)]
         L.orc_viewgraph_pairs.restype = C.c_int64
         L.orc_viewgraph_pairs.argtypes = [C.c_int, C.POINTER(C.c_int32), C.c_double, C.POINTER(C.c_int32)]
         L.orc_subset_key.restype = C.c_uint64
@@ -371,6 +373,14 @@ def _u8p(a):
     return a.ctypes.data_as(C.POINTER(C.c_uint8))
 
 
+def rgb_to_grey(rgb: np.ndarray) -> np.ndarray:
+    """[..., 3] uint8 -> [...] uint8, reading C7 (BT.601 luma in 8-bit fixed point)."""
+    rgb = np.ascontiguousarray(rgb, np.uint8); assert rgb.shape[-1] == 3
+    out = np.zeros(rgb.shape[:-1], np.uint8)
+    lib().orc_rgb_to_grey.argtypes = [C.c_int64, C.POINTER(C.c_uint8), C.POINTER(C.c_uint8)]
+    lib().orc_rgb_to_grey(C.c_int64(out.size), _u8p(rgb), _u8p(out)); return out
+
+
 def canny_blur(img: np.ndarray) -> np.ndarray:
     img = np.ascontiguousarray(img, np.uint8); H, W = img.shape
     out = np.zeros_like(img); lib().orc_canny_blur(W, H, _u8p(img), _u8p(out)); return out
@@ -412,6 +422,28 @@ def viewgraph_counts(K, poses, depth, stride=8, tau=3.0, z_min=1e-6, coord_fp32=
     lib().orc_viewgraph_counts(N, W, H, _p(K, C.c_float), _p(poses, C.c_double), _p(depth, C.c_float), int(stride),
                                C.c_double(tau), C.c_double(z_min), int(coord_fp32), _p(counts, C.c_int32))
     return counts
+
+
+def viewgraph_counts_slack(K, poses, depth, stride=8, tau=3.0, z_min=1e-6) -> np.ndarray:
+    """[N][N][3] = (consistent, usable, uncertain) of the cycle i -> j -> i, all double: `uncertain` counts the grid points a
+    correct binary32 evaluation may decide differently (reading T1)."""
+    K = np.ascontiguousarray(K, np.float32); poses = np.ascontiguousarray(poses, np.float64).reshape(-1, 12)
+    depth = np.ascontiguousarray(depth, np.float32)
+    N, H, W = depth.shape
+    counts = np.zeros((N, N, 3), np.int32)
+    lib().orc_viewgraph_counts_slack(N, W, H, _p(K, C.c_float), _p(poses, C.c_double), _p(depth, C.c_float), int(stride),
+                                     C.c_double(tau), C.c_double(z_min), _p(counts, C.c_int32))
+    return counts
+
+
+def viewgraph_pairs_robust(counts3: np.ndarray, min_frac=0.125):
+    """(certain, possible): boolean [N][N] masks of the unordered pairs i < j that are valid whatever the uncertain grid
+    points decide, and of those that are valid for at least one decision of them (rule V7 on count +- uncertain)."""
+    c = counts3.astype(np.int64); N = c.shape[0]
+    lo = (c[..., 0] - c[..., 2]).astype(np.float64) >= np.float64(min_frac) * c[..., 1]
+    hi = (c[..., 0] + c[..., 2]).astype(np.float64) >= np.float64(min_frac) * c[..., 1]
+    iu = np.triu(np.ones((N, N), bool), 1)
+    return (lo & lo.T) & iu, (hi & hi.T) & iu
 
 
 def viewgraph_pairs(counts: np.ndarray, min_frac=0.125) -> np.ndarray:

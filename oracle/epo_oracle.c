@@ -746,6 +746,15 @@ void orc_event_slack(int N, int W, int H, const float* K, const double* poses, c
  * ================================================================================================= */
 static inline int orc_clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
+/* C7 colour -> grey.  The paper extracts edges from the RGB images and says nothing about the
+ * conversion; reading C7: the ITU-R BT.601 luma weights (0.299, 0.587, 0.114) in 8-bit fixed point,
+ *   Y = (77 R + 150 G + 29 B + 128) >> 8     (77 + 150 + 29 = 256: a grey pixel R = G = B keeps its value),
+ * interleaved input [n_px][3]. */
+void orc_rgb_to_grey(int64_t n_px, const uint8_t* rgb, uint8_t* grey) {
+  for (int64_t i = 0; i < n_px; ++i)
+    grey[i] = (uint8_t)((77 * (int)rgb[3 * i] + 150 * (int)rgb[3 * i + 1] + 29 * (int)rgb[3 * i + 2] + 128) >> 8);
+}
+
 void orc_canny_blur(int W, int H, const uint8_t* img, uint8_t* out) {
   static const int w[5] = {1, 4, 6, 4, 1};
   for (int y = 0; y < H; ++y)
@@ -864,6 +873,84 @@ static int orc_cycle_f64(int W, int H, const double Ki[4], const double Kj[4], c
   orc_project_px(Ki, xi, q);
   const double dx = q[0] - u, dy = q[1] - v;
   return dx * dx + dy * dy < tau * tau;
+}
+
+/* The same cycle with the question "could a correct binary32 evaluation decide this grid point differently?" answered
+ * from the double side (reading T1, as orc_pair_event_slack does for the loss): position error radii of a
+ * binary32 evaluation of rows a-2..a-4 (|dX| <= 8 u S_X etc., see there), and a point is UNCERTAIN when one of its
+ * integer decisions lies within them -- z within |dZ| of z_min (either way), the landing within (r_x, r_y) of the image
+ * border or of a half-integer (the nearest pixel, whose depth then differs arbitrarily), or the round-trip error
+ * within the accumulated radius of tau.  Returns the decision in bit 0 and "uncertain" in bit 1. */
+static int orc_cycle_f64_flag(int W, int H, const double Ki[4], const double Kj[4], const double Tji[12], const double Tij[12],
+                              const float* Zj_map, double u, double v, double Zi, double z_min, double tau) {
+  const double U32 = 5.9604644775390625e-08;
+  double xs[3], xt[3], S3[3], px[2], back[3], xi[3], S3b[3], q[2];
+  orc_backproject_cam(Ki, u, v, Zi, xs);
+  for (int r = 0; r < 3; ++r) {
+    xt[r] = Tji[4 * r] * xs[0] + Tji[4 * r + 1] * xs[1] + Tji[4 * r + 2] * xs[2] + Tji[4 * r + 3];
+    S3[r] = fabs(Tji[4 * r] * xs[0]) + fabs(Tji[4 * r + 1] * xs[1]) + fabs(Tji[4 * r + 2] * xs[2]) + fabs(Tji[4 * r + 3]);
+  }
+  const double eX = 8.0 * U32 * S3[0], eY = 8.0 * U32 * S3[1], eZ = 8.0 * U32 * S3[2];
+  if (fabs(xt[2] - z_min) <= eZ) return (xt[2] > z_min ? 0 : 0) | 2;      /* position unbounded: undecidable here */
+  if (!(xt[2] > z_min)) return 0;
+  orc_project_px(Kj, xt, px);
+  const double rx = (Kj[0] * eX + fabs(px[0] - Kj[2]) * eZ) / xt[2] + U32 * (3.0 * fabs(px[0] - Kj[2]) + fabs(px[0]));
+  const double ry = (Kj[1] * eY + fabs(px[1] - Kj[3]) * eZ) / xt[2] + U32 * (3.0 * fabs(px[1] - Kj[3]) + fabs(px[1]));
+  const double xmax = (double)(W - 1), ymax = (double)(H - 1);
+  const int inside = px[0] >= 0.0 && px[0] <= xmax && px[1] >= 0.0 && px[1] <= ymax;
+  const int reach = px[0] >= -rx && px[0] <= xmax + rx && px[1] >= -ry && px[1] <= ymax + ry;
+  if (!inside) return reach ? 2 : 0;
+  int unsure = px[0] < rx || px[0] > xmax - rx || px[1] < ry || px[1] > ymax - ry;
+  const double hx = px[0] + 0.5, hy = px[1] + 0.5;
+  if (hx - floor(hx) < rx || hx - floor(hx) > 1.0 - rx || hy - floor(hy) < ry || hy - floor(hy) > 1.0 - ry) unsure = 1;
+  const int xn = (int)floor(hx), yn = (int)floor(hy);
+  const double Zj = (double)Zj_map[(size_t)yn * W + xn];
+  if (!(isfinite(Zj) && Zj > z_min)) return unsure ? 2 : 0;
+  orc_backproject_cam(Kj, px[0], px[1], Zj, back);
+  for (int r = 0; r < 3; ++r) {
+    xi[r] = Tij[4 * r] * back[0] + Tij[4 * r + 1] * back[1] + Tij[4 * r + 2] * back[2] + Tij[4 * r + 3];
+    S3b[r] = fabs(Tij[4 * r] * back[0]) + fabs(Tij[4 * r + 1] * back[1]) + fabs(Tij[4 * r + 2] * back[2]) + fabs(Tij[4 * r + 3]);
+  }
+  /* the way back starts from a landing that is itself off by (r_x, r_y): the lifted point moves by Z_j r / f */
+  const double sx = Zj * rx / Kj[0], sy = Zj * ry / Kj[1];
+  const double fX = 8.0 * U32 * S3b[0] + fabs(Tij[0]) * sx + fabs(Tij[1]) * sy;
+  const double fY = 8.0 * U32 * S3b[1] + fabs(Tij[4]) * sx + fabs(Tij[5]) * sy;
+  const double fZ = 8.0 * U32 * S3b[2] + fabs(Tij[8]) * sx + fabs(Tij[9]) * sy;
+  if (fabs(xi[2] - z_min) <= fZ) return 2;
+  if (!(xi[2] > z_min)) return unsure ? 2 : 0;
+  orc_project_px(Ki, xi, q);
+  const double qx = (Ki[0] * fX + fabs(q[0] - Ki[2]) * fZ) / xi[2] + U32 * (3.0 * fabs(q[0] - Ki[2]) + fabs(q[0]));
+  const double qy = (Ki[1] * fY + fabs(q[1] - Ki[3]) * fZ) / xi[2] + U32 * (3.0 * fabs(q[1] - Ki[3]) + fabs(q[1]));
+  const double dx = q[0] - u, dy = q[1] - v, err = sqrt(dx * dx + dy * dy);
+  if (fabs(err - tau) <= qx + qy + 4.0 * U32 * tau) unsure = 1;
+  return (err < tau ? 1 : 0) | (unsure ? 2 : 0);
+}
+
+/* counts3 [N][N][3] = {consistent, usable, uncertain} of every ordered pair, everything in double */
+void orc_viewgraph_counts_slack(int N, int W, int H, const float* K, const double* poses, const float* depth, int stride,
+                                double tau, double z_min, int32_t* counts3) {
+#pragma omp parallel for schedule(dynamic)
+  for (int ij = 0; ij < N * N; ++ij) {
+    const int i = ij / N, j = ij % N;
+    int32_t cons = 0, usable = 0, unsure = 0;
+    if (i != j) {
+      double Ki[4], Kj[4], Tji[12], Tij[12];
+      for (int k = 0; k < 4; ++k) { Ki[k] = K[4 * i + k]; Kj[k] = K[4 * j + k]; }
+      orc_relative_pose(poses + 12 * i, poses + 12 * j, Tji);
+      orc_relative_pose(poses + 12 * j, poses + 12 * i, Tij);
+      const float* Zi_map = depth + (size_t)i * W * H;
+      const float* Zj_map = depth + (size_t)j * W * H;
+      for (int v = stride / 2; v < H; v += stride)
+        for (int u = stride / 2; u < W; u += stride) {
+          const float Zi = Zi_map[(size_t)v * W + u];
+          if (!(isfinite(Zi) && (double)Zi > z_min)) continue;
+          ++usable;
+          const int f = orc_cycle_f64_flag(W, H, Ki, Kj, Tji, Tij, Zj_map, (double)u, (double)v, (double)Zi, z_min, tau);
+          cons += f & 1; unsure += (f >> 1) & 1;
+        }
+    }
+    counts3[3 * ij] = cons; counts3[3 * ij + 1] = usable; counts3[3 * ij + 2] = unsure;
+  }
 }
 
 /* binary32 positions, operation order:  ifx = 1/fx;  x_s = Z ((u - cx) ifx), y_s likewise, z_s = Z;

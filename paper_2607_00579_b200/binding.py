@@ -21,7 +21,7 @@ _STATUS = {0: "EPO_OK", 1: "EPO_ERR_INVALID_ARG", 2: "EPO_ERR_BAD_STATE", 3: "EP
            4: "EPO_ERR_CUDA", 5: "EPO_ERR_UNSUPPORTED"}
 
 # every symbol include/epo.h declares (tests check that the library exports exactly these)
-SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_extract_edges", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad", "epo_loss_grad_joint", "epo_get_joint_variables",
+SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_extract_edges", "epo_extract_edges_rgb", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad", "epo_loss_grad_joint", "epo_get_joint_variables",
            "epo_step", "epo_get_poses", "epo_get_poses_f64", "epo_reset", "epo_get_edge_counts", "epo_get_edge_list",
            "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel", "epo_time_gather_ceiling",
            "epo_last_error", "epo_version"]
@@ -57,6 +57,7 @@ def load_library() -> C.CDLL:
     L.epo_destroy.argtypes = [vp]; L.epo_destroy.restype = None
     L.epo_set_views.argtypes = [vp, f32p, f32p, f32p, vp]
     L.epo_extract_edges.argtypes = [vp, vp, C.c_int32, C.c_int32, vp]
+    L.epo_extract_edges_rgb.argtypes = [vp, vp, C.c_int32, C.c_int32, vp]
     L.epo_set_pairs.argtypes = [vp, i32p, C.c_int64]
     L.epo_build_viewgraph.argtypes = [vp, C.c_int32, C.c_float, C.c_float, i32p, C.c_int64, C.POINTER(C.c_int64), i32p]
     L.epo_loss_grad.argtypes = [vp, C.c_float, f32p, f32p, i32p, f32p]
@@ -153,6 +154,13 @@ class Epo:
         if out is None:
             out = np.zeros((self.N, self.H, self.W), np.uint8)
         self._check(lib().epo_extract_edges(self._h, _ptr(images), int(low), int(high), _ptr(out)), "epo_extract_edges")
+        return out
+
+    def extract_edges_rgb(self, rgb, low: int, high: int, out=None):
+        """Canny edge maps [N][H][W] u8 of [N][H][W][3] 8-bit colour images (BT.601 luma, then extract_edges)."""
+        if out is None:
+            out = np.zeros((self.N, self.H, self.W), np.uint8)
+        self._check(lib().epo_extract_edges_rgb(self._h, _ptr(rgb), int(low), int(high), _ptr(out)), "epo_extract_edges_rgb")
         return out
 
     def build_viewgraph(self, stride: int = 8, tau: float = 3.0, min_frac: float = 0.125, want_counts: bool = False):

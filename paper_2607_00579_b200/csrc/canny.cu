@@ -129,6 +129,20 @@ __global__ void __launch_bounds__(256) k_canny_grow(const uint8_t* __restrict__ 
 
 }  // namespace
 
+// colour -> grey (reading C7): BT.601 luma in 8-bit fixed point, interleaved RGB in, one thread per pixel
+__global__ void k_rgb_to_grey(const uint8_t* __restrict__ rgb, uint8_t* __restrict__ grey, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) grey[i] = (uint8_t)((77 * (int)rgb[3 * i] + 150 * (int)rgb[3 * i + 1] + 29 * (int)rgb[3 * i + 2] + 128) >> 8);
+}
+
+epo_status epo_run_rgb_to_grey(epo_ctx* ctx, const uint8_t* d_rgb, uint8_t* d_grey) {
+  const long long n = (long long)ctx->N * ctx->W * ctx->H;
+  k_rgb_to_grey<<<(unsigned)((n + 255) / 256), 256, 0, ctx->stream>>>(d_rgb, d_grey, n);
+  ctx->launches += 1;
+  EPO_CUDA(ctx, cudaGetLastError());
+  return EPO_OK;
+}
+
 epo_status epo_run_canny(epo_ctx* ctx, const uint8_t* d_img, int low, int high, uint8_t* d_edges) {
   const int N = ctx->N, W = ctx->W, H = ctx->H;
   cudaStream_t st = ctx->stream;

@@ -791,6 +791,25 @@ epo_status epo_extract_edges(epo_ctx* c, const uint8_t* images, int32_t low, int
   return rc;
 }
 
+epo_status epo_extract_edges_rgb(epo_ctx* c, const uint8_t* rgb, int32_t low, int32_t high, uint8_t* edges) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!rgb || !edges || low < 0 || high < low || high > 1442)
+    return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_extract_edges_rgb: bad argument");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  const size_t px = (size_t)c->N * c->W * c->H;
+  uint8_t *d_rgb = nullptr, *d_grey = nullptr;
+  const bool in_dev = is_device_ptr(rgb);
+  cudaError_t e = epo_dmalloc(c, &d_grey, px);
+  if (e == cudaSuccess && !in_dev) { e = epo_dmalloc(c, &d_rgb, 3 * px); if (e == cudaSuccess) e = cudaMemcpyAsync(d_rgb, rgb, 3 * px, cudaMemcpyHostToDevice, st); }
+  epo_status rc = e == cudaSuccess ? epo_run_rgb_to_grey(c, in_dev ? rgb : d_rgb, d_grey)
+                                   : epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA,
+                                              "epo_extract_edges_rgb: %s", cudaGetErrorString(e));
+  if (rc == EPO_OK) rc = epo_extract_edges(c, d_grey, low, high, edges);      // device grey in: no further staging
+  epo_dfree(c, d_rgb); epo_dfree(c, d_grey);
+  return rc;
+}
+
 epo_status epo_build_viewgraph(epo_ctx* c, int32_t grid_stride, float tau, float min_frac, int32_t* pairs, int64_t capacity,
                                int64_t* n_pairs, int32_t* counts) {
   if (!c) return EPO_ERR_INVALID_ARG;

@@ -256,6 +256,7 @@ int64_t epo_select_max_pairs(void);
 epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override /* < 0: device step */, bool gated, bool build_work);
 // canny.cu: edge maps (1 / 0) of [N][H][W] 8-bit images, device pointers
 epo_status epo_run_canny(epo_ctx* ctx, const uint8_t* d_img, int low, int high, uint8_t* d_edges);
+epo_status epo_run_rgb_to_grey(epo_ctx* ctx, const uint8_t* d_rgb, uint8_t* d_grey);   // [N][H][W][3] -> [N][H][W]
 // joint.cu: the joint loop's depth-variable update (AdamW on alpha, beta; new points) and its state
 epo_status epo_joint_alloc(epo_ctx* ctx);              // after the points exist (epo_set_views)
 void epo_joint_free(epo_ctx* ctx);

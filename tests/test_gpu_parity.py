@@ -566,6 +566,23 @@ def test_edge_extraction_bit_exact(shape, low, high):
     e.destroy()
 
 
+def test_edge_extraction_from_rgb():
+    """epo_extract_edges_rgb (reading C7): byte-exact against the oracle's luma + Canny, host and device."""
+    import torch
+    from paper_2607_00579_b200 import Epo, epo_config_default
+    n, H, W = 3, 101, 67
+    rng = np.random.default_rng(9)
+    base = _test_images(n, H, W, seed=77).astype(np.int32)
+    rgb = np.clip(np.stack([base + rng.integers(-30, 30, base.shape), base // 2 + 40, 255 - base], axis=-1), 0, 255).astype(np.uint8)
+    e = Epo(epo_config_default(n_views=n, width=W, height=H, stream=torch.cuda.current_stream().cuda_stream))
+    ref = oracle.canny(oracle.rgb_to_grey(rgb), 10, 40)
+    assert np.array_equal(e.extract_edges_rgb(rgb, 10, 40), ref) and 0.005 < ref.mean() < 0.6
+    d_out = torch.zeros((n, H, W), dtype=torch.uint8, device="cuda")
+    e.extract_edges_rgb(torch.from_numpy(rgb).cuda(), 10, 40, out=d_out)
+    assert np.array_equal(d_out.cpu().numpy(), ref)
+    e.destroy()
+
+
 def test_edge_extraction_feeds_the_pipeline_and_rejects_bad_thresholds():
     import paper_2607_00579_b200 as pkg
     sc = scene("tiny")
@@ -587,24 +604,37 @@ def test_edge_extraction_feeds_the_pipeline_and_rejects_bad_thresholds():
 # ------------------------------------------------------------------------------ viewgraph estimation
 @pytest.mark.parametrize("name,stride", [("tiny", 4), ("room6", 8), ("orbit8", 8), ("orbit10_dense", 5)])
 def test_viewgraph_counts_and_pairs_bit_exact(name, stride):
-    """epo_build_viewgraph at the initial poses: the (consistent, usable) counts of every
-    ordered pair and the resulting directed pair list equal the oracle's binary32-position variant exactly; against
-    the all-double oracle the counts differ by a handful of borderline grid points at most."""
+    """epo_build_viewgraph at the initial poses against the ALL-DOUBLE oracle: the usable
+    counts of every ordered pair are equal, the consistent counts differ by at most the number of grid points the
+    oracle itself flags as undecidable in binary32 (reading T1), and the pair list contains every pair that
+    is valid whatever those points decide and no pair that is invalid whatever they decide.  (Diagnostic, printed: the
+    distance to the oracle's binary32-position variant.)"""
     sc = scene(name)
     e = make_ctx(sc)
     pairs, counts = e.build_viewgraph(stride=stride, tau=3.0, min_frac=0.125, want_counts=True)
     poses = sc.poses_init.astype(np.float64)
+
+    def check(pairs, counts, tau, min_frac):
+        c3 = oracle.viewgraph_counts_slack(sc.K, poses, sc.depth, stride=stride, tau=tau, z_min=Z_MIN)
+        assert np.array_equal(counts[..., 1], c3[..., 1])
+        assert np.all(np.abs(counts[..., 0] - c3[..., 0]) <= c3[..., 2])
+        certain, possible = oracle.viewgraph_pairs_robust(c3, min_frac)
+        got = np.zeros_like(certain)
+        P = np.asarray(pairs).reshape(-1, 2)
+        assert len(P) % 2 == 0 and np.array_equal(P[0::2], P[1::2][:, ::-1])          # (i, j), (j, i) for i < j, ascending
+        assert np.all(P[0::2, 0] < P[0::2, 1]) and np.all(np.diff(P[0::2, 0] * sc.n_views + P[0::2, 1]) > 0)
+        got[P[0::2, 0], P[0::2, 1]] = True
+        assert np.all(got[certain]) and not np.any(got & ~possible)
+        return c3
+
+    c3 = check(pairs, counts, 3.0, 0.125)
     ref32 = oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=3.0, z_min=Z_MIN, coord_fp32=1)
-    ref64 = oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=3.0, z_min=Z_MIN)
-    assert np.array_equal(counts, ref32)
-    assert np.array_equal(pairs, oracle.viewgraph_pairs(ref32, 0.125))
-    assert np.abs(counts - ref64).max() <= 4 and np.array_equal(counts[..., 1], ref64[..., 1])
-    print(f"{name}: {len(pairs)} directed pairs of {sc.n_views * (sc.n_views - 1)}; max count difference to the double oracle "
-          f"{np.abs(counts - ref64).max()}")
+    print(f"{name}: {len(pairs)} directed pairs of {sc.n_views * (sc.n_views - 1)}; largest count difference to the all-double oracle "
+          f"{np.abs(counts[..., 0] - c3[..., 0]).max()} (uncertain points: up to {c3[..., 2].max()} per pair, {c3[..., 2].sum()} of "
+          f"{c3[..., 1].sum()} in all) [diagnostic: to the binary32-position variant {np.abs(counts - ref32).max()}]")
     # other thresholds; a capacity that is too small is reported, not overrun
-    p2 = e.build_viewgraph(stride=stride, tau=1.0, min_frac=0.5)
-    assert np.array_equal(p2, oracle.viewgraph_pairs(
-        oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=1.0, z_min=Z_MIN, coord_fp32=1), 0.5))
+    p2, c2 = e.build_viewgraph(stride=stride, tau=1.0, min_frac=0.5, want_counts=True)
+    check(p2, c2, 1.0, 0.5)
     if len(pairs) > 2:
         import ctypes as C
         import paper_2607_00579_b200 as pkg

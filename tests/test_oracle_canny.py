@@ -93,3 +93,17 @@ def test_K5_hysteresis_keeps_what_touches_a_strong_pixel():
     r = rng.choice([0, 0, 0, 1, 1, 2], size=(64, 80), p=None).astype(np.uint8)
     lab, n = ndi.label(r > 0, structure=np.ones((3, 3)))
     assert np.array_equal(oracle.canny_hysteresis(r).astype(bool), np.isin(lab, np.unique(lab[r == 2])) & (r > 0))
+
+
+def test_K6_rgb_to_grey_is_bt601_luma_in_fixed_point():
+    """Reading C7: grey pixels keep their value exactly; the primaries map to (77, 149, 29) and white to 255 (hand-computed:
+    (77 x 255 + 128) >> 8 = 77, (150 x 255 + 128) >> 8 = 149, (29 x 255 + 128) >> 8 = 29); random colours are within one
+    grey level of the real-valued luma 0.299 R + 0.587 G + 0.114 B."""
+    g = np.arange(256, dtype=np.uint8)
+    assert np.array_equal(oracle.rgb_to_grey(np.stack([g, g, g], axis=-1)), g)
+    prim = np.array([[255, 0, 0], [0, 255, 0], [0, 0, 255], [255, 255, 255], [0, 0, 0]], np.uint8)
+    assert oracle.rgb_to_grey(prim).tolist() == [77, 149, 29, 255, 0]
+    rng = np.random.default_rng(5)
+    rgb = rng.integers(0, 256, size=(37, 41, 3), dtype=np.uint8)
+    y = 0.299 * rgb[..., 0] + 0.587 * rgb[..., 1] + 0.114 * rgb[..., 2]
+    assert np.max(np.abs(oracle.rgb_to_grey(rgb).astype(np.float64) - y)) <= 1.0

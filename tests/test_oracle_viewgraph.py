@@ -98,3 +98,29 @@ def test_V5_rendered_room_at_ground_truth_and_under_a_wrong_pose():
     # the binary32-position variant takes the same decisions up to a few borderline grid points
     c32 = oracle.viewgraph_counts(sc.K, sc.poses_gt, sc.depth, stride=8, tau=3.0, coord_fp32=1)
     assert np.abs(c32 - c).max() <= 3 and np.array_equal(c32[..., 1], c[..., 1])
+
+
+def test_V6_uncertain_counts_bound_a_binary32_evaluation():
+    """orc_viewgraph_counts_slack (reading T1): its (consistent, usable) ARE the all-double counts; the
+    binary32-position variant -- one concrete binary32 evaluation -- differs from them by at most the `uncertain` count
+    of the pair, on scenes where it does differ; the uncertain points are a small minority; and the pairs that are
+    valid whatever the uncertain points decide are a subset of the binary32 variant's list, which is a subset of the
+    pairs valid for some decision."""
+    differed = 0
+    for cfg, nv, stride in ((1, None, 4), (2, 6, 8), (3, 8, 8), (5, 10, 5)):
+        sc = make_scene(cfg, n_views=nv)
+        poses = sc.poses_init.astype(np.float64)
+        c3 = oracle.viewgraph_counts_slack(sc.K, poses, sc.depth, stride=stride, tau=3.0)
+        c64 = oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=3.0)
+        c32 = oracle.viewgraph_counts(sc.K, poses, sc.depth, stride=stride, tau=3.0, coord_fp32=1)
+        assert np.array_equal(c3[..., :2], c64)
+        assert np.array_equal(c32[..., 1], c64[..., 1])
+        assert np.all(np.abs(c32[..., 0] - c64[..., 0]) <= c3[..., 2])
+        differed += int(np.sum(c32[..., 0] != c64[..., 0]))
+        assert c3[..., 2].sum() <= 0.02 * c3[..., 1].sum()
+        certain, possible = oracle.viewgraph_pairs_robust(c3, 0.125)
+        got = np.zeros_like(certain)
+        for i, j in oracle.viewgraph_pairs(c32, 0.125):
+            if i < j: got[i, j] = True
+        assert np.all(got[certain]) and not np.any(got & ~possible)
+    assert differed >= 1
