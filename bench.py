@@ -432,7 +432,9 @@ def main():
                       ncu=dict(l1tex_pct=rec.get("l1tex_pct"), lts_pct=rec.get("lts_pct"), dram_pct=rec.get("dram_pct"),
                                l1_hit_pct=rec.get("l1_hit_pct"), l2_hit_pct=rec.get("l2_hit_pct"),
                                warp_instructions=rec.get("warp_instructions"), source=rec.get("source"))),
-        warm_l2=dict(ms_per_step=warm_ms, value=world * reproj_eff / (warm_ms / 1e3)),
+        warm_l2=dict(ms_per_step=1e3 * refine_s / max(int(done), 1), value=world * reproj_eff * max(int(done), 1) / refine_s,
+                     note=f"back to back, no L2 flush: the {int(done)} iterations of the refinement below as ONE epo_step call (one graph "
+                          f"launch); {args.steps} iterations as one call cost {warm_ms:.4f} ms each (the call's fixed cost is not amortised)"),
         refinement=dict(iters=int(done), seconds=refine_s, views=sc.n_views,
                         early_stop=dict(iters=int(es_done), seconds=es_s, phase=int(es_phase),
                                         note="one epo_step(2000) call with the pose-change rule active; stops by itself")),

@@ -37,9 +37,6 @@ constexpr int kAccStrideJoint = 16;
 #ifndef EPO_LG_MINBLOCKS
 #define EPO_LG_MINBLOCKS 7
 #endif
-#ifndef EPO_LG_L2PF
-#define EPO_LG_L2PF 2                         // passes ahead the fused kernel prefetches its points into L2 (0 = off)
-#endif
 constexpr int kLgThreads = EPO_LG_THREADS;
 constexpr int kLgPerThread = EPO_LG_PER_THREAD;
 constexpr int kLgOuter = EPO_LG_OUTER;        // most passes per work item (epo_ctx::lg_chunk is what runs)

@@ -52,6 +52,30 @@ def make_ctx(scene, device_inputs=False, **cfg_over):
     return e
 
 
+def trajectory_spread(prob, scene, iters, o64_poses, draws, cfg_kw=None, seed=7):
+    """How far apart correct evaluations of the SAME free-running loop end after `iters` iterations, measured on the oracle
+    alone (reading P7): the largest distance (degrees, scene units) from the all-double run `o64_poses` of
+      - the oracle's binary32-position variant, and
+      - `draws` all-double runs whose initial poses differ from the given ones by at most ONE ulp of binary32 per entry
+        (seeded +-1 / 0 on the bit pattern): the inputs are binary32, so this is the smallest change of the problem.
+    The loss's gradient jumps at bilinear-cell borders and Adam normalises the step, so such last-bit differences are not
+    damped but carried on; a free-running comparison cannot be asked for more than a small multiple of this spread."""
+    import oracle
+    kw = dict(early_stop=0)
+    kw.update(cfg_kw or {})
+    runs = []
+    o32 = oracle.Optimizer(prob, scene.poses_init, scene.pairs, oracle_config(coord_fp32=1, **kw))
+    o32.run(iters)
+    runs.append(pose_errors(o32.poses, o64_poses))
+    rng = np.random.default_rng(seed)
+    for _ in range(draws):
+        bits = scene.poses_init.copy().view(np.int32) + rng.integers(-1, 2, size=scene.poses_init.shape).astype(np.int32)
+        op = oracle.Optimizer(prob, bits.view(np.float32), scene.pairs, oracle_config(coord_fp32=0, **kw))
+        op.run(iters)
+        runs.append(pose_errors(op.poses, o64_poses))
+    return max(r[0] for r in runs), max(r[1] for r in runs), runs
+
+
 def oracle_eval(prob, poses, pairs, lam, z_min=Z_MIN):
     """All-double oracle evaluation plus its event slack: (ref, slack)."""
     import oracle

@@ -8,7 +8,7 @@ import pytest
 import oracle
 from epo_scenes import make_scene
 from parity_utils import (Z_MIN, check_loss_grad, fmt_lockstep, fmt_report, lockstep, make_ctx, oracle_config, oracle_eval,
-                          pose_errors)
+                          pose_errors, trajectory_spread)
 
 pytestmark = pytest.mark.gpu
 
@@ -62,20 +62,22 @@ def test_full_size_loss_gradient_and_preprocessing(config):
 @pytest.mark.parametrize("config", [2, 3, 4, 5])
 def test_full_size_free_running_prefix(config):
     """The first 25 iterations, free-running on both sides (no re-synchronisation), at full size, against the all-double
-    oracle: final poses within the contract's 1e-3 degrees / 1e-4 scene units where binary32 can meet that at all --
-    else within 3x the distance at which the oracle's own binary32-position variant ends (one-step differences of a
-    few 1e-4 degrees, see the lock-step test above, accumulate over 25 steps); the loss trace within 1e-4."""
+    oracle: final poses within the contract's 1e-3 degrees / 1e-4 scene units where correct evaluations of this loop can
+    meet that at all -- else within 3x their spread, measured on the oracle alone (parity_utils.trajectory_spread: the
+    binary32-position variant and all-double runs from initial poses moved by at most one binary32 ulp; one-step
+    differences of a few 1e-4 degrees, see the lock-step test above, are carried on over 25 steps; DESIGN.md reading P7);
+    the loss trace within 1e-4."""
     sc, e, prob = _full(config, early_stop=0)
     opt = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0))
-    o32 = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0, coord_fp32=1))
-    assert e.step(25)[0] == 25 and opt.run(25)[0] == 25 and o32.run(25)[0] == 25
+    assert e.step(25)[0] == 25 and opt.run(25)[0] == 25
     rot, tr = pose_errors(e.get_poses_f64(), opt.poses)
-    orot, otr = pose_errors(o32.poses, opt.poses)
+    srot, str_, runs = trajectory_spread(prob, sc, 25, opt.poses, draws=2)
     loss, _ = e.get_trace(0, 25)
     lrel = float(np.max(np.abs(loss - opt.loss[:25]) / opt.loss[:25]))
     print(f"config {config} full size, 25 free-running iterations vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e}, "
-          f"loss trace rel {lrel:.2e} (the oracle's own binary32-position variant: rot {orot:.2e}, trans {otr:.2e})")
-    assert rot <= max(1e-3, 3 * orot) and tr <= max(1e-4, 3 * otr)
+          f"loss trace rel {lrel:.2e}; spread of the oracle's own runs (binary32-position variant, then 2 runs from initial "
+          f"poses moved by <= 1 binary32 ulp): " + ", ".join(f"{a:.2e} / {b:.2e}" for a, b in runs))
+    assert rot <= max(1e-3, 3 * srot) and tr <= max(1e-4, 3 * str_)
     assert lrel <= 1e-4
     e.destroy()
 

@@ -6,7 +6,7 @@ import pytest
 import oracle
 from epo_scenes import SplitMix64, make_scene
 from parity_utils import (Z_MIN, check_loss_grad, fmt_lockstep, fmt_report, lockstep, make_ctx, oracle_config, oracle_eval,
-                          pose_errors)
+                          pose_errors, trajectory_spread)
 
 pytestmark = pytest.mark.gpu
 
@@ -282,12 +282,13 @@ def test_fixed_200_iterations_free_running_tiny():
 @pytest.mark.parametrize("name,iters,prefix", [("room6", 200, 25), ("orbit8", 100, 25), ("room5_294", 200, 25), ("orbit10_dense", 100, 25)])
 def test_free_running_trajectories(name, iters, prefix):
     """Free-running runs against the all-double oracle.  Asserted: after the first 25 iterations (the warm-up, while the
-    trajectories still contract) the poses agree within the contract's 1e-3 degrees / 1e-4 -- or, on scenes where the
-    oracle's own binary32-position variant is already farther than that from the all-double oracle (every one-step
-    difference of a few 1e-4 degrees accumulates), within 3x that distance.  Beyond that the runs
-    decorrelate (see parity_utils.lockstep: gradient jumps at cell borders, Adam stepping by ~lr), so the end-of-run
-    distance is a chaotic quantity: it is PRINTED next to the distance between the oracle's own two variants
-    (DESIGN.md records these numbers), and only the final loss is asserted."""
+    trajectories still contract) the poses agree within the contract's 1e-3 degrees / 1e-4 -- or, on scenes where correct
+    evaluations of this very loop end farther apart than that, within 3x their spread, measured on the oracle alone
+    (parity_utils.trajectory_spread: its binary32-position variant and all-double runs from initial poses moved by at most
+    one binary32 ulp; reading P7 records the numbers).  Beyond the prefix the runs decorrelate (see
+    parity_utils.lockstep: gradient jumps at cell borders, Adam stepping by ~lr), so the end-of-run distance is a chaotic
+    quantity: it is PRINTED next to the distance between the oracle's own two variants, and only the final loss is
+    asserted."""
     sc = scene(name)
     e = make_ctx(sc, early_stop=0)
     prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
@@ -295,12 +296,11 @@ def test_free_running_trajectories(name, iters, prefix):
     o32 = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0, coord_fp32=1))
     e.step(prefix); o64.run(prefix); o32.run(prefix)
     rot, tr = pose_errors(e.get_poses_f64(), o64.poses)
-    orot, otr = pose_errors(o32.poses, o64.poses)
-    print(f"{name}: after {prefix} free-running its vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e} "
-          f"(the oracle's own binary32-position variant: rot {orot:.2e}, trans {otr:.2e})")
-    # the contract's tolerance where binary32 can meet it at all; else no farther than a small multiple of what
-    # another binary32 evaluation of the same positions is (DESIGN.md records these distances per config)
-    assert rot <= max(1e-3, 3 * orot) and tr <= max(1e-4, 3 * otr)
+    srot, str_, runs = trajectory_spread(prob, sc, prefix, o64.poses, draws=4)
+    print(f"{name}: after {prefix} free-running its vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e}; spread of the "
+          f"oracle's own runs (binary32-position variant, then 4 runs from initial poses moved by <= 1 binary32 ulp): "
+          + ", ".join(f"{a:.2e} / {b:.2e}" for a, b in runs))
+    assert rot <= max(1e-3, 3 * srot) and tr <= max(1e-4, 3 * str_)
     rest = iters - prefix
     e.step(rest); o64.run(rest); o32.run(rest)
     d_go = pose_errors(e.get_poses_f64(), o64.poses); d_oo = pose_errors(o32.poses, o64.poses)
