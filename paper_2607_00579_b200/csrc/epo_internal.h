@@ -132,6 +132,8 @@ struct epo_ctx {
   float2* d_dz;           // [n_work][chunk / 2] a . t_ts of both samples of every slot of every work item (the fused
                           // kernel's joint output of the iteration in flight; allocated with the pair list)
   double* d_glogf;        // [N] d L / d ln f (k_finish)
+  int32_t* d_depth_stepped;  // [1] 1 once a depth step has been applied since the variables were last at the identity: until
+                          // then the packed points are the ones built from (K0, Z0) and the fused kernel rescales them
   int32_t* d_edge_off;    // [N+1]
   EdgeRec* d_edges;       // [E]
   float* d_depth;         // [N][H][W] the depth maps as given (kept for epo_build_viewgraph)

@@ -34,6 +34,7 @@ struct JointParams {
   int W, chunk;
   double beta1, beta2, adam_eps, wd;
   int force;                 // rebuild the points from the current variables without stepping (epo_joint_reset)
+  int32_t* depth_stepped;    // [1] see epo_ctx::d_depth_stepped
 };
 
 // one AdamW step of a scalar; c1 = 1 - beta1^t, c2 = 1 - beta2^t of the group's step count t; moments in fp32 (a
@@ -65,6 +66,8 @@ __device__ __forceinline__ double2 gather_dz(const float2* __restrict__ dz, cons
   return make_double2(ga, gb);
 }
 
+constexpr int kJointPairsSmem = 512;   // pairs per source view whose weights k_joint_points keeps in shared memory
+
 __global__ void k_joint_points(const JointParams q) {
   const int view = blockIdx.y;
   const int slots = (q.pk_off[view + 1] - q.pk_off[view]) / 2;
@@ -79,9 +82,30 @@ __global__ void k_joint_points(const JointParams q) {
   const double c1 = depth_on ? 1.0 - pow(q.beta1, (double)t) : 1.0, c2 = depth_on ? 1.0 - pow(q.beta2, (double)t) : 1.0;
   const float ifx = 1.0f / __ldcg(q.K + 4 * view), ify = 1.0f / __ldcg(q.K + 4 * view + 1);
   const float cx = __ldcg(q.K + 4 * view + 2), cy = __ldcg(q.K + 4 * view + 3);
-  // until phase 1 is reached no depth step has happened: alpha = 1, beta = 0 everywhere and Z = Z0 exactly -- the
-  // 32 bytes per edge pixel of (alpha, beta) need not be read to rescale the points for the new focal lengths
-  const bool identity = q.state->phase == 0 && !depth_on;
+  // until the first depth step alpha = 1, beta = 0 everywhere and Z = Z0 exactly: the stored points are the ones built
+  // from (K0, Z0), and the focal step is a per-camera scaling of x_s and y_s that the fused kernel folds into the first
+  // two columns of R_ts (lossgrad.cu) -- nothing to rewrite, this launch returns.  From the first depth step on the
+  // points are rebuilt here in every iteration.
+  const bool identity = __ldcg(q.depth_stepped) == 0 && !depth_on;
+  if (identity && !q.force) return;
+  if (depth_on && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) *q.depth_stepped = 1;
+  // the pairs this view is the source of, once per CTA: weight 1 / (P n_p) (0: not in this iteration's subset, or no
+  // valid sample) and first work item -- the per-pixel sums below then issue independent loads only (the same terms
+  // in the same ascending order as gather_dz: identical results)
+  __shared__ double s_w[kJointPairsSmem];
+  __shared__ int s_wo[kJointPairsSmem];
+  const int k0 = q.src_off[view], np = q.src_off[view + 1] - k0;
+  const bool pairs_in_smem = depth_on && np <= kJointPairsSmem;
+  if (pairs_in_smem) {
+    for (int i = threadIdx.x; i < np; i += blockDim.x) {
+      const int p = q.src_inc[k0 + i];
+      const int n = __ldcg(q.pair_valid + p);
+      const bool skip = (q.sel_flag != nullptr && q.sel_flag[p] == 0) || n <= 0;
+      s_w[i] = skip ? 0.0 : q.inv_P / (double)n;
+      s_wo[i] = q.work_off[p];
+    }
+    __syncthreads();
+  }
   for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < slots; j += gridDim.x * blockDim.x) {
     const size_t sl = base + j, o = sl / kLgThreads * (3 * kLgThreads) + sl % kLgThreads;
     const int2 px = q.pix[sl];
@@ -89,7 +113,20 @@ __global__ void k_joint_points(const JointParams q) {
     double4 ab = identity ? make_double4(1.0, 0.0, 1.0, 0.0) : q.ab[sl];
     if (depth_on) {
       const float2 zc = q.xyz[o + 2 * kLgThreads];  // the depth the loss of this iteration was evaluated at
-      const double2 g = gather_dz(q.dz, q.pair_valid, q.src_off, q.src_inc, q.work_off, q.sel_flag, view, j, q.chunk, q.inv_P);
+      double2 g;
+      if (pairs_in_smem) {
+        const int half = q.chunk / 2, it = j / half, so = j % half;
+        double ga = 0.0, gb = 0.0;
+        for (int i = 0; i < np; ++i) {
+          const double w = s_w[i];
+          if (w == 0.0) continue;
+          const float2 v = __ldcg(q.dz + (size_t)(s_wo[i] + it) * half + so);
+          ga += w * (double)v.x; gb += w * (double)v.y;
+        }
+        g = make_double2(ga, gb);
+      } else {
+        g = gather_dz(q.dz, q.pair_valid, q.src_off, q.src_inc, q.work_off, q.sel_flag, view, j, q.chunk, q.inv_P);
+      }
       float4 ma = q.abm[2 * sl], mb = q.abm[2 * sl + 1];
       if (px.x >= 0) {
         const double gz = -g.x / (double)zc.x;
@@ -181,7 +218,7 @@ JointParams make_params(epo_ctx* c, bool subset) {
   q.inv_P = 1.0 / (double)(subset ? (int64_t)c->cfg.pair_budget : (c->P > 0 ? c->P : 1));
   q.W = c->W; q.chunk = c->lg_chunk;
   q.beta1 = c->cfg.beta1; q.beta2 = c->cfg.beta2; q.adam_eps = c->cfg.adam_eps; q.wd = c->cfg.weight_decay;
-  q.force = 0;
+  q.force = 0; q.depth_stepped = c->d_depth_stepped;
   return q;
 }
 
@@ -189,8 +226,8 @@ JointParams make_params(epo_ctx* c, bool subset) {
 
 void epo_joint_free(epo_ctx* c) {
   epo_dfree(c, c->d_K0); epo_dfree(c, c->d_gamma); epo_dfree(c, c->d_ab); epo_dfree(c, c->d_abm);
-  epo_dfree(c, c->d_z0); epo_dfree(c, c->d_glogf);
-  c->d_K0 = nullptr; c->d_gamma = nullptr; c->d_ab = nullptr; c->d_abm = nullptr; c->d_z0 = nullptr; c->d_glogf = nullptr;
+  epo_dfree(c, c->d_z0); epo_dfree(c, c->d_glogf); epo_dfree(c, c->d_depth_stepped);
+  c->d_depth_stepped = nullptr; c->d_K0 = nullptr; c->d_gamma = nullptr; c->d_ab = nullptr; c->d_abm = nullptr; c->d_z0 = nullptr; c->d_glogf = nullptr;
 }
 
 // d_glogf exists in every context (epo_loss_grad_joint works without cfg.joint_phase); the variables only with it
@@ -204,6 +241,8 @@ epo_status epo_joint_alloc(epo_ctx* c) {
     if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_ab, S * sizeof(double4));
     if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_abm, 2 * S * sizeof(float4));
     if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_z0, S * sizeof(float2));
+    if (e == cudaSuccess) e = epo_dmalloc(c, &c->d_depth_stepped, sizeof(int32_t));
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->d_depth_stepped, 0, sizeof(int32_t), c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_K0, c->d_K, N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d_gamma, 0, 3 * N * sizeof(double), c->stream);
     if (e == cudaSuccess && n_slots(c) > 0) {
@@ -225,6 +264,7 @@ epo_status epo_joint_reset(epo_ctx* c) {
   if (!c->cfg.joint_phase || !c->d_gamma) return EPO_OK;
   EPO_CUDA(c, cudaMemsetAsync(c->d_gamma, 0, 3 * (size_t)c->N * sizeof(double), c->stream));
   EPO_CUDA(c, cudaMemcpyAsync(c->d_K, c->d_K0, (size_t)c->N * 4 * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+  EPO_CUDA(c, cudaMemsetAsync(c->d_depth_stepped, 0, sizeof(int32_t), c->stream));
   if (n_slots(c) > 0) {
     k_joint_init<<<(unsigned)((n_slots(c) + 255) / 256), 256, 0, c->stream>>>(c->packed.xyz, c->d_z0, c->d_ab, c->d_abm,
                                                                                (long long)n_slots(c), 0);
