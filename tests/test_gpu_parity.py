@@ -503,6 +503,46 @@ def test_joint_loop_with_pair_subsampling_matches_the_oracle():
     _joint_lockstep(scene("room6"), kw, dict(early_stop=0, w1=6, eps1=float(np.float32(5.0))), 20, 3)
 
 
+def test_joint_variables_survive_a_new_pair_list():
+    """epo_set_pairs restarts the optimiser (phase 0 again) but keeps poses and joint variables: the iterations that
+    follow must evaluate the loss at the KEPT depths and focal lengths.  (Before the first depth step the library leaves
+    the stored points alone and folds the focal step into R_ts; after a depth step it rebuilds them every iteration --
+    which regime holds is a device flag that epo_set_pairs does not clear.)  Checked against the all-double oracle
+    evaluated at the library's own state, before and after the new list and one more iteration."""
+    import copy
+    sc = scene("room6")
+    e = make_ctx(sc, early_stop=0, joint_phase=1, w1=6, eps1=5.0)
+    prob0 = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
+    N = sc.n_views
+    view = np.repeat(np.arange(N), np.diff(prob0.edge_off)); uu = prob0.uv[:, 0].astype(int); vv = prob0.uv[:, 1].astype(int)
+
+    def oracle_loss_at_library_state(lam):
+        gamma, amap, bmap = e.get_joint_variables()
+        prob = copy.copy(prob0)
+        prob.K = prob0.K.copy()
+        prob.K[:, 0] = (prob0.K[:, 0].astype(np.float64) * (1.0 + gamma)).astype(np.float32)
+        prob.K[:, 1] = (prob0.K[:, 1].astype(np.float64) * (1.0 + gamma)).astype(np.float32)
+        prob.z = (prob0.z.astype(np.float64) * amap[view, vv, uu] + bmap[view, vv, uu]).astype(np.float32)
+        return oracle_eval(prob, e.get_poses_f64(), sc.pairs, lam), amap[view, vv, uu]
+
+    done, phase = e.step(16)
+    assert done == 16 and phase >= 1
+    (ref, sl), alpha = oracle_loss_at_library_state(10.0)
+    assert np.abs(alpha - 1.0).max() > 1e-4                          # depth steps have happened
+    got = e.loss_grad(10.0)
+    assert abs(got["loss"] - ref["loss"]) <= 1e-5 * abs(ref["loss"]) + float(np.mean(sl["pair_loss"]))
+    e.set_pairs(sc.pairs)                                            # phase 0 again, variables kept
+    assert np.array_equal(e.get_joint_variables()[1][view, vv, uu], alpha)
+    got = e.loss_grad(10.0)
+    assert abs(got["loss"] - ref["loss"]) <= 1e-5 * abs(ref["loss"]) + float(np.mean(sl["pair_loss"]))
+    assert e.step(2)[0] == 2                                         # two iterations in phase 0: gamma steps, depths stay
+    (ref2, sl2), alpha2 = oracle_loss_at_library_state(10.0)
+    assert np.array_equal(alpha2, alpha)
+    got2 = e.loss_grad(10.0)
+    assert abs(got2["loss"] - ref2["loss"]) <= 1e-5 * abs(ref2["loss"]) + float(np.mean(sl2["pair_loss"]))
+    e.destroy()
+
+
 def test_joint_loop_is_bit_reproducible():
     """No atomics anywhere in the joint phase: two runs give identical poses and variables, bit for bit."""
     sc = scene("orbit8")
