@@ -87,6 +87,30 @@ def test_Z1_gradient_matches_central_finite_differences(tiny_scene, tiny_problem
     assert np.linalg.norm(fd - g) <= 5e-5 * np.linalg.norm(g)
 
 
+def test_Z1_binary32_position_variant_against_finite_differences(tiny_scene, tiny_problem):
+    """The oracle's binary32-position variant (a printed diagnostic of the GPU tests, reading P1) has every
+    entry of its gradient pinned too: central finite differences of ITS OWN loss.  With positions rounded to binary32 the
+    loss is a staircase at the 1e-4 px scale, so the step is larger (h = 1e-5) and the tolerance looser (5e-3 per camera,
+    1e-3 of the largest entry per entry; observed 1.3e-3 and 6e-4) -- a dropped term, a wrong sign or a transposed
+    operand is an O(1) error."""
+    s = tiny_scene
+    poses = s.poses_init.astype(np.float64)
+    g = oracle.loss_grad(tiny_problem, poses, s.pairs, 10.0, coord_fp32=1)["grad"]
+    h = 1e-5
+    fd = np.zeros_like(g)
+    for c in range(s.n_views):
+        for k in range(6):
+            Pp = poses.copy(); Pm = poses.copy()
+            Pp[c] = _exp_left(poses[c], k, +h); Pm[c] = _exp_left(poses[c], k, -h)
+            op = oracle.loss_grad(tiny_problem, Pp, s.pairs, 10.0, coord_fp32=1)
+            om = oracle.loss_grad(tiny_problem, Pm, s.pairs, 10.0, coord_fp32=1)
+            assert np.array_equal(op["pair_valid"], om["pair_valid"])
+            fd[c, k] = (op["loss"] - om["loss"]) / (2 * h)
+    for c in range(s.n_views):
+        assert np.linalg.norm(fd[c] - g[c]) <= 5e-3 * np.linalg.norm(g[c]), (c, fd[c], g[c])
+    assert np.abs(fd - g).max() <= 1e-3 * np.abs(g).max()
+
+
 # ------------------------------------------------------------------------------------------------ Z2
 def _raycast_room(K, T12, x, y):
     """Analytic z-depth of the room seen through the SUB-PIXEL position (x, y) (independent of the oracle)."""
