@@ -14,7 +14,13 @@
 namespace {
 
 constexpr double kPi = 3.14159265358979323846;
-constexpr int kFinThreads = 256;
+// k_finish: 512 threads (16 warps share a camera's incident pairs) at two CTAs per SM (<= 64 registers); measured against
+// 256 / 1024 threads and 1..6 CTAs per SM: the time between two fused kernels falls from 74 to 49 us at config 4 and from
+// 62 to 44 us at config 5
+#ifndef EPO_FIN_THREADS
+#define EPO_FIN_THREADS 512
+#endif
+constexpr int kFinThreads = EPO_FIN_THREADS;
 
 struct FinParams {
   // a-9 inputs: pair lists and the fused kernel's per-CTA partial sums
@@ -151,8 +157,11 @@ __device__ bool converged_loss(const double* trace, double loss_s, int s, int w,
   return __syncthreads_and(ok) != 0;
 }
 
+#ifndef EPO_FIN_MINBLOCKS
+#define EPO_FIN_MINBLOCKS 2
+#endif
 template <bool kJoint>
-__global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
+__global__ void __launch_bounds__(kFinThreads, EPO_FIN_MINBLOCKS) k_finish(const FinParams p) {
   // partial records: 8 values x 4 chunk classes per warp round, or (joint phase) 16 slots x 2 classes
   constexpr int kVal = kJoint ? kAccStrideJoint : kAccStride, kCls = 32 / kVal;
   DevState* st = p.state;
@@ -170,16 +179,17 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   const int t0 = p.tgt_off[c], nt = p.tgt_off[c + 1] - t0, s0 = p.src_off[c], n_inc = nt + p.src_off[c + 1] - s0;
   int G = (n_inc + kWarps - 1) / kWarps;
   G = G < 1 ? 1 : (G > 32 ? 32 : G);
-  auto fetch = [&](int j0, int* q, int* w0, int* w1) {
+  auto fetch = [&](int j0, int* q, int* w0, int* w1, int* tv) {
     const int j = j0 + lane;
-    *q = -1; *w0 = 0; *w1 = 0;
+    *q = -1; *w0 = 0; *w1 = 0; *tv = 0;
     if (lane < G && j < n_inc) {
       *q = j < nt ? t0 + j : p.src_inc[s0 + j - nt];
       *w0 = p.work_off[*q]; *w1 = p.work_off[*q + 1];
+      *tv = p.pairs[*q].y;                           // the pair's target view (needed when c is its source)
     }
   };
-  int j0 = warp * G, q, w0, w1;
-  fetch(j0, &q, &w0, &w1);
+  int j0 = warp * G, q, w0, w1, tv;
+  fetch(j0, &q, &w0, &w1, &tv);
   cudaTriggerProgrammaticLaunchCompletion();       // the next fused kernel may start its own static prologue
   cudaGridDependencySynchronize();                 // partial sums, poses and the control block are final now
   if (p.gated && st->halt) {
@@ -195,14 +205,15 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
   double acc = 0.0;
   while (j0 < n_inc) {
     unsigned todo = __ballot_sync(0xffffffffu, q >= 0 && (p.sel_flag == nullptr || p.sel_flag[q] != 0));
-    const int jc = j0, qm = q, w0m = w0, w1m = w1;
+    const int jc = j0, qm = q, w0m = w0, w1m = w1, tvm = tv;
     j0 += kWarps * G;
-    if (j0 < n_inc) fetch(j0, &q, &w0, &w1);       // the next group's ranges, in flight
+    if (j0 < n_inc) fetch(j0, &q, &w0, &w1, &tv);  // the next group's ranges, in flight
     while (todo) {
       const int b = __ffs(todo) - 1;
       todo &= todo - 1;
       const int qc = __shfl_sync(0xffffffffu, qm, b);
       const int wa = __shfl_sync(0xffffffffu, w0m, b), wb = __shfl_sync(0xffffffffu, w1m, b);
+      const int tview = __shfl_sync(0xffffffffu, tvm, b);
       const bool tgt = jc + b < nt;
       // per-pair sums: lane l adds value (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... (independent loads), then
       // the four chunk classes are combined by two xor-shuffles: a fixed order
@@ -224,7 +235,7 @@ __global__ void __launch_bounds__(kFinThreads) k_finish(const FinParams p) {
         const double A0 = __shfl_sync(0xffffffffu, v, 2), A1 = __shfl_sync(0xffffffffu, v, 3), A2 = __shfl_sync(0xffffffffu, v, 4);
         double m0 = __shfl_sync(0xffffffffu, v, 5), m1 = __shfl_sync(0xffffffffu, v, 6), m2 = __shfl_sync(0xffffffffu, v, 7);
         if (lane >= 2 && lane < 8 && n > 0.0) {
-          const double* Pt = p.poses + 12 * (size_t)p.pairs[qc].y;
+          const double* Pt = p.poses + 12 * (size_t)tview;
           const int i = (lane - 2) % 3;
           const double r0 = rel_pose_entry(Pc, Pt, i), r1 = rel_pose_entry(Pc, Pt, 4 + i), r2 = rel_pose_entry(Pc, Pt, 8 + i);
           if (lane < 5) {
