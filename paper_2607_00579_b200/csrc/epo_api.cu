@@ -609,9 +609,17 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
     // kernels these iterations run if no rule stops them (what the host loop would have launched)
     c->launches += 1 + (int64_t)in_graph * (2 + (c->subsample ? 1 : 0) + (c->cfg.joint_phase ? 1 : 0));
     for (int i = in_graph; i < n_iters; ++i) EPO_TRY(enqueue_iteration(c, 0));
+  } else if (n_iters == 0) {
+    EPO_TRY(epo_launch_begin_step_call(c, 0));
   } else {
-    EPO_TRY(epo_launch_begin_step_call(c, n_iters));
-    for (int i = 0; i < n_iters; ++i) EPO_TRY(enqueue_iteration(c, 0));
+    // no k_begin_step_call: the first iteration's kernels gate on DevState.stopped and its k_finish opens the call
+    // (iters_done, budget, halt); one launch less per call, which is what a step-by-step caller pays per iteration
+    for (int i = 0; i < n_iters; ++i) {
+      c->first_budget = i == 0 ? n_iters : 0;
+      const epo_status rc = enqueue_iteration(c, 0);
+      c->first_budget = 0;
+      if (rc != EPO_OK) return rc;
+    }
   }
   bool sync = false;
   if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));

@@ -114,6 +114,8 @@ struct epo_ctx {
   cudaGraphNode_t step_begin_node;
   cudaGraphConditionalHandle step_cond;
   bool static_dirty;   // work list / points / fields were (re)built since the last fused launch: launch it serialised
+  int first_budget;    // > 0 while epo_step enqueues the FIRST iteration of a call that has no k_begin_step_call in front
+                       // of it: its kernels gate on DevState.stopped and k_finish opens the call (iters_done, budget)
   int64_t P, E, n_work, reproj_per_eval, launches;
   int lg_chunk;        // samples per work item of the fused kernel (a multiple of kLgPass), chosen in epo_set_pairs
 

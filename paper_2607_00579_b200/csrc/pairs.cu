@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(kSelThreads, 1) k_select_pairs(const SelParams
   for (int i = tid; i < kSelBins; i += kSelThreads) hist[i] = 0;
   cudaTriggerProgrammaticLaunchCompletion();
   cudaGridDependencySynchronize();
-  if (p.gated && p.state->halt) return;
+  if (p.gated && (p.gated == 2 ? p.state->stopped : p.state->halt)) return;
   const int step = p.step_override >= 0 ? p.step_override : p.state->step;
   unsigned long long key[kSelUnroll];
 #pragma unroll
@@ -370,7 +370,7 @@ epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override, bool gated, 
   p.perm = ctx->d_perm; p.work_off = ctx->d_work_off; p.state = ctx->d_state; p.flag = ctx->d_sel_flag;
   p.sel_work = build_work ? ctx->d_sel_work : nullptr; p.info = ctx->d_sel_info; p.scratch = ctx->d_sel_scratch;
   p.seed = ctx->cfg.subsample_seed;
-  p.P = (int)ctx->P; p.M = ctx->cfg.pair_budget; p.step_override = step_override; p.gated = gated ? 1 : 0;
+  p.P = (int)ctx->P; p.M = ctx->cfg.pair_budget; p.step_override = step_override; p.gated = gated ? (ctx->first_budget > 0 ? 2 : 1) : 0;
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)((ctx->P + kSelChunk - 1) / kSelChunk));   // <= kSelMaxCtas, checked in epo_set_pairs
   lc.blockDim = dim3(kSelThreads); lc.dynamicSmemBytes = 0; lc.stream = ctx->stream;

@@ -46,7 +46,9 @@ struct FinParams {
   const double* sched;          // [max_steps][4] {lr_s, 1 - beta1^(s+1), 1 - beta2^(s+1), lambda_s}
   int max_steps, w1, w2, smooth, early_stop, stop_rule, w_loss;
   double eps_loss;
-  int gated, step_mode;
+  int gated, step_mode;      // gated: 1 = by DevState.halt; 2 = first iteration of a call without k_begin_step_call: by
+                             // DevState.stopped, and this launch opens the call (iters_done = 0, budget = call_budget)
+  int call_budget;
   cudaGraphConditionalHandle cond;   // the loop graph's WHILE condition (0 outside the graph)
 };
 
@@ -192,9 +194,11 @@ __global__ void __launch_bounds__(kFinThreads, EPO_FIN_MINBLOCKS) k_finish(const
   fetch(j0, &q, &w0, &w1, &tv);
   cudaTriggerProgrammaticLaunchCompletion();       // the next fused kernel may start its own static prologue
   cudaGridDependencySynchronize();                 // partial sums, poses and the control block are final now
-  if (p.gated && st->halt) {
+  const bool first = p.gated == 2;
+  if (p.gated && (first ? st->stopped : st->halt)) {
     if (blockIdx.x == 0 && threadIdx.x == 0) {
       st->joint_pending = 0;
+      if (first) { st->iters_done = 0; st->budget = p.call_budget; st->halt = 1; }
       if (p.cond) cudaGraphSetConditional(p.cond, 0);
     }
     return;
@@ -385,10 +389,11 @@ __global__ void __launch_bounds__(kFinThreads, EPO_FIN_MINBLOCKS) k_finish(const
     st->phase_prev = phase0; st->joint_pending = 1;
     if (phase0 == 0 && phase == 1) st->phase1_step = s;
     st->step = s + 1;
-    const int done = st->iters_done + 1;
+    const int done = (first ? 0 : st->iters_done) + 1;
+    const int budget = first ? p.call_budget : st->budget;
     const int stopped = (s + 1 >= p.max_steps) || (p.early_stop && phase == 2);
-    const int halt = stopped || done >= st->budget;
-    st->iters_done = done; st->stopped = stopped; st->halt = halt;
+    const int halt = stopped || done >= budget;
+    st->iters_done = done; st->budget = budget; st->stopped = stopped; st->halt = halt;
     // the loop graph runs its body again only while the call may go on: nothing is launched after the stop
     if (p.cond) cudaGraphSetConditional(p.cond, (stopped || done >= st->graph_limit) ? 0u : 1u);
     st->ticket = 0;
@@ -444,7 +449,7 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool subs
   p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.max_steps = ctx->cfg.max_steps;
   p.w1 = ctx->cfg.w1; p.w2 = ctx->cfg.w2; p.smooth = ctx->cfg.smooth_window; p.early_stop = ctx->cfg.early_stop;
   p.stop_rule = ctx->cfg.stop_rule; p.w_loss = ctx->cfg.w_loss; p.eps_loss = ctx->cfg.eps_loss;
-  p.gated = gated ? 1 : 0; p.step_mode = step_mode ? 1 : 0; p.cond = cond;
+  p.gated = gated ? (ctx->first_budget > 0 ? 2 : 1) : 0; p.call_budget = ctx->first_budget; p.step_mode = step_mode ? 1 : 0; p.cond = cond;
   const size_t smem = (size_t)2 * ctx->N * sizeof(double);   // the last CTA's copy of dR, dt
   if (smem > 200 * 1024) return epo_fail(ctx, EPO_ERR_UNSUPPORTED, "more than %d views", 200 * 1024 / 16);
   if (smem > 48 * 1024) {
