@@ -81,21 +81,55 @@ void free_pairs(epo_ctx* c) {
   c->have_pairs = false; c->P = 0; c->n_work = 0;
 }
 
-// Samples per work item (= per CTA) of the fused kernel, a multiple of kLgPass.  Every CTA pays a fixed price
-// (scheduling, the pose prologue, the block reduction: measured ~1.4 ns of GPU time each at config 3), so items are
-// made as long as possible -- up to kLgOuter passes -- while the grid still has about two waves of CTAs to
-// balance the SMs.  EPO_LG_PASSES in the environment overrides the choice (tuning).
+// Samples per work item (= per CTA) of the fused kernel, a multiple of kLgPass, chosen per problem by simulating the
+// launch.  EPO_LG_PASSES in the environment overrides the choice (tuning).
 int choose_chunk(const epo_ctx* c, const std::vector<int32_t>& pairs, int64_t P) {
-  int64_t samples = 0;
-  for (int64_t k = 0; k < P; ++k) samples += c->h_edge_off[pairs[2 * k] + 1] - c->h_edge_off[pairs[2 * k]];
   int sms = 148;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->cfg.device);
   const int64_t slots = (int64_t)sms * EPO_LG_MINBLOCKS;
-  int64_t passes = samples / (2 * slots * kLgPass);
-  if (passes < 4) passes = 4;
-  if (passes > kLgOuter) passes = kLgOuter;
-  if (const char* v = std::getenv("EPO_LG_PASSES")) { int k = std::atoi(v); if (k >= 1 && k <= kLgMaxOuter) passes = k; }
-  return (int)passes * kLgPass;
+  // passes of every pair; for the simulation below in the order the CTAs are dispatched (canonical: by target, then source)
+  std::vector<std::pair<int64_t, int32_t>> order((size_t)P);
+  int64_t total_passes = 0;
+  for (int64_t k = 0; k < P; ++k) {
+    const int32_t s = pairs[2 * k], t = pairs[2 * k + 1];
+    order[(size_t)k] = {((int64_t)t << 32) | (uint32_t)s, (c->h_edge_off[s + 1] - c->h_edge_off[s] + kLgPass - 1) / kLgPass};
+    total_passes += order[(size_t)k].second;
+  }
+  // The launch as the block scheduler runs it: items in list order, each to the slot that frees first; an item of p
+  // passes holds its slot for t_f + p t_p (measured on B200: 2.1 us of launch gap, prologue and reduction, 0.62 us per
+  // pass at full residency).  Short items pay t_f too often, long ones quantise the last wave: take the
+  // item length with the shortest simulated launch.  Time in units of t_p / 5 (t_f = 17 units), so that the slots' free
+  // times are integers and a calendar of counters replaces a priority queue; with eight or more full waves at the
+  // longest item the quantisation is immaterial and the longest item wins without a simulation.
+  int best = kLgMaxOuter;
+  if (total_passes < slots * kLgMaxOuter * 8) {
+    std::sort(order.begin(), order.end());
+    constexpr int kTf = 17, kTp = 5;
+    int64_t best_t = INT64_MAX;
+    std::vector<int32_t> cal;
+    for (int maxp = 4; maxp <= kLgMaxOuter; maxp += (maxp < 24 ? 1 : 4)) {
+      const int64_t horizon = (total_passes * kTp + (total_passes / maxp + P) * kTf) / slots + 2 * (kTf + kLgMaxOuter * kTp) + 2;
+      cal.assign((size_t)horizon + kTf + kLgMaxOuter * kTp + 2, 0);
+      cal[0] = (int32_t)slots;
+      int64_t cur = 0, end = 0;
+      auto run_item = [&](int passes) {
+        while (cal[(size_t)cur] == 0) ++cur;
+        --cal[(size_t)cur];
+        const int64_t t = cur + kTf + (int64_t)passes * kTp;
+        if ((size_t)t >= cal.size()) cal.resize((size_t)t + 64, 0);
+        ++cal[(size_t)t];
+        if (t > end) end = t;
+      };
+      for (const auto& o : order) {
+        int left = o.second;
+        for (; left > maxp; left -= maxp) run_item(maxp);
+        if (left > 0) run_item(left);
+      }
+      if (end * 200 < best_t * 199) { best_t = end; best = maxp; }     // near-ties: the shorter item
+    }
+  }
+  if (const char* v = std::getenv("EPO_LG_PASSES")) { int k = std::atoi(v); if (k >= 1 && k <= kLgMaxOuter) best = k; }
+  return best * kLgPass;
 }
 
 void destroy_step_graph(epo_ctx* c) {
