@@ -241,11 +241,14 @@ EPO_API epo_status epo_get_work(epo_ctx* ctx, int64_t* reprojections_per_eval, i
 EPO_API epo_status epo_time_loss_grad_kernel(epo_ctx* ctx, float lambda, int32_t reps, int32_t flush_l2,
                                              float* ms_mean, float* ms_min);
 
-/* Measurement hook (bench.py "roofline.gather"): the same launches with the fused kernel's MEMORY SIDE only -- the
- * point stream, the projected positions, validity and the 2x2 gather of every valid sample (the real tap index
- * stream), the samples merely summed; no robust loss, no Jacobian.  Its duration is the kernel's gather roofline on
- * this workload (north_star).  It overwrites the per-CTA partial sums; the next evaluation recomputes
- * them. */
+/* Measurement hook (bench.py "roofline", the gather ceiling; SURVEY.md 8(d) micro-benchmarks g1 / g2, north_star): the
+ * fused kernel's tap stream replayed with NOTHING else.  One launch of the kernel's `record` instantiation writes the
+ * texel coordinates of every sample's 2x2 footprint (4 bytes per sample; not valid: a marker) to a scratch buffer; the
+ * timed launches then run the same grid (one CTA per work item, same passes and lanes), read those 4 bytes and issue
+ * one four-texel gather per valid sample from the same atlas, summing the codes in integers -- no position arithmetic,
+ * no square-root table, no loss.  Their duration is what the L1TEX / L2 path needs for this workload's gathers.
+ * Arguments and results as for epo_time_loss_grad_kernel.  Allocates and frees its scratch; does not touch the
+ * context's state. */
 EPO_API epo_status epo_time_gather_ceiling(epo_ctx* ctx, float lambda, int32_t reps, int32_t flush_l2,
                                            float* ms_mean, float* ms_min);
 
