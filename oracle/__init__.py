@@ -22,13 +22,17 @@ _lib = None
 
 
 def build(force: bool = False) -> str:
-    """Compile epo_oracle.c with gcc (-O2, no fast-math, no FMA contraction, OpenMP over pairs)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + ".%d.tmp" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
-                               "-o", tmp, _SRC, "-lm"])
-        os.replace(tmp, _LIB)
-    return _LIB
+    """Compile epo_oracle.c with gcc (-O2, no fast-math, no FMA contraction, OpenMP over pairs).
+    EPO_ORACLE_SANITIZE=1 builds and loads an AddressSanitizer + UndefinedBehaviorSanitizer instance instead
+    (liboracle_san.so; run python with LD_PRELOAD=$(gcc -print-file-name=libasan.so): profiles/r2_sanitizer.md)."""
+    san = os.environ.get("EPO_ORACLE_SANITIZE", "") not in ("", "0")
+    lib = os.path.join(_HERE, "liboracle_san.so") if san else _LIB
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(_SRC):
+        tmp = lib + ".%d.tmp" % os.getpid()
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if san else ["-O2"]
+        subprocess.check_call(["gcc"] + flags + ["-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, lib)
+    return lib
 
 
 class _Cfg(C.Structure):
@@ -77,8 +81,7 @@ def _p(a, t):
 def lib():
     global _lib
     if _lib is None:
-        build()
-        L = C.CDLL(_LIB)
+        L = C.CDLL(build())
         L.orc_lambda.restype = C.c_double
         L.orc_lambda.argtypes = [C.c_int, C.c_double, C.c_double, C.c_int]
         L.orc_lr.restype = C.c_double
