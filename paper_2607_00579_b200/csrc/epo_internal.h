@@ -199,6 +199,16 @@ __device__ __forceinline__ double rel_pose_entry(const double* Ts, const double*
 }
 #endif
 
+// ---- bounds checks of the hot kernels' indices (compute-sanitizer is closed on the GPU pool, profiles/r2_sanitizer.md):
+// a library built with -DEPO_DEBUG_BOUNDS=1 asserts every index below against the size of what it indexes; a failed
+// assert traps the kernel and the next API call returns EPO_ERR_CUDA.  Off (and free) in the product build.
+#if defined(EPO_DEBUG_BOUNDS) && EPO_DEBUG_BOUNDS
+#include <cassert>
+#define EPO_CHECK(cond) assert(cond)
+#else
+#define EPO_CHECK(cond) ((void)0)
+#endif
+
 // ---- error plumbing ---------------------------------------------------------------------------
 epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...);
 

@@ -35,6 +35,7 @@ struct JointParams {
   double beta1, beta2, adam_eps, wd;
   int force;                 // rebuild the points from the current variables without stepping (epo_joint_reset)
   int32_t* depth_stepped;    // [1] see epo_ctx::d_depth_stepped
+  long long n_slots, n_work; // sizes EPO_CHECK tests indices against
 };
 
 // one AdamW step of a scalar; c1 = 1 - beta1^t, c2 = 1 - beta2^t of the group's step count t; moments in fp32 (a
@@ -108,6 +109,7 @@ __global__ void k_joint_points(const JointParams q) {
   }
   for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < slots; j += gridDim.x * blockDim.x) {
     const size_t sl = base + j, o = sl / kLgThreads * (3 * kLgThreads) + sl % kLgThreads;
+    EPO_CHECK((long long)sl < q.n_slots);
     const int2 px = q.pix[sl];
     const float2 Z0 = q.z0[sl];
     double4 ab = identity ? make_double4(1.0, 0.0, 1.0, 0.0) : q.ab[sl];
@@ -120,6 +122,7 @@ __global__ void k_joint_points(const JointParams q) {
         for (int i = 0; i < np; ++i) {
           const double w = s_w[i];
           if (w == 0.0) continue;
+          EPO_CHECK(s_wo[i] + it < q.n_work);
           const float2 v = __ldcg(q.dz + (size_t)(s_wo[i] + it) * half + so);
           ga += w * (double)v.x; gb += w * (double)v.y;
         }
@@ -218,7 +221,7 @@ JointParams make_params(epo_ctx* c, bool subset) {
   q.inv_P = 1.0 / (double)(subset ? (int64_t)c->cfg.pair_budget : (c->P > 0 ? c->P : 1));
   q.W = c->W; q.chunk = c->lg_chunk;
   q.beta1 = c->cfg.beta1; q.beta2 = c->cfg.beta2; q.adam_eps = c->cfg.adam_eps; q.wd = c->cfg.weight_decay;
-  q.force = 0; q.depth_stepped = c->d_depth_stepped;
+  q.force = 0; q.depth_stepped = c->d_depth_stepped; q.n_slots = (long long)n_slots(c); q.n_work = (long long)c->n_work;
   return q;
 }
 

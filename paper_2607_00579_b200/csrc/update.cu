@@ -41,7 +41,7 @@ struct FinParams {
   double *m, *v, *dR, *dt, *theta, *loss_trace;
   DevState* state;
   int N;
-  int64_t P;
+  int64_t P, n_pairs, n_work;   // P: pairs the mean runs over; n_pairs, n_work: list sizes (EPO_CHECK)
   double beta1, beta2, adam_eps, eps1, eps2;
   const double* sched;          // [max_steps][4] {lr_s, 1 - beta1^(s+1), 1 - beta2^(s+1), lambda_s}
   int max_steps, w1, w2, smooth, early_stop, stop_rule, w_loss;
@@ -219,6 +219,7 @@ __global__ void __launch_bounds__(kFinThreads, EPO_FIN_MINBLOCKS) k_finish(const
       const int wa = __shfl_sync(0xffffffffu, w0m, b), wb = __shfl_sync(0xffffffffu, w1m, b);
       const int tview = __shfl_sync(0xffffffffu, tvm, b);
       const bool tgt = jc + b < nt;
+      EPO_CHECK(qc >= 0 && qc < p.n_pairs && wa >= 0 && wa <= wb && wb <= p.n_work && tview >= 0 && tview < N);
       // per-pair sums: lane l adds value (l & 7) of chunks (l >> 3), (l >> 3) + 4, ... (independent loads), then
       // the four chunk classes are combined by two xor-shuffles: a fixed order
       double v = 0.0;
@@ -443,7 +444,7 @@ epo_status epo_launch_finish(epo_ctx* ctx, bool step_mode, bool gated, bool subs
   p.grad = ctx->d_grad; p.loss_part = ctx->d_loss_part;
   p.poses = ctx->d_poses; p.poses_next = ctx->d_poses_next; p.m = ctx->d_m; p.v = ctx->d_v;
   p.dR = ctx->d_dR; p.dt = ctx->d_dt; p.theta = ctx->d_theta; p.loss_trace = ctx->d_loss_trace;
-  p.state = ctx->d_state; p.N = ctx->N;
+  p.state = ctx->d_state; p.N = ctx->N; p.n_pairs = ctx->P; p.n_work = ctx->n_work;
   p.P = subset ? (int64_t)ctx->cfg.pair_budget : ctx->P;     // the mean runs over the pairs that were evaluated
   p.sched = ctx->d_sched; p.beta1 = ctx->cfg.beta1; p.beta2 = ctx->cfg.beta2; p.adam_eps = ctx->cfg.adam_eps;
   p.eps1 = ctx->cfg.eps1; p.eps2 = ctx->cfg.eps2; p.max_steps = ctx->cfg.max_steps;
