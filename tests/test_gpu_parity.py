@@ -503,6 +503,32 @@ def test_joint_loop_with_pair_subsampling_matches_the_oracle():
     _joint_lockstep(scene("room6"), kw, dict(early_stop=0, w1=6, eps1=float(np.float32(5.0))), 20, 3)
 
 
+def test_item_length_changes_only_the_summation_order(monkeypatch):
+    """The fused kernel's work items (`choose_chunk`: 4 .. 32 passes of 256 samples, picked by simulating the launch) cut
+    a pair's sample list at different places: valid counts must be identical and losses / gradients equal up to fp32
+    summation order, whatever the item length (EPO_LG_PASSES overrides the choice; ragged last items at every length)."""
+    sc = scene("orbit8")
+    ref = None
+    for passes in ("4", "7", "16", "32", None):
+        if passes is None:
+            monkeypatch.delenv("EPO_LG_PASSES", raising=False)
+        else:
+            monkeypatch.setenv("EPO_LG_PASSES", passes)
+        e = make_ctx(sc, early_stop=0)
+        got = e.loss_grad(10.0)
+        e.step(3)
+        poses = e.get_poses_f64()
+        e.destroy()
+        if ref is None:
+            ref = (got, poses)
+            continue
+        assert np.array_equal(got["pair_valid"], ref[0]["pair_valid"])
+        assert np.allclose(got["pair_loss"], ref[0]["pair_loss"], rtol=2e-6, atol=0)
+        gn = np.linalg.norm(ref[0]["grad"], axis=1)
+        assert np.all(np.linalg.norm(got["grad"] - ref[0]["grad"], axis=1) <= 2e-6 * gn)
+        assert np.allclose(poses, ref[1], rtol=0, atol=1e-7)
+
+
 def test_joint_variables_survive_a_new_pair_list():
     """epo_set_pairs restarts the optimiser (phase 0 again) but keeps poses and joint variables: the iterations that
     follow must evaluate the loss at the KEPT depths and focal lengths.  (Before the first depth step the library leaves
