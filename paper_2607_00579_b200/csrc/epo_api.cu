@@ -96,7 +96,7 @@ int choose_chunk(const epo_ctx* c, const std::vector<int32_t>& pairs, int64_t P)
     total_passes += order[(size_t)k].second;
   }
   // The launch as the block scheduler runs it: items in list order, each to the slot that frees first; an item of p
-  // passes holds its slot for t_f + p t_p (measured on B200: 2.1 us of launch gap, prologue and reduction, 0.62 us per
+  // passes holds its slot for t_f + p t_p (measured on B200: 2.1 us of drain, prologue and pipeline refill, 0.62 us per
   // pass at full residency).  Short items pay t_f too often, long ones quantise the last wave: take the
   // item length with the shortest simulated launch.  Time in units of t_p / 5 (t_f = 17 units), so that the slots' free
   // times are integers and a calendar of counters replaces a priority queue; with eight or more full waves at the
