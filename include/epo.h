@@ -252,6 +252,39 @@ EPO_API epo_status epo_time_loss_grad_kernel(epo_ctx* ctx, float lambda, int32_t
 EPO_API epo_status epo_time_gather_ceiling(epo_ctx* ctx, float lambda, int32_t reps, int32_t flush_l2,
                                            float* ms_mean, float* ms_min);
 
+/*
+ * Distance transform of ONE edge map without any device-memory allocation (the a-P2 / a-P3 kernels of epo_set_views:
+ * PAPER.md:378-379 Alg. 1 l.7, "exact L2 distance transform"; result bit-identical to epo_get_dtf's fp32 field).
+ *
+ * Who needs it.  epo_set_views takes its work buffers from a memory pool, i.e. it allocates.  Two kinds of caller cannot
+ * accept that: (1) a process whose HBM is already owned by its own allocator -- an inference server or a training job
+ * that reserved everything at start-up -- where a cudaMalloc from a library either fails or steals the block the host
+ * program was about to ask for; (2) a loop with a per-frame deadline, because cudaMalloc and cudaFree synchronise the
+ * device.  This call needs no context and allocates nothing, ever: its only work buffer (the row pass's
+ * int32 [height][width]) is an array compiled into libepo.so, EPO_EDT_NO_ALLOC_MAX_PIXELS entries = 2 MiB, that every
+ * GPU which loads the library carries until the process exits.
+ *
+ *   d_edges  [height][width] u8, DEVICE pointer, non-zero = edge          (input, caller-owned, read only)
+ *   d_dtf    [height][width] fp32, DEVICE pointer: distance in pixels to the nearest edge pixel, width + height
+ *            everywhere if there is none                                   (output, caller-owned, fully overwritten)
+ *   stream   cudaStream_t of the CURRENT device (NULL = legacy default stream); the two kernels are enqueued on it and the
+ *            call returns without synchronising -- d_dtf is ready when that stream reaches this point
+ *   err      nullable, err_len bytes: receives a NUL-terminated description when the result is not EPO_OK
+ * Runs on the calling thread's current device (it never switches devices); both pointers must belong to it.
+ * Limits.  width * height <= EPO_EDT_NO_ALLOC_MAX_PIXELS (the paper's 518 x 392 frames use 39 % of it); anything larger is
+ * refused with EPO_ERR_UNSUPPORTED and nothing is launched.  2 <= width, height <= 65535 as for epo_create.
+ * First call on each device: looks up that device's address of the built-in array (and, as for any CUDA library, the
+ * driver loads the kernels then).  Make that first call during start-up, before the stream is ever put into capture mode;
+ * later calls only launch.
+ * Sharing.  There is one array per GPU, shared by every call, thread and stream of the process, and it still holds the
+ * previous call's row distances.  Nothing has to be cleared (each call overwrites the part it reads before reading it),
+ * but two calls that can run at the same time on one GPU -- different streams, or different threads -- overwrite each
+ * other's rows and both results are garbage: put them on one stream or order them with events.
+ */
+#define EPO_EDT_NO_ALLOC_MAX_PIXELS (512 * 1024)
+EPO_API epo_status epo_edt_no_alloc(const uint8_t* d_edges, int32_t width, int32_t height, float* d_dtf, void* stream,
+                                    char* err, int32_t err_len);
+
 EPO_API const char* epo_last_error(const epo_ctx* ctx);
 EPO_API const char* epo_version(void);
 

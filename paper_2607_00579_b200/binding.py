@@ -24,7 +24,7 @@ _STATUS = {0: "EPO_OK", 1: "EPO_ERR_INVALID_ARG", 2: "EPO_ERR_BAD_STATE", 3: "EP
 SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_extract_edges", "epo_extract_edges_rgb", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad", "epo_loss_grad_joint", "epo_get_joint_variables",
            "epo_step", "epo_get_poses", "epo_get_poses_f64", "epo_reset", "epo_get_edge_counts", "epo_get_edge_list",
            "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel", "epo_time_gather_ceiling",
-           "epo_last_error", "epo_version"]
+           "epo_edt_no_alloc", "epo_last_error", "epo_version"]
 
 
 class EpoConfig(C.Structure):
@@ -76,6 +76,7 @@ def load_library() -> C.CDLL:
     L.epo_get_work.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.epo_time_loss_grad_kernel.argtypes = [vp, C.c_float, C.c_int32, C.c_int32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.epo_time_gather_ceiling.argtypes = L.epo_time_loss_grad_kernel.argtypes
+    L.epo_edt_no_alloc.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, C.c_char_p, C.c_int32]
     L.epo_last_error.argtypes = [vp]; L.epo_last_error.restype = C.c_char_p
     L.epo_version.argtypes = []; L.epo_version.restype = C.c_char_p
     return L
@@ -114,6 +115,22 @@ def epo_config_default(**overrides) -> EpoConfig:
     for k, v in overrides.items():
         setattr(cfg, k, v)
     return cfg
+
+
+EDT_NO_ALLOC_MAX_PIXELS = 512 * 1024     # EPO_EDT_NO_ALLOC_MAX_PIXELS of include/epo.h
+
+
+def edt_no_alloc(edges, dtf, stream: int = 0):
+    """epo_edt_no_alloc: distance field of one [H][W] u8 edge map into the [H][W] fp32 tensor `dtf`, both CUDA tensors of
+    the current device that the CALLER allocated -- this call takes no device memory of its own (see include/epo.h for
+    who needs that, the 512 Ki-pixel limit and the rule that overlapping calls on one GPU race).  `stream` is a raw
+    cudaStream_t (0 = default stream); the call does not synchronise."""
+    H, W = int(edges.shape[0]), int(edges.shape[1])
+    assert tuple(dtf.shape) == (H, W), (tuple(dtf.shape), (H, W))
+    buf = C.create_string_buffer(256)
+    st = lib().epo_edt_no_alloc(_ptr(edges, np.uint8), W, H, _ptr(dtf, np.float32), stream, buf, len(buf))
+    if st != EPO_OK:
+        raise EpoError(st, "epo_edt_no_alloc", buf.value.decode())
 
 
 class Epo:

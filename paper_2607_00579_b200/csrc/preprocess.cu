@@ -3,9 +3,11 @@
 //   PAPER.md:374-376 (Alg. 1 l.6)  "Canny edges, sub-sampled to <= E_max points / image"
 //   PAPER.md:378-379 (Alg. 1 l.7), 396  "exact L2 distance transform [14]" kept on the GPU
 #include <climits>
+#include <cstdarg>
 #include <cstring>
 
 #include <algorithm>
+#include <mutex>
 
 #include "epo_internal.h"
 
@@ -540,4 +542,123 @@ epo_status epo_build_points(epo_ctx* ctx, const float* d_K, const int32_t* d_off
   epo_dfree(ctx, pts);                               // stream-ordered: after the packing kernel
   if (rc == EPO_OK) *out = pk;
   return rc;
+}
+
+// =============================================================================================
+// epo_edt_no_alloc (include/epo.h): the distance transform of ONE edge map for callers that must not allocate.
+//
+// The ordinary path (epo_set_views -> epo_build_dtf_atlas above) takes its row-pass buffer g[H][W] from the context's
+// memory pool.  Some programs cannot let a library do that: a serving or training process that has already given all of
+// HBM to its own caching allocator (a cudaMalloc made behind its back fails, or succeeds and later makes ITS next
+// allocation fail), and a per-frame loop with a latency budget, where cudaMalloc / cudaFree stall the whole device.
+// For them the row-pass buffer lives in the library image instead: a file-scope __device__ array, present on every GPU
+// that loads libepo.so from the moment the module is loaded until the process exits.  The entry point below makes no
+// cudaMalloc / cudaFree / pool / array / texture / surface / event call, in its first call or in any later one.
+//
+// k_edt_cols_linear is k_edt_cols with a plain row-major fp32 output instead of the surface stores into the atlas, and
+// without the staged strip (no opt-in shared memory): same outward integer search, same square root, so the field is
+// bit-identical to epo_get_dtf's.
+// =============================================================================================
+namespace {
+
+// the scratch: EPO_EDT_NO_ALLOC_MAX_PIXELS int32 = 2 MiB per GPU
+static __device__ __align__(256) int32_t g_edt_na_scratch[EPO_EDT_NO_ALLOC_MAX_PIXELS];
+
+// In host code `g_edt_na_scratch` is only the host-side shadow of the symbol, not an address the GPU can use: the real
+// address differs per device and comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr int kNaMaxDevices = 64;
+std::mutex g_edt_na_mu;
+int32_t* g_edt_na_ptr[kNaMaxDevices] = {};
+
+template <typename I>
+__global__ void __launch_bounds__(kEdtStrip * kEdtWarps)
+k_edt_cols_linear(const int32_t* __restrict__ g, int W, int H, float* __restrict__ dtf) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int x = blockIdx.x * kEdtStrip + lane;
+  const bool in = x < W;
+  const int32_t* gv = g + (in ? x : W - 1);
+  auto G = [&](int y) -> I { return (I)__ldg(gv + (size_t)y * W); };
+  for (int y = blockIdx.y * kEdtWarps + warp; y < H; y += gridDim.y * kEdtWarps) {
+    const I g0 = G(y);
+    I best = g0 * g0;
+    const int dmax = max(y, H - 1 - y);
+    for (int dy = 1; dy <= dmax; ++dy) {
+      const I dd = (I)dy * dy;
+      if (dd >= best) break;
+      const I a = G(max(y - dy, 0)), b = G(min(y + dy, H - 1));
+      const I m = a < b ? a : b;
+      const I c = m * m + dd;
+      best = c < best ? c : best;
+    }
+    if (in) dtf[(size_t)y * W + x] = (best < (I)(1 << 24)) ? __fsqrt_rn((float)best) : (float)sqrt((double)best);
+  }
+}
+
+epo_status na_fail(char* err, int32_t err_len, epo_status st, const char* fmt, ...) {
+  if (err && err_len > 0) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(err, (size_t)err_len, fmt, ap);
+    va_end(ap);
+  }
+  return st;
+}
+
+bool na_on_device(const void* p, int dev) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return (a.type == cudaMemoryTypeDevice && a.device == dev) || a.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+extern "C" epo_status epo_edt_no_alloc(const uint8_t* d_edges, int32_t width, int32_t height, float* d_dtf, void* stream,
+                                       char* err, int32_t err_len) {
+  if (err && err_len > 0) err[0] = 0;
+  if (!d_edges || !d_dtf) return na_fail(err, err_len, EPO_ERR_INVALID_ARG, "epo_edt_no_alloc: d_edges and d_dtf are required");
+  if (width < 2 || height < 2 || width > 65535 || height > 65535)
+    return na_fail(err, err_len, EPO_ERR_INVALID_ARG, "epo_edt_no_alloc: need 2 <= width, height <= 65535 (got %d x %d)", width, height);
+  const int64_t px = (int64_t)width * height;
+  if (px > (int64_t)EPO_EDT_NO_ALLOC_MAX_PIXELS)
+    return na_fail(err, err_len, EPO_ERR_UNSUPPORTED,
+                   "epo_edt_no_alloc: %d x %d = %lld pixels exceed the built-in scratch of %d pixels "
+                   "(EPO_EDT_NO_ALLOC_MAX_PIXELS); use epo_set_views / epo_get_dtf, which allocate",
+                   width, height, (long long)px, (int)EPO_EDT_NO_ALLOC_MAX_PIXELS);
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return na_fail(err, err_len, EPO_ERR_CUDA, "epo_edt_no_alloc: cudaGetDevice: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kNaMaxDevices)
+    return na_fail(err, err_len, EPO_ERR_UNSUPPORTED, "epo_edt_no_alloc: device ordinal %d (at most %d devices)", dev, kNaMaxDevices);
+  if (!na_on_device(d_edges, dev) || !na_on_device(d_dtf, dev))
+    return na_fail(err, err_len, EPO_ERR_INVALID_ARG, "epo_edt_no_alloc: d_edges and d_dtf must be device pointers of the current device (%d)", dev);
+
+  // set-up, once per device and with that device current (it is: `dev` is what cudaGetDevice just returned)
+  int32_t* scratch = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_edt_na_mu);
+    if (!g_edt_na_ptr[dev]) {
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_edt_na_scratch);
+      if (e != cudaSuccess || !p)
+        return na_fail(err, err_len, EPO_ERR_CUDA, "epo_edt_no_alloc: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+      g_edt_na_ptr[dev] = static_cast<int32_t*>(p);
+    }
+    scratch = g_edt_na_ptr[dev];
+  }
+
+  // Nothing in the scratch has to start at zero: the row pass writes all width x height entries before the column pass
+  // reads any of them (same stream), and entries beyond them -- left by an earlier, larger call -- are never read.
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const int grid_rows = (height + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  k_edt_rows<<<grid_rows, kWarpsPerBlock * 32, 0, st>>>(d_edges, (int64_t)height, width, width + height, scratch);
+  const bool wide = (int64_t)(width + height) * (width + height) + (int64_t)height * height >= (int64_t)INT32_MAX / 2;
+  const int strips = (width + kEdtStrip - 1) / kEdtStrip;
+  int bands = (height + kEdtWarps - 1) / kEdtWarps;          // row bands per strip: enough CTAs to fill the machine
+  if (bands > 65535) bands = 65535;
+  const dim3 grid((unsigned)strips, (unsigned)bands);
+  if (wide) k_edt_cols_linear<long long><<<grid, kEdtStrip * kEdtWarps, 0, st>>>(scratch, width, height, d_dtf);
+  else      k_edt_cols_linear<int><<<grid, kEdtStrip * kEdtWarps, 0, st>>>(scratch, width, height, d_dtf);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return na_fail(err, err_len, EPO_ERR_CUDA, "epo_edt_no_alloc: launch: %s", cudaGetErrorString(e));
+  return EPO_OK;
 }
