@@ -154,6 +154,8 @@ EPO_API epo_status epo_set_views(epo_ctx* ctx, const float* K, const float* pose
  *             EPO_ERR_INVALID_ARG after setting it, and writes no pairs.
  *   counts    [N][N][2] out, nullable: (consistent, usable) of the cycle i -> j -> i (0, 0 on the diagonal).
  * Synchronises the stream.  Does not change the context (call epo_set_pairs with the result).
+ * Depth: always the maps Z0 given to epo_set_views.  With cfg.joint_phase = 1 the refined depth (Z0 alpha + beta) exists
+ * only at the listed edge pixels, not on the dense grid this test samples, so it is NOT used here; the current poses are.
  */
 EPO_API epo_status epo_build_viewgraph(epo_ctx* ctx, int32_t grid_stride, float tau, float min_frac, int32_t* pairs,
                                        int64_t capacity, int64_t* n_pairs, int32_t* counts);
@@ -165,6 +167,11 @@ EPO_API epo_status epo_build_viewgraph(epo_ctx* ctx, int32_t grid_stride, float 
  * work list of the fused kernel.  Resets the optimiser (Adam / AdamW moments, step counter, phase and traces)
  * and nothing else: the CURRENT poses (and joint variables) stay, so a viewgraph re-estimated from refined poses
  * can be installed without losing them.  epo_reset rewinds to the initial poses.
+ * Synchronises the stream even when `pairs` is a DEVICE pointer (the exception to the rule at the top of this file): the
+ * list is copied to the host, validated there, and the work-item length of the fused kernel is chosen on the host.
+ * With cfg.pair_budget > 0 the list may hold at most 524,288 pairs (128 CTAs x 4096 pairs of the selection kernel, which
+ * must all be resident at once); a longer list is refused with EPO_ERR_UNSUPPORTED.  Without sub-sampling the only limit
+ * is memory.
  */
 EPO_API epo_status epo_set_pairs(epo_ctx* ctx, const int32_t* pairs, int64_t n_pairs);
 

@@ -263,6 +263,7 @@ epo_status epo_create(const epo_config* cfg, epo_ctx** out) {
   if (const char* v = std::getenv("EPO_GRAPH_UNROLL")) { const int k = std::atoi(v); if (k >= 1 && k <= 64) c->graph_unroll = k; }
   c->capture_stream = nullptr; c->step_graph = nullptr; c->step_exec = nullptr; c->step_begin_node = nullptr; c->step_cond = 0;
   { const char* v = std::getenv("EPO_NO_PDL"); c->pdl = !(v && v[0] && v[0] != '0'); }
+  { const char* v = std::getenv("EPO_NO_COOP"); c->coop_select = !(v && v[0] && v[0] != '0'); }
   c->static_dirty = true;
   cudaError_t e = cudaSetDevice(cfg->device);
   const size_t N = (size_t)c->N;
@@ -655,6 +656,11 @@ epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* p
       if (rc != EPO_OK) return rc;
     }
   }
+  // joint loop: the iterations just enqueued rewrite K (k_finish) and the packed points (k_joint_points, which signals
+  // programmatic completion at its top).  A fused launch that reads them BEFORE its dependency wait -- every non-joint
+  // one, e.g. the next epo_loss_grad -- must therefore not overlap them: keep it serialised.  Joint fused launches read
+  // after the wait and ignore the flag.
+  if (c->cfg.joint_phase && n_iters > 0) c->static_dirty = true;
   bool sync = false;
   if (iters_done) EPO_CUDA(c, copy_out(iters_done, &c->d_state->iters_done, sizeof(int32_t), st, &sync));
   if (phase) EPO_CUDA(c, copy_out(phase, &c->d_state->phase, sizeof(int32_t), st, &sync));
@@ -930,6 +936,13 @@ static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flu
   if (!c) return EPO_ERR_INVALID_ARG;
   if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_time_loss_grad_kernel before set_views/set_pairs");
   if (reps < 1 || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_time_loss_grad_kernel: bad argument");
+  if (gather_only) {
+    // the recorded taps are 16-bit atlas coordinates (x | y << 16, all ones = "not valid"): refuse atlases they cannot hold
+    const int64_t aw = (int64_t)c->atlas.cols * c->W, ah = (int64_t)((c->N + c->atlas.cols - 1) / c->atlas.cols) * c->H;
+    if (aw > 65535 || ah > 65535)
+      return epo_fail(c, EPO_ERR_UNSUPPORTED, "epo_time_gather_ceiling: atlas of %lld x %lld texels exceeds the 16-bit tap record",
+                      (long long)aw, (long long)ah);
+  }
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
   const size_t flush_bytes = (size_t)256 << 20;   // > 126 MB L2

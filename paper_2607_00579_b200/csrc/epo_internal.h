@@ -113,6 +113,7 @@ struct epo_ctx {
   cudaGraphExec_t step_exec;
   cudaGraphNode_t step_begin_node;
   cudaGraphConditionalHandle step_cond;
+  bool coop_select;    // k_select_pairs with more than one CTA is launched cooperatively (EPO_NO_COOP=1 turns it off)
   bool static_dirty;   // work list / points / fields were (re)built since the last fused launch: launch it serialised
   int first_budget;    // > 0 while epo_step enqueues the FIRST iteration of a call that has no k_begin_step_call in front
                        // of it: its kernels gate on DevState.stopped and k_finish opens the call (iters_done, budget)

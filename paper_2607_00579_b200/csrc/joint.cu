@@ -95,7 +95,9 @@ __global__ void k_joint_points(const JointParams q) {
   // in the same ascending order as gather_dz: identical results)
   __shared__ double s_w[kJointPairsSmem];
   __shared__ int s_wo[kJointPairsSmem];
-  const int k0 = q.src_off[view], np = q.src_off[view + 1] - k0;
+  // (the pair tables are read only when the depth steps: a forced rebuild may run before any pair list exists, with
+  // src_off == nullptr -- epo_set_views -> epo_reset)
+  const int k0 = depth_on ? q.src_off[view] : 0, np = depth_on ? q.src_off[view + 1] - k0 : 0;
   const bool pairs_in_smem = depth_on && np <= kJointPairsSmem;
   if (pairs_in_smem) {
     for (int i = threadIdx.x; i < np; i += blockDim.x) {

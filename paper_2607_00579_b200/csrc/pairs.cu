@@ -374,11 +374,17 @@ epo_status epo_launch_select_pairs(epo_ctx* ctx, int step_override, bool gated, 
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)((ctx->P + kSelChunk - 1) / kSelChunk));   // <= kSelMaxCtas, checked in epo_set_pairs
   lc.blockDim = dim3(kSelThreads); lc.dynamicSmemBytes = 0; lc.stream = ctx->stream;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchAttribute at[2];
+  int na = 0;
   // programmatic dependent launch only inside the loop and only when the static lists are not the work of the
   // kernels just before this one (the same rule as for the fused kernel)
-  lc.attrs = at; lc.numAttrs = (ctx->pdl && gated && !ctx->static_dirty) ? 1 : 0;
+  if (ctx->pdl && gated && !ctx->static_dirty) {
+    at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization; at[na].val.programmaticStreamSerializationAllowed = 1; ++na;
+  }
+  // more than one CTA: they meet at grid_barrier, so the launch is a COOPERATIVE one -- the runtime then checks that the
+  // whole grid can be resident at once (cudaErrorCooperativeLaunchTooLarge otherwise) instead of this code assuming it
+  if (lc.gridDim.x > 1 && ctx->coop_select) { at[na].id = cudaLaunchAttributeCooperative; at[na].val.cooperative = 1; ++na; }
+  lc.attrs = at; lc.numAttrs = na;
   EPO_CUDA(ctx, cudaLaunchKernelEx(&lc, k_select_pairs, p));
   ctx->launches += 1;
   return EPO_OK;

@@ -584,6 +584,57 @@ def test_joint_loop_is_bit_reproducible():
     assert np.abs(out[0][2] - 1.0).max() > 0                       # depth steps did happen
 
 
+def test_joint_step_without_host_sync_then_loss_grad():
+    """epo_step with NULL iters_done / phase does not synchronise; the epo_loss_grad that follows is a NON-joint fused
+    launch and must still see the K and the points the last iteration wrote (k_finish, k_joint_points), not a stale or
+    half-written copy: same bits as after a synchronised run.  Device outputs, so that the call itself adds no sync."""
+    import torch
+    sc = scene("room6")
+    kw = dict(early_stop=0, joint_phase=1, w1=6, eps1=5.0)
+    ref = None
+    for sync in (True, False, False, False):
+        e = make_ctx(sc, **kw)
+        loss = torch.zeros(1, device="cuda"); pl = torch.zeros(e.P, device="cuda")
+        pv = torch.zeros(e.P, dtype=torch.int32, device="cuda"); g = torch.zeros((e.N, 6), device="cuda")
+        if sync:
+            assert e.step(19)[0] == 19
+            torch.cuda.synchronize()
+        else:
+            e.step(19, sync=False)                                   # 16 iterations in the loop graph + 3 enqueued one by one
+        e.loss_grad_into(8.0, loss, pl, pv, g)
+        torch.cuda.synchronize()
+        got = (loss.cpu().numpy(), pl.cpu().numpy(), pv.cpu().numpy(), g.cpu().numpy())
+        assert np.abs(e.get_joint_variables()[1] - 1.0).max() > 0    # the depth did step: the points were being rewritten
+        e.destroy()
+        if ref is None:
+            ref = got
+        for a, b in zip(ref, got):
+            assert np.array_equal(a, b)
+
+
+def test_joint_reset_before_any_pair_list():
+    """epo_set_views -> epo_reset -> epo_set_pairs with joint_phase = 1: the reset rebuilds the points from (K0, Z0) with
+    no pair table in existence; it must not touch one.  The context then behaves like a fresh one."""
+    from paper_2607_00579_b200 import Epo, epo_config_default
+    import torch
+    sc = scene("room6")
+    cfg = epo_config_default(n_views=sc.n_views, width=sc.W, height=sc.H, stream=torch.cuda.current_stream().cuda_stream,
+                             early_stop=0, joint_phase=1)
+    e = Epo(cfg)
+    e.set_views(sc.K, sc.poses_init, sc.depth, sc.edges)
+    e.reset()
+    e.reset(sc.poses_init)
+    torch.cuda.synchronize()                                         # a faulting kernel would surface here
+    e.set_pairs(sc.pairs)
+    got = e.loss_grad(10.0)
+    f = make_ctx(sc, early_stop=0, joint_phase=1)
+    want = f.loss_grad(10.0)
+    assert got["loss"] == want["loss"] and np.array_equal(got["grad"], want["grad"]) and np.array_equal(got["pair_valid"], want["pair_valid"])
+    assert e.step(5)[0] == 5 and f.step(5)[0] == 5
+    assert np.array_equal(e.get_poses_f64(), f.get_poses_f64())
+    e.destroy(); f.destroy()
+
+
 # ---------------------------------------------------------------------------------- edge extraction
 def _test_images(n, H, W, seed):
     """Seeded 8-bit images with edges of every orientation and strength: rectangles and discs of random grey levels
