@@ -12,7 +12,7 @@ they can move (`oracle.event_slack`, pinned by tests/test_oracle_slack.py), and 
     | gpu - oracle | <= contract tolerance x | oracle | + slack(oracle)
 with the slack reported next to the observed error; for a camera's gradient "| oracle |" is the larger of its norm
 and the root-sum-square of its per-sample terms (T2: at a minimum the terms cancel and the norm alone is no scale).  The oracle's binary32-position variant (`coord_fp32=1`) is a
-diagnostic only: it is printed, never asserted.
+diagnostic only: it is printed, never asserted, and it takes part in no bound.
 """
 import math
 
@@ -53,20 +53,17 @@ def make_ctx(scene, device_inputs=False, **cfg_over):
 
 
 def trajectory_spread(prob, scene, iters, o64_poses, draws, cfg_kw=None, seed=7):
-    """How far apart correct evaluations of the SAME free-running loop end after `iters` iterations, measured on the oracle
-    alone (reading P7): the largest distance (degrees, scene units) from the all-double run `o64_poses` of
-      - the oracle's binary32-position variant, and
-      - `draws` all-double runs whose initial poses differ from the given ones by at most ONE ulp of binary32 per entry
-        (seeded +-1 / 0 on the bit pattern): the inputs are binary32, so this is the smallest change of the problem.
+    """How far apart correct evaluations of the SAME free-running loop end after `iters` iterations, measured on the
+    all-double oracle alone (reading P7): the distances (degrees, scene units) from the all-double run
+    `o64_poses` of `draws` all-double runs whose initial poses differ from the given ones by at most ONE ulp of binary32
+    per entry (seeded +-1 / 0 on the bit pattern): the inputs are binary32, so this is the smallest change of the problem.
     The loss's gradient jumps at bilinear-cell borders and Adam normalises the step, so such last-bit differences are not
-    damped but carried on; a free-running comparison cannot be asked for more than a small multiple of this spread."""
+    damped but carried on.  Returns (farthest rotation, farthest translation, all draws).  No kernel-shaped code takes part:
+    the oracle's binary32-position variant is not run here."""
     import oracle
     kw = dict(early_stop=0)
     kw.update(cfg_kw or {})
     runs = []
-    o32 = oracle.Optimizer(prob, scene.poses_init, scene.pairs, oracle_config(coord_fp32=1, **kw))
-    o32.run(iters)
-    runs.append(pose_errors(o32.poses, o64_poses))
     rng = np.random.default_rng(seed)
     for _ in range(draws):
         bits = scene.poses_init.copy().view(np.int32) + rng.integers(-1, 2, size=scene.poses_init.shape).astype(np.int32)
@@ -74,6 +71,19 @@ def trajectory_spread(prob, scene, iters, o64_poses, draws, cfg_kw=None, seed=7)
         op.run(iters)
         runs.append(pose_errors(op.poses, o64_poses))
     return max(r[0] for r in runs), max(r[1] for r in runs), runs
+
+
+# Free-running rule (reading P7): the library's run may end no farther from the all-double oracle than the
+# contract's 1e-3 degrees / 1e-4 scene units, or -- where correct runs of this very loop end farther apart than that -- than
+# TWICE the farthest of the perturbed all-double runs above.  Why a factor at all: the draws and the library's run are
+# samples of one heavy-tailed quantity (a chaotic divergence), and a ninth sample exceeds the largest of eight with
+# probability 1/9 -- over the eight scenes of the suite a bare "no farther than the farthest" would fail a CORRECT
+# implementation about once.  Why 2: the draws of one scene spread over a factor 3 to 10 (recorded in DESIGN.md P7).
+SPREAD_FACTOR = 2.0
+
+
+def within_spread(rot, tr, srot, str_):
+    return rot <= max(1e-3, SPREAD_FACTOR * srot) and tr <= max(1e-4, SPREAD_FACTOR * str_)
 
 
 def oracle_eval(prob, poses, pairs, lam, z_min=Z_MIN):
@@ -113,6 +123,21 @@ def check_loss_grad(got, ref, sl, rtol_loss=1e-5, rtol_grad=1e-4, what=""):
         slack_rel_median=float(np.median(sl["cam"][live] / nrm[live])) if live.any() else 0.0,
         flagged_frac=float(sl["flagged"].sum() / max(int(rv.sum()), 1)))
     return rep
+
+
+def assert_slack_is_small(rep, what=""):
+    """Guards on the slack rule, set from what the B200 runs of round 3 show on all nine scenes (reading T1 has the
+    table; observed maxima in brackets):
+      - at most 0.2 % of the valid samples are flagged                        [0.14 %]
+      - at most 0.5 % of the pairs need any slack for their loss              [0.2 %]
+      - the median camera's slack is at most 5 % of its gradient scale        [3.3 %, orbit8 at lambda 6]
+      - the median camera's ERROR is at most 1e-4 + a tenth of the median slack [ratio error : slack 0.006 .. 0.043]: the
+        slack is a bound on what the flagged samples could move, and a correct kernel uses a small part of it -- a
+        systematic gradient error of a few 1e-3 relative fails here even where every camera has flagged samples."""
+    assert rep["flagged_frac"] <= 2e-3, (what, rep)
+    assert rep["pairs_needing_slack"] <= 5e-3, (what, rep)
+    assert rep["slack_rel_median"] <= 5e-2, (what, rep)
+    assert rep["grad_rel_median"] <= 1e-4 + 0.1 * rep["slack_rel_median"], (what, rep)
 
 
 def fmt_report(rep):

@@ -7,8 +7,8 @@ import pytest
 
 import oracle
 from epo_scenes import make_scene
-from parity_utils import (Z_MIN, check_loss_grad, fmt_lockstep, fmt_report, lockstep, make_ctx, oracle_config, oracle_eval,
-                          pose_errors, trajectory_spread)
+from parity_utils import (Z_MIN, assert_slack_is_small, check_loss_grad, fmt_lockstep, fmt_report, lockstep, make_ctx, oracle_config, oracle_eval,
+                          pose_errors, trajectory_spread, within_spread)
 
 pytestmark = pytest.mark.gpu
 
@@ -51,11 +51,12 @@ def test_full_size_loss_gradient_and_preprocessing(config):
         ref, sl = oracle_eval(prob, poses, sc.pairs, lam)
         rep = check_loss_grad(got, ref, sl, what=f"config {config} lam={lam}")
         print(f"config {config} full size lam={lam}: {len(sc.pairs)} pairs, {int(got['pair_valid'].sum())} valid samples; {fmt_report(rep)}")
-        assert rep["flagged_frac"] <= 1e-2 and rep["slack_rel_median"] <= 1e-1
-    # three lock-step iterations of the loop at full size
-    worst, _, n = lockstep(sc, e, 3, oracle_config(early_stop=0), prob=prob, label=f"config {config}")
-    assert n == 3
-    print(f"config {config} full size, 3 lock-step iterations: {fmt_lockstep(worst)}")
+        assert_slack_is_small(rep, what=f"config {config} lam={lam}")
+    # lock-step iterations of the loop at full size, through the 25-step warm-up (config 4: 10, the oracle needs ~4 s each)
+    n_lock = 10 if config == 4 else 30
+    worst, _, n = lockstep(sc, e, n_lock, oracle_config(early_stop=0), prob=prob, label=f"config {config}")
+    assert n == n_lock
+    print(f"config {config} full size, {n_lock} lock-step iterations: {fmt_lockstep(worst)}")
     e.destroy()
 
 
@@ -63,22 +64,25 @@ def test_full_size_loss_gradient_and_preprocessing(config):
 def test_full_size_free_running_prefix(config):
     """The first 25 iterations, free-running on both sides (no re-synchronisation), at full size, against the all-double
     oracle: final poses within the contract's 1e-3 degrees / 1e-4 scene units where correct evaluations of this loop can
-    meet that at all -- else within 3x their spread, measured on the oracle alone (parity_utils.trajectory_spread: the
-    binary32-position variant and all-double runs from initial poses moved by at most one binary32 ulp; one-step
-    differences of a few 1e-4 degrees, see the lock-step test above, are carried on over 25 steps; DESIGN.md reading P7);
-    the loss trace within 1e-4."""
+    meet that at all -- else within twice the farthest of FOUR all-double oracle runs from initial poses moved by at most
+    one binary32 ulp (parity_utils.within_spread; reading P7); the loss trace within 1e-4.  Config 2 (the room
+    layout whose oracle runs take seconds) is carried on to north_star's fixed 200 iterations under the same rule; at
+    config 4 the five oracle runs of 200 iterations would take ~40 minutes, so its 200-iteration point is not asserted."""
     sc, e, prob = _full(config, early_stop=0)
     opt = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0))
-    assert e.step(25)[0] == 25 and opt.run(25)[0] == 25
-    rot, tr = pose_errors(e.get_poses_f64(), opt.poses)
-    srot, str_, runs = trajectory_spread(prob, sc, 25, opt.poses, draws=1)
-    loss, _ = e.get_trace(0, 25)
-    lrel = float(np.max(np.abs(loss - opt.loss[:25]) / opt.loss[:25]))
-    print(f"config {config} full size, 25 free-running iterations vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e}, "
-          f"loss trace rel {lrel:.2e}; spread of the oracle's own runs (binary32-position variant, then one run from initial "
-          f"poses moved by <= 1 binary32 ulp): " + ", ".join(f"{a:.2e} / {b:.2e}" for a, b in runs))
-    assert rot <= max(1e-3, 3 * srot) and tr <= max(1e-4, 3 * str_)
-    assert lrel <= 1e-4
+    done = 0
+    for upto in ((25, 200) if config == 2 else (25,)):
+        assert e.step(upto - done)[0] == upto - done and opt.run(upto - done)[0] == upto - done
+        done = upto
+        rot, tr = pose_errors(e.get_poses_f64(), opt.poses)
+        srot, str_, runs = trajectory_spread(prob, sc, upto, opt.poses, draws=4)
+        loss, _ = e.get_trace(0, upto)
+        lrel = float(np.max(np.abs(loss[:25] - opt.loss[:25]) / opt.loss[:25]))
+        print(f"config {config} full size, {upto} free-running iterations vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e}, "
+              f"loss trace rel (first 25) {lrel:.2e}; 4 all-double runs from initial poses moved by <= 1 binary32 ulp: "
+              + ", ".join(f"{a:.2e} / {b:.2e}" for a, b in runs))
+        assert within_spread(rot, tr, srot, str_), (config, upto, rot, tr, srot, str_)
+        assert lrel <= 1e-4
     e.destroy()
 
 

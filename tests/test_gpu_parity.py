@@ -5,8 +5,8 @@ import pytest
 
 import oracle
 from epo_scenes import SplitMix64, make_scene
-from parity_utils import (Z_MIN, check_loss_grad, fmt_lockstep, fmt_report, lockstep, make_ctx, oracle_config, oracle_eval,
-                          pose_errors, trajectory_spread)
+from parity_utils import (Z_MIN, assert_slack_is_small, check_loss_grad, fmt_lockstep, fmt_report, lockstep, make_ctx, oracle_config, oracle_eval,
+                          pose_errors, trajectory_spread, within_spread)
 
 pytestmark = pytest.mark.gpu
 
@@ -97,6 +97,43 @@ def test_preprocessing_adversarial_inputs():
         e.destroy()
 
 
+def test_distance_transform_worst_case_is_bounded():
+    """The column pass searches outwards for as many rows as the distance itself: at the paper's edge densities a few
+    rows, on a view with no or one edge pixel up to H of them.  At the paper's frame size (518 x 392, 100 views) that
+    worst case stays exact and costs epo_set_views 4.8-4.9 ms against 1.7 ms on config 3's own edge maps (B200, round 3,
+    device-resident inputs): a factor 2.9, one-time.  Asserted: bit-exact fields (closed form) and less than 6x."""
+    import time
+    import torch
+    from paper_2607_00579_b200 import Epo, epo_config_default
+    N, W, H = 100, 518, 392
+    rng = np.random.default_rng(5)
+    typical = (rng.random((N, H, W)) < 0.03).astype(np.uint8)
+    empty = np.zeros((N, H, W), np.uint8)
+    one = np.zeros((N, H, W), np.uint8); one[:, 3, 5] = 1
+    K = np.tile(np.array([400.0, 400.0, W / 2, H / 2], np.float32), (N, 1))
+    poses = np.tile(np.eye(4, dtype=np.float32)[:3].reshape(1, 12), (N, 1))
+    dK, dP, dD = torch.from_numpy(K).cuda(), torch.from_numpy(poses).cuda(), torch.ones((N, H, W), device="cuda")
+    e = Epo(epo_config_default(n_views=N, width=W, height=H, stream=torch.cuda.current_stream().cuda_stream))
+
+    def timed(edges):
+        d = torch.from_numpy(edges).cuda()
+        best = 1e9
+        for _ in range(3):
+            torch.cuda.synchronize(); t0 = time.perf_counter(); e.set_views(dK, dP, dD, d); torch.cuda.synchronize()
+            best = min(best, time.perf_counter() - t0)
+        return best
+
+    t_typ = timed(typical)
+    t_empty = timed(empty)
+    assert np.all(e.get_dtf(N - 1) == W + H)
+    t_one = timed(one)
+    yy, xx = np.mgrid[0:H, 0:W]
+    assert np.array_equal(e.get_dtf(7), np.sqrt(((yy - 3) ** 2 + (xx - 5) ** 2).astype(np.float64)).astype(np.float32))
+    print(f"epo_set_views, 100 views of 518x392: 3 % edge density {1e3 * t_typ:.2f} ms, no edge {1e3 * t_empty:.2f} ms, one edge pixel {1e3 * t_one:.2f} ms")
+    assert t_empty <= 6 * t_typ and t_one <= 6 * t_typ
+    e.destroy()
+
+
 def test_fp16_field_is_rne_of_fp32_field():
     sc = scene("room5_294")
     e = make_ctx(sc, dtf_format=1)
@@ -125,7 +162,7 @@ def test_loss_and_gradient_parity(name, lam):
     print(f"{name} lam={lam}: {fmt_report(rep)}  [diagnostic, binary32-position variant: valid counts "
           f"{'equal' if np.array_equal(got['pair_valid'], d32['pair_valid']) else 'differ'}, camera grad rel err {g32:.1e}]")
     # the slack must stay what it is meant to be: a few flagged samples, not a licence
-    assert rep["flagged_frac"] <= 1e-2 and rep["slack_rel_median"] <= 1e-1
+    assert_slack_is_small(rep, what=f"{name} lam={lam}")
     # the evaluation must not move the state
     again = e.loss_grad(lam)
     assert again["loss"] == got["loss"] and np.array_equal(again["grad"], got["grad"])
@@ -281,32 +318,29 @@ def test_fixed_200_iterations_free_running_tiny():
 
 @pytest.mark.parametrize("name,iters,prefix", [("room6", 200, 25), ("orbit8", 100, 25), ("room5_294", 200, 25), ("orbit10_dense", 100, 25)])
 def test_free_running_trajectories(name, iters, prefix):
-    """Free-running runs against the all-double oracle.  Asserted: after the first 25 iterations (the warm-up, while the
-    trajectories still contract) the poses agree within the contract's 1e-3 degrees / 1e-4 -- or, on scenes where correct
-    evaluations of this very loop end farther apart than that, within 3x their spread, measured on the oracle alone
-    (parity_utils.trajectory_spread: its binary32-position variant and all-double runs from initial poses moved by at most
-    one binary32 ulp; reading P7 records the numbers).  Beyond the prefix the runs decorrelate (see
-    parity_utils.lockstep: gradient jumps at cell borders, Adam stepping by ~lr), so the end-of-run distance is a chaotic
-    quantity: it is PRINTED next to the distance between the oracle's own two variants, and only the final loss is
-    asserted."""
+    """Free-running runs against the all-double oracle, asserted at TWO points: after the first 25 iterations (the
+    warm-up) and at the end (200 iterations on the room layouts -- north_star's "fixed 200 iterations" --, 100 on the
+    orbits).  At both the poses agree within the contract's 1e-3 degrees / 1e-4, or, on scenes where correct evaluations
+    of this very loop end farther apart than that, within twice the farthest of EIGHT all-double oracle runs from initial
+    poses moved by at most one binary32 ulp (parity_utils.within_spread; reading P7 records the numbers).  No
+    kernel-shaped code is in the bound: the oracle's binary32-position variant is printed as a diagnostic only."""
     sc = scene(name)
     e = make_ctx(sc, early_stop=0)
     prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=Z_MIN)
     o64 = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0, coord_fp32=0))
     o32 = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0, coord_fp32=1))
-    e.step(prefix); o64.run(prefix); o32.run(prefix)
-    rot, tr = pose_errors(e.get_poses_f64(), o64.poses)
-    srot, str_, runs = trajectory_spread(prob, sc, prefix, o64.poses, draws=4)
-    print(f"{name}: after {prefix} free-running its vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e}; spread of the "
-          f"oracle's own runs (binary32-position variant, then 4 runs from initial poses moved by <= 1 binary32 ulp): "
-          + ", ".join(f"{a:.2e} / {b:.2e}" for a, b in runs))
-    assert rot <= max(1e-3, 3 * srot) and tr <= max(1e-4, 3 * str_)
-    rest = iters - prefix
-    e.step(rest); o64.run(rest); o32.run(rest)
-    d_go = pose_errors(e.get_poses_f64(), o64.poses); d_oo = pose_errors(o32.poses, o64.poses)
+    done = 0
+    for upto in (prefix, iters):
+        e.step(upto - done); o64.run(upto - done); o32.run(upto - done); done = upto
+        rot, tr = pose_errors(e.get_poses_f64(), o64.poses)
+        srot, str_, runs = trajectory_spread(prob, sc, upto, o64.poses, draws=8)
+        d32 = pose_errors(o32.poses, o64.poses)
+        print(f"{name}: after {upto} free-running its vs the all-double oracle: rot {rot:.2e} deg, trans {tr:.2e}; 8 all-double runs "
+              f"from initial poses moved by <= 1 binary32 ulp: " + ", ".join(f"{a:.2e} / {b:.2e}" for a, b in runs)
+              + f" [diagnostic, binary32-position variant: {d32[0]:.2e} / {d32[1]:.2e}]")
+        assert within_spread(rot, tr, srot, str_), (name, upto, rot, tr, srot, str_)
     loss, _ = e.get_trace(0, iters)
-    print(f"{name}: after {iters} its: GPU vs all-double oracle rot {d_go[0]:.2e} deg trans {d_go[1]:.2e}; oracle binary32-position "
-          f"variant vs all-double oracle rot {d_oo[0]:.2e} trans {d_oo[1]:.2e}; final loss {loss[-1]:.6f} vs {o64.loss[iters - 1]:.6f}")
+    print(f"{name}: final loss {loss[-1]:.6f} vs {o64.loss[iters - 1]:.6f}")
     assert abs(loss[-1] - o64.loss[iters - 1]) <= 2e-2 * o64.loss[iters - 1]
     e.destroy()
 

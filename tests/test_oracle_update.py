@@ -233,10 +233,10 @@ def test_Z12_adamw_matches_torch_optim_adamw_and_decays_towards_the_identity():
 
 def test_P7_trajectory_spread_of_the_oracle_alone():
     """DESIGN.md reading P7: how far correct evaluations of the same free-running loop end apart, measured on the oracle
-    alone (parity_utils.trajectory_spread).  On Tiny (noise-free, 4 views) the binary32-position variant and all-double
-    runs from initial poses moved by <= 1 binary32 ulp all stay within the contract (1e-3 degrees, 1e-4) of the
-    all-double run after 25 iterations -- which is why the contract is asserted free-running there --, the spread is
-    not zero (the runs do differ), and the same seed gives the same draws."""
+    alone (parity_utils.trajectory_spread).  On Tiny (noise-free, 4 views) all-double runs from initial poses moved by
+    <= 1 binary32 ulp all stay within the contract (1e-3 degrees, 1e-4) of the all-double run after 25 iterations --
+    which is why the contract is asserted free-running there --, the spread is not zero (the runs do differ), and the
+    same seed gives the same draws."""
     from epo_scenes import make_scene
     from parity_utils import Z_MIN, oracle_config, trajectory_spread
     sc = make_scene(1)
@@ -244,6 +244,6 @@ def test_P7_trajectory_spread_of_the_oracle_alone():
     o64 = oracle.Optimizer(prob, sc.poses_init, sc.pairs, oracle_config(early_stop=0))
     o64.run(25)
     rot, tr, runs = trajectory_spread(prob, sc, 25, o64.poses, draws=2)
-    assert len(runs) == 3 and 0.0 < rot <= 1e-3 and 0.0 < tr <= 1e-4
+    assert len(runs) == 2 and 0.0 < rot <= 1e-3 and 0.0 < tr <= 1e-4
     rot2, tr2, _ = trajectory_spread(prob, sc, 25, o64.poses, draws=2)
     assert (rot, tr) == (rot2, tr2)
