@@ -221,6 +221,25 @@ EPO_API epo_status epo_get_poses_f64(epo_ctx* ctx, double* poses);
  * moments, step counter, phase and traces.  Preprocessing and pair lists are kept. */
 EPO_API epo_status epo_reset(epo_ctx* ctx, const float* poses);
 
+/*
+ * Checkpoint / resume of the optimisation (Alg. 2: everything the loop carries from one iteration to the
+ * next).  The blob holds the current poses (fp64), the Adam moments, the step counter, phase and stop flags, the theta95
+ * and loss traces, and -- cfg.joint_phase = 1 -- gamma, alpha, beta with their AdamW moments, the current intrinsics and
+ * points.  It does NOT hold views, distance fields or pair lists: restore into a context that was given the SAME
+ * epo_config, epo_set_views and epo_set_pairs inputs (sizes are checked -- views, resolution, max_steps, joint_phase, pair
+ * and edge-pixel counts --, contents are the caller's responsibility).  After epo_set_state the context continues exactly
+ * where the exporting one stood: the following iterations are bit-identical to those the exporter would have run.
+ *   epo_get_state_size  bytes [1] out (host)
+ *   epo_get_state       blob: host or device pointer, capacity >= that size (else EPO_ERR_INVALID_ARG)
+ *   epo_set_state       blob as written by epo_get_state of this library version; a blob from another problem or
+ *                       configuration is refused with EPO_ERR_INVALID_ARG and the context is left unchanged
+ * Both copy on cfg.stream and synchronise it.  The layout is private to the library version (header-checked), native
+ * endianness; not an interchange format.
+ */
+EPO_API epo_status epo_get_state_size(epo_ctx* ctx, int64_t* bytes);
+EPO_API epo_status epo_get_state(epo_ctx* ctx, void* blob, int64_t capacity);
+EPO_API epo_status epo_set_state(epo_ctx* ctx, const void* blob, int64_t bytes);
+
 /* Joint-phase variables (cfg.joint_phase = 1), all nullable, host or device pointers, fp64: gamma [N]; alpha and beta
  * as [N][H][W] maps (1 and 0 off the edge lists).  The current intrinsics are K0 (1 + gamma), the current depth of a
  * listed edge pixel is Z0 alpha + beta. */

@@ -24,7 +24,7 @@ _STATUS = {0: "EPO_OK", 1: "EPO_ERR_INVALID_ARG", 2: "EPO_ERR_BAD_STATE", 3: "EP
 SYMBOLS = ["epo_config_default", "epo_create", "epo_destroy", "epo_extract_edges", "epo_extract_edges_rgb", "epo_set_views", "epo_build_viewgraph", "epo_set_pairs", "epo_loss_grad", "epo_loss_grad_joint", "epo_get_joint_variables",
            "epo_step", "epo_get_poses", "epo_get_poses_f64", "epo_reset", "epo_get_edge_counts", "epo_get_edge_list",
            "epo_get_dtf", "epo_get_pair_order", "epo_get_trace", "epo_get_work", "epo_get_pair_subset", "epo_time_loss_grad_kernel", "epo_time_gather_ceiling",
-           "epo_edt_no_alloc", "epo_last_error", "epo_version"]
+           "epo_edt_no_alloc", "epo_get_state_size", "epo_get_state", "epo_set_state", "epo_last_error", "epo_version"]
 
 
 class EpoConfig(C.Structure):
@@ -77,6 +77,9 @@ def load_library() -> C.CDLL:
     L.epo_time_loss_grad_kernel.argtypes = [vp, C.c_float, C.c_int32, C.c_int32, C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.epo_time_gather_ceiling.argtypes = L.epo_time_loss_grad_kernel.argtypes
     L.epo_edt_no_alloc.argtypes = [vp, C.c_int32, C.c_int32, vp, vp, C.c_char_p, C.c_int32]
+    L.epo_get_state_size.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.epo_get_state.argtypes = [vp, vp, C.c_int64]
+    L.epo_set_state.argtypes = [vp, vp, C.c_int64]
     L.epo_last_error.argtypes = [vp]; L.epo_last_error.restype = C.c_char_p
     L.epo_version.argtypes = []; L.epo_version.restype = C.c_char_p
     return L
@@ -246,6 +249,19 @@ class Epo:
 
     def reset(self, poses=None):
         self._check(lib().epo_reset(self._h, _ptr(poses, np.float32)), "epo_reset")
+
+    def get_state(self):
+        """The optimiser state as a uint8 numpy array (epo_get_state): restore with set_state into a context with the same
+        configuration, views and pairs."""
+        n = C.c_int64(0)
+        self._check(lib().epo_get_state_size(self._h, C.byref(n)), "epo_get_state_size")
+        blob = np.zeros(n.value, np.uint8)
+        self._check(lib().epo_get_state(self._h, _ptr(blob), n.value), "epo_get_state")
+        return blob
+
+    def set_state(self, blob):
+        self._check(lib().epo_set_state(self._h, _ptr(blob), int(blob.size if isinstance(blob, np.ndarray) else blob.numel())),
+                    "epo_set_state")
 
     def get_edge_counts(self):
         off = np.zeros(self.N + 1, np.int32)

@@ -8,6 +8,8 @@
 #include <cstring>
 #include <new>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "epo_internal.h"
 
 epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...) {
@@ -21,6 +23,15 @@ epo_status epo_fail(epo_ctx* ctx, epo_status st, const char* fmt, ...) {
 }
 
 namespace {
+
+// NVTX range around a phase of the public API: shows up as "epo: <call>" on the timeline of a
+// profiler that injects NVTX (Nsight Systems / Compute); without one nvtxRangePush is a null function-pointer check.
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+  NvtxRange(const NvtxRange&) = delete;
+  NvtxRange& operator=(const NvtxRange&) = delete;
+};
 
 bool is_device_ptr(const void* p) {
   cudaPointerAttributes a;
@@ -334,6 +345,7 @@ void epo_destroy(epo_ctx* c) {
 
 epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const float* depth, const uint8_t* edges) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_set_views");
   if (!K || !poses || !depth || !edges) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_views: NULL argument");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
@@ -425,6 +437,7 @@ epo_status epo_set_views(epo_ctx* c, const float* K, const float* poses, const f
 
 epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_set_pairs");
   if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_set_pairs before epo_set_views");
   if (!pairs || P <= 0 || P > (int64_t)1 << 30) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_pairs: NULL list or bad count");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
@@ -520,6 +533,7 @@ epo_status epo_set_pairs(epo_ctx* c, const int32_t* pairs, int64_t P) {
 
 epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss, int32_t* pair_valid, float* grad) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_loss_grad");
   if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_loss_grad before epo_set_views/epo_set_pairs");
   if (!loss || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_loss_grad: NULL loss or negative lambda");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
@@ -553,6 +567,7 @@ epo_status epo_loss_grad(epo_ctx* c, float lambda, float* loss, float* pair_loss
 
 epo_status epo_loss_grad_joint(epo_ctx* c, float lambda, float* loss, float* g_logf, float* g_depth) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_loss_grad_joint");
   if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_loss_grad_joint before epo_set_views/epo_set_pairs");
   if (!g_logf || !g_depth || !(lambda >= 0.f)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_loss_grad_joint: NULL output or negative lambda");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
@@ -624,6 +639,7 @@ epo_status epo_get_joint_variables(epo_ctx* c, double* gamma, double* alpha, dou
 
 epo_status epo_step(epo_ctx* c, int32_t n_iters, int32_t* iters_done, int32_t* phase) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_step");
   if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_step before epo_set_views/epo_set_pairs");
   if (n_iters < 0) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_step: negative iteration count");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
@@ -681,6 +697,7 @@ epo_status epo_get_poses_f64(epo_ctx* c, double* poses) {
 
 epo_status epo_get_poses(epo_ctx* c, float* poses) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_get_poses");
   if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_poses before epo_set_views");
   if (!poses) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_poses: NULL output");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
@@ -705,6 +722,7 @@ epo_status epo_get_poses(epo_ctx* c, float* poses) {
 
 epo_status epo_reset(epo_ctx* c, const float* poses) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_reset");
   if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_reset before epo_set_views");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
   cudaStream_t st = c->stream;
@@ -817,6 +835,7 @@ epo_status epo_get_trace(epo_ctx* c, int32_t first, int32_t count, float* loss, 
 
 epo_status epo_extract_edges(epo_ctx* c, const uint8_t* images, int32_t low, int32_t high, uint8_t* edges) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_extract_edges");
   if (!images || !edges || low < 0 || high < low || high > 1442)    // |g| <= 1020 sqrt(2)
     return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_extract_edges: bad argument");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
@@ -841,6 +860,7 @@ epo_status epo_extract_edges(epo_ctx* c, const uint8_t* images, int32_t low, int
 
 epo_status epo_extract_edges_rgb(epo_ctx* c, const uint8_t* rgb, int32_t low, int32_t high, uint8_t* edges) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_extract_edges_rgb");
   if (!rgb || !edges || low < 0 || high < low || high > 1442)
     return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_extract_edges_rgb: bad argument");
   EPO_CUDA(c, cudaSetDevice(c->cfg.device));
@@ -861,6 +881,7 @@ epo_status epo_extract_edges_rgb(epo_ctx* c, const uint8_t* rgb, int32_t low, in
 epo_status epo_build_viewgraph(epo_ctx* c, int32_t grid_stride, float tau, float min_frac, int32_t* pairs, int64_t capacity,
                                int64_t* n_pairs, int32_t* counts) {
   if (!c) return EPO_ERR_INVALID_ARG;
+  NvtxRange nvtx_("epo: epo_build_viewgraph");
   if (!c->have_views) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_build_viewgraph before epo_set_views");
   if (!n_pairs || grid_stride < 1 || !(tau > 0.f) || !(min_frac >= 0.f && min_frac <= 1.f) || capacity < 0 || (capacity > 0 && !pairs))
     return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_build_viewgraph: bad argument");
@@ -980,6 +1001,108 @@ static epo_status time_fused(epo_ctx* c, float lambda, int32_t reps, int32_t flu
   if (e != cudaSuccess) return epo_fail(c, e == cudaErrorMemoryAllocation ? EPO_ERR_OUT_OF_MEMORY : EPO_ERR_CUDA, "epo_time_loss_grad_kernel: %s", cudaGetErrorString(e));
   if (ms_mean) *ms_mean = (float)(sum / reps);
   if (ms_min) *ms_min = mn;
+  return EPO_OK;
+}
+
+// ---- optimiser state export / import (SURVEY.md section 5 "checkpoint / resume") -----------------------------------------
+// Everything epo_step changes, as one flat blob: header | poses | Adam m | Adam v | DevState | theta trace | loss trace
+// [ | gamma + AdamW moments | K | depth_stepped | (alpha, beta) | their moments | packed points ]  (joint contexts).
+// Views, fields, pair lists and work lists are NOT in it: they are functions of the inputs the caller still has.
+namespace {
+struct StateHeader {
+  uint64_t magic;                 // "EPOSTATE"
+  int32_t version, n_views, width, height, max_steps, joint;
+  int64_t n_pairs, n_edges, n_slots, bytes;
+};
+constexpr uint64_t kStateMagic = 0x4554415453'4f5045ull;   // 'E' 'P' 'O' 'S' 'T' 'A' 'T' 'E' little-endian
+struct StateSeg { void* p; size_t bytes; };
+
+size_t state_align(size_t b) { return (b + 15) & ~(size_t)15; }
+
+std::vector<StateSeg> state_segments(epo_ctx* c) {
+  const size_t N = (size_t)c->N, T = (size_t)c->cfg.max_steps;
+  std::vector<StateSeg> v = {{c->d_poses, N * 12 * sizeof(double)}, {c->d_m, N * 6 * sizeof(double)}, {c->d_v, N * 6 * sizeof(double)},
+                             {c->d_state, sizeof(DevState)}, {c->d_theta, T * sizeof(double)}, {c->d_loss_trace, T * sizeof(double)}};
+  if (c->cfg.joint_phase) {
+    const size_t S = c->packed.h_off.empty() ? 0 : (size_t)c->packed.h_off[c->N] / 2;
+    v.push_back({c->d_gamma, 3 * N * sizeof(double)});
+    v.push_back({c->d_K, N * 4 * sizeof(float)});
+    v.push_back({c->d_depth_stepped, sizeof(int32_t)});
+    if (S > 0) {
+      v.push_back({c->d_ab, S * sizeof(double4)});
+      v.push_back({c->d_abm, 2 * S * sizeof(float4)});
+      v.push_back({c->packed.xyz, S * 3 * sizeof(float2)});
+    }
+  }
+  return v;
+}
+
+StateHeader state_header(epo_ctx* c) {
+  StateHeader h = {};
+  h.magic = kStateMagic; h.version = 1; h.n_views = c->N; h.width = c->W; h.height = c->H; h.max_steps = c->cfg.max_steps;
+  h.joint = c->cfg.joint_phase; h.n_pairs = c->P; h.n_edges = c->E;
+  h.n_slots = c->packed.h_off.empty() ? 0 : (int64_t)c->packed.h_off[c->N] / 2;
+  size_t b = state_align(sizeof(StateHeader));
+  for (const StateSeg& sg : state_segments(c)) b += state_align(sg.bytes);
+  h.bytes = (int64_t)b;
+  return h;
+}
+}  // namespace
+
+epo_status epo_get_state_size(epo_ctx* c, int64_t* bytes) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!bytes) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_state_size: NULL output");
+  if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_state_size before epo_set_views/epo_set_pairs");
+  *bytes = state_header(c).bytes;
+  return EPO_OK;
+}
+
+epo_status epo_get_state(epo_ctx* c, void* blob, int64_t capacity) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_get_state before epo_set_views/epo_set_pairs");
+  const StateHeader h = state_header(c);
+  if (!blob || capacity < h.bytes) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_get_state: need %lld bytes, got %lld", (long long)h.bytes, (long long)capacity);
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  char* out = static_cast<char*>(blob);
+  EPO_CUDA(c, cudaMemcpyAsync(out, &h, sizeof(h), cudaMemcpyDefault, st));
+  size_t off = state_align(sizeof(StateHeader));
+  for (const StateSeg& sg : state_segments(c)) {
+    EPO_CUDA(c, cudaMemcpyAsync(out + off, sg.p, sg.bytes, cudaMemcpyDefault, st));
+    off += state_align(sg.bytes);
+  }
+  EPO_CUDA(c, cudaStreamSynchronize(st));              // the header is copied from this frame
+  return EPO_OK;
+}
+
+epo_status epo_set_state(epo_ctx* c, const void* blob, int64_t bytes) {
+  if (!c) return EPO_ERR_INVALID_ARG;
+  if (!c->have_views || !c->have_pairs) return epo_fail(c, EPO_ERR_BAD_STATE, "epo_set_state before epo_set_views/epo_set_pairs");
+  if (!blob || bytes < (int64_t)sizeof(StateHeader)) return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_state: blob too short");
+  EPO_CUDA(c, cudaSetDevice(c->cfg.device));
+  cudaStream_t st = c->stream;
+  StateHeader got;
+  EPO_CUDA(c, cudaMemcpyAsync(&got, blob, sizeof(got), cudaMemcpyDefault, st));
+  EPO_CUDA(c, cudaStreamSynchronize(st));
+  const StateHeader want = state_header(c);
+  if (got.magic != kStateMagic || got.version != want.version)
+    return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_state: not a state blob of this library version");
+  if (got.n_views != want.n_views || got.width != want.width || got.height != want.height || got.max_steps != want.max_steps ||
+      got.joint != want.joint || got.n_pairs != want.n_pairs || got.n_edges != want.n_edges || got.n_slots != want.n_slots ||
+      got.bytes != want.bytes || bytes < want.bytes)
+    return epo_fail(c, EPO_ERR_INVALID_ARG, "epo_set_state: the blob was taken from a different problem or configuration "
+                    "(views %d/%d, %dx%d/%dx%d, max_steps %d/%d, joint %d/%d, pairs %lld/%lld, edge pixels %lld/%lld, bytes %lld/%lld)",
+                    got.n_views, want.n_views, got.width, got.height, want.width, want.height, got.max_steps, want.max_steps,
+                    got.joint, want.joint, (long long)got.n_pairs, (long long)want.n_pairs, (long long)got.n_edges,
+                    (long long)want.n_edges, (long long)got.bytes, (long long)want.bytes);
+  const char* in = static_cast<const char*>(blob);
+  size_t off = state_align(sizeof(StateHeader));
+  for (const StateSeg& sg : state_segments(c)) {
+    EPO_CUDA(c, cudaMemcpyAsync(sg.p, in + off, sg.bytes, cudaMemcpyDefault, st));
+    off += state_align(sg.bytes);
+  }
+  c->static_dirty = true;                               // K / points may have changed under the next fused launch
+  EPO_CUDA(c, cudaStreamSynchronize(st));              // the caller may free the blob on return
   return EPO_OK;
 }
 

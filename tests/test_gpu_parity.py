@@ -959,6 +959,46 @@ def test_loop_is_bit_reproducible(kw):
             assert np.array_equal(a, b)
 
 
+@pytest.mark.parametrize("kw", [dict(), dict(pair_budget=7, subsample_seed=11), dict(joint_phase=1, w1=6, eps1=5.0),
+                                dict(stop_rule=1, w1=4, eps1=5.0, w_loss=16, eps_loss=0.5, early_stop=1)],
+                         ids=["poses", "subsampled", "joint", "early-stop"])
+def test_state_export_and_import_resume_bit_exactly(kw):
+    """epo_get_state / epo_set_state: a second context with the same inputs, given the blob, runs the SAME following
+    iterations as the exporter -- poses, traces, phase, joint variables bit for bit --, as does the exporter itself when
+    rewound to the blob; a blob of another problem is refused and changes nothing."""
+    sc = scene("orbit8")
+    kw = dict(dict(early_stop=0), **kw)
+    a = make_ctx(sc, **kw)
+    n1 = a.step(12)[0]
+    blob = a.get_state()
+    done_a, phase_a = a.step(13)                                     # 8 iterations in the loop graph + 5 enqueued one by one
+    total = n1 + done_a
+    want = (a.get_poses_f64(),) + a.get_trace(0, total) + (a.get_joint_variables() if kw.get("joint_phase") else ())
+    b = make_ctx(sc, **kw)
+    b.set_state(blob)
+    assert np.array_equal(b.get_state(), blob)
+    for ctx in (b, a):                                               # a fresh context, then the exporter rewound
+        if ctx is a:
+            a.set_state(blob)
+        assert ctx.step(13) == (done_a, phase_a)
+        got = (ctx.get_poses_f64(),) + ctx.get_trace(0, total) + (ctx.get_joint_variables() if kw.get("joint_phase") else ())
+        for x, y in zip(want, got):
+            if isinstance(x, tuple):
+                assert all(np.array_equal(p, q) for p, q in zip(x, y))
+            else:
+                assert np.array_equal(x, y)
+    if kw.get("joint_phase"):
+        assert np.abs(want[4] - 1.0).max() > 0                       # the depth variables (alpha) were part of what was carried over
+    if kw.get("early_stop"):
+        assert n1 == 12 and phase_a == 2 and done_a < 13             # the stop came after the export: the loss window was carried over
+    other = make_ctx(scene("room6"), **kw)
+    before = other.get_state()
+    with pytest.raises(Exception) as ei:
+        other.set_state(blob)
+    assert getattr(ei.value, "status", None) == 1 and np.array_equal(other.get_state(), before)   # EPO_ERR_INVALID_ARG
+    a.destroy(); b.destroy(); other.destroy()
+
+
 def test_step_in_pieces_equals_one_call():
     sc = scene("tiny")
     a = make_ctx(sc, early_stop=0); b = make_ctx(sc, early_stop=0)
