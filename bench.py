@@ -197,7 +197,13 @@ def cpu_baseline(sc, seconds_target=9.0):
 
 def run_reference(args, sc):
     """--impl reference: K timed steps of the oracle (one iteration of Alg. 2 each) on the host cores."""
+    # Same process environment as the cpu_baseline leg of the main arm, which runs after `import torch`: torch loads its own
+    # OpenMP runtime first and the oracle's parallel loops then run on that one -- measured 1.45x faster than on the
+    # system libgomp alone (8 cores, config 2: 102 against 152 ms per iteration).  Round 2's two legs differed by exactly
+    # this (124 against 185 M reprojections/s on the same box); the thread count is set explicitly in both.
+    import torch  # noqa: F401
     import oracle
+    oracle.set_num_threads(len(os.sched_getaffinity(0)))
     prob = oracle.preprocess(sc.K, sc.depth, sc.edges, z_min=float(np.float32(1e-6)))
     reproj = int(sum(prob.edge_off[s + 1] - prob.edge_off[s] for s, _ in sc.pairs))
     # bound the run to a few minutes: each step is a sample of `frac` of the pairs (whole pairs, list order)
@@ -211,8 +217,7 @@ def run_reference(args, sc):
     pairs = sc.pairs[:n_pairs]
     r_step = int(sum(prob.edge_off[s + 1] - prob.edge_off[s] for s, _ in pairs))
     opt = oracle.Optimizer(prob, sc.poses_init, pairs, oracle_cfg_like_library())
-    # untimed: the requested warm-up steps, and at least ~2 s of iterations so that the OpenMP pool is up and the fields
-    # are in the host caches (a cold pool made this arm read 1.5x slower than bench.py's own cpu_baseline leg in round 2)
+    # untimed: the requested warm-up steps, and at least ~2 s of iterations (thread pool up, fields in the host caches)
     opt.run(args.warmup)
     t0 = time.time(); extra = 0
     while time.time() - t0 < 2.0 and extra < 50:
@@ -392,11 +397,24 @@ def main():
             torch.cuda.synchronize(); times.append(time.perf_counter() - t0)
             e2.destroy()
         t_e2e = float(np.median(times))                                # the median of ALL repetitions, first ones included
+        # where the time goes: ONE extra run, not part of the number above, with a device synchronisation after every call
+        # (so the phases cannot overlap and their sum may exceed `seconds`)
+        bd = {}
+        def lap(name, fn):
+            t = time.perf_counter(); r = fn(); torch.cuda.synchronize(); bd[name] = round(time.perf_counter() - t, 6); return r
+        torch.cuda.synchronize()
+        e3 = lap("epo_create", lambda: Epo(cfg))
+        lap("epo_set_views (H2D of K, poses, depth, edges + edge lists + EDT + points)", lambda: e3.set_views(hK, hP, hD, hE))
+        lap("epo_set_pairs (H2D + sort + work list + host validation)", lambda: e3.set_pairs(hpairs))
+        lap(f"epo_step({args.refine_iters}) (graph build on this first call + the loop)", lambda: e3.step(args.refine_iters))
+        lap("epo_get_poses (D2H)", lambda: e3.get_poses(hout))
+        lap("epo_destroy", lambda: e3.destroy())
         h2d = sum(int(x.numel() * x.element_size()) for x in (hK, hP, hD, hE, hpairs))
         d2h = int(hout.numel() * 4) + 8
         e2e = dict(value=world * reproj_eff * args.refine_iters / t_e2e, unit=UNIT,
                    h2d_bytes_per_step=h2d / args.refine_iters, d2h_bytes_per_step=d2h / args.refine_iters,
                    h2d_bytes_per_run=h2d, d2h_bytes_per_run=d2h, seconds=t_e2e, seconds_all_repetitions=[round(t, 6) for t in times],
+                   breakdown_s=bd,
                    what=f"one run = epo_create + epo_set_views(host) + epo_set_pairs(host) + epo_step({args.refine_iters}) + "
                         f"epo_get_poses(host); a step = one of its {args.refine_iters} iterations; median of {len(times)} runs")
 
